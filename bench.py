@@ -1,0 +1,388 @@
+#!/usr/bin/env python
+"""bench.py -- coarse multi-RHS matvec + block-CG hot path on B200 (arXiv:2409.03904), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--nrhs S] [--config I]
+
+A STEP is one pass of the whole hot path over one block of Nrhs synthetic
+vectors: one BlockCGrQ iteration = stencil-GEMM apply Z = H D, Gram D^H Z, s x s algebra, the four block
+rotations and the Gram T^H T (Fig. 2 left, statements 8-13), driven through the C ABI
+(block_cg_begin / block_cg_step / block_cg_end).  Workload: BASELINE.json configs[3] -- the configuration
+the metric "TFLOP/s & roofline fraction vs Nrhs" is quoted on (12^3 x 24 coarse lattice, 81-point stencil,
+nbasis 32, complex64, ~27.5 GB of stencil matrices) -- at Nrhs = 16 unless --nrhs is given; the Nrhs sweep
+1,4,8,16,32,64 of the apply kernel is reported under "sweep".  Inputs are seeded and synthetic
+(DESIGN.md "Synthetic inputs"), resident in HBM before the timed region; the 27.5 GB operator is far larger
+than L2, so no L2 flush is needed between iterations.
+
+value      = algorithmic FLOP of K steps / device time (CUDA events, max over ranks), whole job, TFLOP/s
+e2e        = same metric through block_cg_solve_host: pinned HOST buffers for B and X, H2D/D2H inside the timed region
+roofline   = the dominant kernel (the stencil-GEMM apply) timed live with CUDA event pairs on its launch stream
+cpu_baseline / --impl reference = the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from inputs import synth  # noqa: E402
+
+METRIC = "coarse multi-RHS matvec TFLOP/s & roofline fraction vs Nrhs; block-CG solve s"      # BASELINE.json "metric"
+METRIC_NOTE = ("value = algorithmic FLOP (8 per complex MAC) of one BlockCGrQ iteration (apply + 2 Gram + 4 rotations) / time; "
+               "per-Nrhs apply TFLOP/s and roofline fractions under 'sweep'; solve seconds under 'block_cg_solve'")
+UNIT = "TFLOP/s"
+SM_COUNT, FP32_LANES, FP64_LANES = 148, 128, 64      # B200: guide's unit counts (blackwell_cuda_programming.md)
+SWEEP = (1, 4, 8, 16, 32, 64)
+
+
+# ---- algorithmic work (SURVEY.md section 8 / DESIGN.md "Algorithmic work") -----------------------------------
+def apply_flops(V, nb, s):
+    return 8.0 * 81 * V * nb * nb * s
+
+
+def apply_bytes(V, nb, s, esize):
+    return float(esize) * (81.0 * V * nb * nb + 2.0 * V * nb * s)          # A once, X once, Y once
+
+
+def linalg_flops(V, nb, s):
+    return 6.0 * 8.0 * V * nb * s * s                                        # 2 Gram products + 4 block rotations
+
+
+def step_flops(V, nb, s):
+    return apply_flops(V, nb, s) + linalg_flops(V, nb, s)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")        # B200_PROFILING.md fallback
+
+
+def alu_peak_tflops(dtype, sm_mhz):
+    lanes = FP32_LANES if dtype == "c64" else FP64_LANES
+    return SM_COUNT * lanes * 2.0 * sm_mhz * 1e6 / 1e12
+
+
+def roofline_tflops(V, nb, s, dtype, peaks):
+    esize = 8 if dtype == "c64" else 16
+    intensity = apply_flops(V, nb, s) / apply_bytes(V, nb, s, esize)
+    hbm = intensity * peaks["hbm_gbs"] / 1e3
+    alu = alu_peak_tflops(dtype, peaks["sm_max_mhz"])
+    return dict(intensity=intensity, hbm_tflops=hbm, alu_tflops=alu, roof_tflops=min(hbm, alu),
+                bound="hbm" if hbm <= alu else "alu")
+
+
+# ---- clocks during the timed region (B200_PROFILING.md "clocks line") ----------------------------------------
+class ClockSampler:
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu, self.proc, self.path = gpu_index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ---- the CPU oracle on a bounded sample of the same workload ---------------------------------------------------
+def oracle_sample_step(dims, nb, s, sites, A_s, X_full, K_small):
+    """One 'step' of the oracle restricted to the sampled sites: apply on those sites (needs the whole X block for
+    the neighbours), the two Gram products and the four block rotations on those sites' rows.  Returns seconds."""
+    from oracle import oracle
+    t0 = time.perf_counter()
+    Z = oracle.apply(dims, A_s, X_full, sites=sites)                      # a2
+    D = X_full[sites]
+    G = oracle.gram(D, Z)                                                  # a3
+    W = oracle.block_rotate(D, K_small, D, 1.0)                            # a5 (x4)
+    T = oracle.block_rotate(Z, K_small, D, 1.0)
+    G2 = oracle.gram(T, T)
+    Q = oracle.block_rotate(T, K_small, T, 0.0)
+    D2 = oracle.block_rotate(D, K_small, Q, 1.0)
+    dt = time.perf_counter() - t0
+    assert np.isfinite(G).all() and np.isfinite(G2).all() and np.isfinite(W).all() and np.isfinite(D2).all()
+    return dt
+
+
+def sample_sites(V, n, seed):
+    rng = np.random.default_rng(seed)
+    return np.sort(rng.choice(V, size=min(n, V), replace=False)).astype(np.int64)
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle alone, on the box's host cores, each step a bounded sample of the workload."""
+    from oracle import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    dims, nb, s = cfg["dims"], cfg["nbasis"], args.nrhs
+    V = synth.volume(dims)
+    n_sites = args.ref_sites
+    sites = sample_sites(V, n_sites, 1)
+    A_s = synth.stencil_matrices(dims, nb, cfg["seed"], sites)             # same seeded operator, sampled sites
+    synth.add_shift(A_s, 90.0)                                             # representative diagonal shift (timing only)
+    X = synth.make_block(dims, nb, s, cfg["seed"], synth.TAG_X)
+    Ks = np.eye(s, dtype=np.complex128) * 0.5
+    for _ in range(args.warmup):
+        oracle_sample_step(dims, nb, s, sites[:max(1, n_sites // 8)], A_s[:max(1, n_sites // 8)], X, Ks)
+    times = [oracle_sample_step(dims, nb, s, sites, A_s, X, Ks) for _ in range(args.steps)]
+    total = float(np.sum(times))
+    flops = step_flops(len(sites), nb, s) * args.steps
+    value = flops / total / 1e12
+    sample = f"{len(sites)} of {V} sites per step (apply on sampled sites with the full X block + Gram/rotations on their rows)"
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload=cfg["name"], dims=list(dims), nbasis=nb, nrhs=s, storage="c64", sample=sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=oracle.num_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+# ---- our arm ---------------------------------------------------------------------------------------------------
+def load_traffic(kernel_name):
+    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture, or None."""
+    path = os.path.join(ROOT, "profiles", "apply_traffic.json")
+    if os.path.exists(path):
+        return json.load(open(path)).get(kernel_name)
+    return None
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2409_03904_b200 as cm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    dims, nb, s, dtype = cfg["dims"], cfg["nbasis"], args.nrhs, cfg["dtype"]
+    tdt = torch.complex64 if dtype == "c64" else torch.complex128
+    esize = 8 if dtype == "c64" else 16
+    V = synth.volume(dims)
+    peaks = measured_peaks()
+    K, W = args.steps, args.warmup
+    # replicas only: every rank holds the whole operator and iterates on its own block
+    seed = cfg["seed"]
+    A, c = cm.fill_synthetic(dims, nb, tdt, seed, cfg["factor"])
+    nrhs_max = max(SWEEP) if (args.sweep and rank == 0) else s
+    op = cm.CoarseOperator(dims, A, nrhs_max)
+    kernel_name = op.kernel_name(s)
+
+    # bounded sample of canonical A for the oracle leg (inputs, read back before A is released)
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        sites = sample_sites(V, args.cpu_sites, 1)
+        A_s = A[torch.from_numpy(sites).cuda()].cpu().numpy()
+    del A
+    torch.cuda.empty_cache()
+
+    B = cm.fill_block(dims, nb, s, tdt, seed + 1000 * rank, synth.TAG_B)
+    X = torch.zeros_like(B)
+    st, r0 = op.block_cg_begin(B, X, tol=1e-300)
+    assert st == cm.binding.NOT_CONVERGED, st
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    op.block_cg_step(W)                                             # W untimed warm-up steps
+    barrier()
+    clocks = ClockSampler(local_rank)
+    if rank == 0:
+        clocks.start()
+    op.profile(True)
+    l0 = cm.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    op.block_cg_step(K)                                             # exactly K timed steps
+    e1.record()
+    barrier()
+    launches = cm.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    apply_ms = op.profile_read()
+    op.profile(False)
+    clk = clocks.stop() if rank == 0 else None
+    out = op.block_cg_end()
+    assert out["status"] == 0, "block CG broke down inside the timed region"
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * K * step_flops(V, nb, s) / (ms * 1e-3) / 1e12
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline object: the stencil-GEMM apply, timed per launch inside the timed region -----------------
+    rf = roofline_tflops(V, nb, s, dtype, peaks)
+    a_ms = float(np.mean(apply_ms)) if apply_ms else float("nan")
+    a_tflops = apply_flops(V, nb, s) / (a_ms * 1e-3) / 1e12
+    a_gbs = apply_bytes(V, nb, s, esize) / (a_ms * 1e-3) / 1e9
+    if rf["bound"] == "hbm":
+        roofline = dict(bound="hbm", achieved=a_gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=a_gbs / peaks["hbm_gbs"])
+    else:
+        roofline = dict(bound="alu", achieved=a_tflops, peak=rf["alu_tflops"], unit="TFLOP/s", frac=a_tflops / rf["alu_tflops"])
+    roofline.update(traffic=load_traffic(kernel_name), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
+                    share_of_step=a_ms * len(apply_ms) / ms if apply_ms else None, peak_source=peaks["source"],
+                    intensity_flop_per_byte=rf["intensity"], hbm_gbs_achieved=a_gbs,
+                    frac_of_min_peak_IxBW=a_tflops / rf["roof_tflops"])
+
+    # ---- Nrhs sweep of the apply kernel (the metric's "vs Nrhs") --------------------------------------------
+    sweep = []
+    if args.sweep:
+        for sv in SWEEP:
+            Xs = cm.fill_block(dims, nb, sv, tdt, seed, synth.TAG_X)
+            Ys = torch.empty_like(Xs)
+            for _ in range(3):
+                op.apply(Xs, Ys)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            reps = 5
+            torch.cuda.synchronize()
+            ev[0].record()
+            for _ in range(reps):
+                op.apply(Xs, Ys)
+            ev[1].record()
+            torch.cuda.synchronize()
+            t_ms = ev[0].elapsed_time(ev[1]) / reps
+            r = roofline_tflops(V, nb, sv, dtype, peaks)
+            tf = apply_flops(V, nb, sv) / (t_ms * 1e-3) / 1e12
+            sweep.append(dict(nrhs=sv, ms=t_ms, tflops=tf, hbm_gbs=apply_bytes(V, nb, sv, esize) / (t_ms * 1e-3) / 1e9,
+                              roof_tflops=r["roof_tflops"], bound=r["bound"], frac=tf / r["roof_tflops"],
+                              kernel=op.kernel_name(sv)))
+            del Xs, Ys
+
+    # ---- block-CG solve seconds (the metric's second half), device-resident -----------------------------------
+    Xs = torch.zeros_like(B)
+    sol = op.block_cg(B, Xs, tol=cfg["tol"], maxiter=100)
+    bcg = dict(seconds=sol["seconds"], iterations=sol["iterations"], status=sol["status"], tol=cfg["tol"],
+               max_true_rel_res=max(sol["rel_res_true"]))
+
+    # ---- e2e: the same solve through the C-ABI call with pinned HOST buffers ----------------------------------
+    Bh = B.cpu().pin_memory()
+    Xh = torch.zeros_like(Bh).pin_memory()
+    op.block_cg_host(Bh, Xh, tol=cfg["tol"], maxiter=100)                       # warm-up
+    Xh.zero_()
+    l1 = cm.launch_count()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    sol_h = op.block_cg_host(Bh, Xh, tol=cfg["tol"], maxiter=100)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    its = sol_h["iterations"]
+    fl_e2e = (its + 2) * apply_flops(V, nb, s) + its * linalg_flops(V, nb, s) + 4 * 8.0 * V * nb * s * s
+    blk_bytes = V * nb * s * esize
+    e2e = dict(value=fl_e2e / t_e2e / 1e12, unit=UNIT, h2d_bytes_per_step=2 * blk_bytes / max(its, 1),
+               d2h_bytes_per_step=blk_bytes / max(its, 1), seconds=t_e2e, iterations=its,
+               call="block_cg_solve_host (B, X0 host->device, solve to tol, X device->host)",
+               launches=cm.launch_count() - l1)
+
+    # ---- CPU oracle on a bounded sample, same run ----------------------------------------------------------------
+    if not args.no_cpu_baseline:
+        from oracle import oracle
+        Xfull = cm.fill_block(dims, nb, s, tdt, seed, synth.TAG_X).cpu().numpy().astype(np.complex128)
+        Ks = np.eye(s, dtype=np.complex128) * 0.5
+        oracle_sample_step(dims, nb, s, sites[:64], A_s[:64], Xfull, Ks)       # warm-up
+        dt = oracle_sample_step(dims, nb, s, sites, A_s, Xfull, Ks)
+        cpu = dict(value=step_flops(len(sites), nb, s) / dt / 1e12, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                   sample=f"one step on {len(sites)} of {V} sites (operator bits read back from the device), {dt:.1f} s")
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms / K,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if dtype == "c64" else "f64",
+                data="synthetic", metric_note=METRIC_NOTE,
+                config=dict(workload=cfg["name"], dims=list(dims), nbasis=nb, nrhs=s, storage=dtype, stencil_points=81,
+                            operator_bytes=81 * V * nb * nb * esize, parallelism="replicas only" if world > 1 else "1 GPU",
+                            l2="inputs (27.5 GB operator) larger than L2; no flush", diagonal_shift_c=c),
+                clocks=clk, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,
+                sweep=sweep, block_cg_solve=bcg,
+                step_breakdown=dict(apply_ms=a_ms, other_ms=ms / K - a_ms, final_recursive_rel_res=max(out["rel_res_recursive"])))
+    print(json.dumps(line))
+    op.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--nrhs", type=int, default=16)
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3: the Nrhs-sweep workload)")
+    ap.add_argument("--no-sweep", dest="sweep", action="store_false")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sites", type=int, default=1536, help="sampled sites of the cpu_baseline leg")
+    ap.add_argument("--ref-sites", type=int, default=384, help="sampled sites per step of --impl reference")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                             # timing rule: at least 3 warm-up steps
+    cfg = synth.config(args.config)
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    return run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

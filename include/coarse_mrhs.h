@@ -1,0 +1,193 @@
+/*
+ * coarse_mrhs.h -- C ABI of the B200-native coarse-grid multi-RHS operator and block CG
+ * (data-parallel hot path of the multiple right-hand-side HDCG method, arXiv:2409.03904).
+ *
+ * Citations are PAPER.md:<line> (the paper text) plus section / equation.
+ *
+ * Conventions shared by every entry point
+ * ---------------------------------------
+ *  - "dev" pointers are CUDA device pointers owned by the CALLER (e.g. torch tensors); "host" pointers
+ *    are ordinary host memory owned by the caller.  The library never frees or keeps a caller pointer
+ *    beyond the call, except where stated (coarse_op_create copies A).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *  - Every function returns a status code (COARSE_OK = 0, negative = error); no exceptions cross the ABI.
+ *    On COARSE_INVALID_ARG / COARSE_UNSUPPORTED the outputs are untouched.  coarse_last_error() returns a
+ *    thread-local, human-readable description of the last failure.
+ *  - There is NO CPU fallback: every entry point that computes runs CUDA kernels on the current device
+ *    and fails with COARSE_CUDA_ERROR when there is none.
+ *
+ * Canonical (boundary) layouts
+ * ----------------------------
+ *  lattice site     x = x0 + L0*(x1 + L1*(x2 + L2*x3)),  dims = {L0, L1, L2, L3}, dims[0] fastest
+ *  stencil point    p = (d0+1) + 3*(d1+1) + 9*(d2+1) + 27*(d3+1),  d_k in {-1,0,1}; centre p = 40,
+ *                   opposite point 80-p.  81 points = all relative shifts (-1..1)^4.
+ *  stencil matrices A : [V][81][nbasis][nbasis], row-major blocks, interleaved (re, im)
+ *  vector blocks    X, Y, B : [V][nbasis][nrhs], right-hand-side index fastest, interleaved (re, im)
+ *                   ("N_basis x N_rhs" per coarse site; the RHS index is the paper's
+ *                   fictitious fifth dimension)
+ *  dtype            COARSE_C64: float re/im pairs; COARSE_C128: double re/im pairs
+ *  boundary         periodic: neighbour = (x_k + d_k + L_k) mod L_k.  With L_k = 1 or 2 several stencil
+ *                   points address the same neighbour; their contributions ADD.
+ */
+#ifndef COARSE_MRHS_H
+#define COARSE_MRHS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct coarse_op coarse_op_t; /* opaque, library-owned */
+
+enum { COARSE_C64 = 0, COARSE_C128 = 1 };
+
+enum {
+    COARSE_OK = 0,
+    COARSE_INVALID_ARG = -1,
+    COARSE_UNSUPPORTED = -2,   /* shape outside 1 <= nbasis <= 64, 1 <= nrhs <= 64 */
+    COARSE_CUDA_ERROR = -3,
+    COARSE_OUT_OF_MEMORY = -4,
+    COARSE_NOT_CONVERGED = -5, /* block_cg_solve hit maxiter; outputs are valid */
+    COARSE_BREAKDOWN = -6      /* a Gram matrix was not positive definite (no column deflation) */
+};
+
+/* create-time flags */
+enum {
+    COARSE_FLAG_FORCE_GENERIC = 1u << 0, /* always use the generic (untiled) stencil kernel: test / debugging aid */
+    COARSE_FLAG_NO_TENSOR = 1u << 1      /* never select a tensor-core kernel variant */
+};
+
+#define COARSE_MAX_NRHS 64
+#define COARSE_MAX_NBASIS 64
+
+/*
+ * coarse_op_create -- build the operator object.  "The coarse matrix coefficients are stored entirely
+ * internal to this object" and the neighbour addressing is precomputed once.
+ *   out       : receives the handle
+ *   dims      : host, 4 extents, each >= 1
+ *   nbasis    : 1..64 (rows/cols of each stencil matrix)
+ *   nrhs_max  : 1..64, largest nrhs later passed to apply / solve; sizes the block-CG workspace
+ *   dtype     : COARSE_C64 or COARSE_C128 (storage and multiply precision of A, X, Y)
+ *   A_dev     : device, canonical layout; COPIED (re-laid-out for the kernels) -- may be freed after return
+ *   flags     : COARSE_FLAG_*
+ * Allocates device memory: one internal copy of A, V*81 int32 neighbour table, 6 vector blocks of
+ * V*nbasis*nrhs_max elements plus O(grid * nrhs_max^2) reduction scratch.  Synchronises `stream`.
+ */
+int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_t nbasis, int32_t nrhs_max,
+                     int32_t dtype, const void *A_dev, uint32_t flags, void *stream);
+
+int coarse_op_destroy(coarse_op_t *op);
+
+/*
+ * coarse_op_apply -- Y(x) = sum_{p=0}^{80} A^p(x) . X(x + delta_p) for all sites, one launch
+ * (Eq. 19 summed over the stencil; the paper issues 81 batched GEMMs).
+ *   X_dev, Y_dev : device, [V][nbasis][nrhs], dtype of the operator; Y must not alias X
+ *   nrhs         : 1..nrhs_max
+ * Asynchronous on `stream`; allocates nothing.
+ */
+int coarse_op_apply(const coarse_op_t *op, const void *X_dev, void *Y_dev, int32_t nrhs, void *stream);
+
+/* Same operation with HOST buffers: copies X host->device, applies, copies Y device->host, synchronises.
+ * Uses the operator's own workspace blocks (the paper's "import/export to preallocated arrays"). */
+int coarse_op_apply_host(coarse_op_t *op, const void *X_host, void *Y_host, int32_t nrhs, void *stream);
+
+/*
+ * block_cg_solve -- BlockCGrQ (Fig. 2 left) for H X = B with the operator above:
+ *   R = B - H X0;  Q C = R (Cholesky QR);  D = Q;  loop:  Z = H D;  M = (D^H Z)^-1;
+ *   X += D M C;  Q S = Q - Z M;  D = Q + D S^H;  C = S C;  stop when max_r ||C[:,r]|| / ||B[:,r]|| <= tol.
+ * (X update carries C_k: DESIGN.md reading R1.)
+ *   B_dev   : device, sources, [V][nbasis][nrhs]
+ *   X_dev   : device, in: initial guess X0, out: solution
+ *   res     : host; iterations = number of H.D products in the loop; rel_res_recursive[r] from C,
+ *             rel_res_true[r] = ||B - H X||/||B|| from one extra apply; history[k] = max_r recursive
+ *             relative residual after k iterations (k <= COARSE_MAX_HISTORY-1)
+ * Returns COARSE_OK, COARSE_NOT_CONVERGED or COARSE_BREAKDOWN (res->status holds the same).
+ * Synchronises `stream` (one scalar is read back per iteration for the stop test).
+ */
+#define COARSE_MAX_HISTORY 256
+typedef struct {
+    int32_t iterations;
+    int32_t status;
+    double rel_res_recursive[COARSE_MAX_NRHS];
+    double rel_res_true[COARSE_MAX_NRHS];
+    double history[COARSE_MAX_HISTORY];
+    double seconds; /* wall time of the solve, host clock, stream synchronised on both sides */
+} block_cg_result;
+
+int block_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol,
+                   int32_t maxiter, block_cg_result *res, void *stream);
+
+/*
+ * The same solve in three calls, for callers that drive the iteration themselves (bench.py times exactly K
+ * iterations on the device this way; block_cg_solve is begin + {step, read stop scalar} + end):
+ *   block_cg_begin : R = B - H X0, Q C = R, D = Q (statements 4-6 of Fig. 2 left).  Synchronises
+ *                    (reads the initial residual into *rel_res0, may be NULL).  Returns COARSE_NOT_CONVERGED when
+ *                    iterations are needed (the normal case), COARSE_OK when X0 already meets tol, or an error.
+ *                    B_dev and X_dev must stay valid until block_cg_end.
+ *   block_cg_step  : `count` iterations (statements 8-13); asynchronous, no host read, no stop test.
+ *   block_cg_end   : one extra apply for the true residual; fills res (status OK or BREAKDOWN); synchronises.
+ */
+int block_cg_begin(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, double *rel_res0,
+                   void *stream);
+int block_cg_step(coarse_op_t *op, int32_t count, void *stream);
+int block_cg_end(coarse_op_t *op, block_cg_result *res, void *stream);
+
+/* Same with HOST buffers for B (in) and X (in: X0, out: solution). */
+int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
+                        int32_t maxiter, block_cg_result *res, void *stream);
+
+/*
+ * The block-CG building blocks, exported so that each can be checked against the oracle on its own.
+ * n = number of rows (V*nbasis), s = nrhs (1..64); blocks are [n][s] in `dtype`; s x s matrices are
+ * ALWAYS complex128, row-major, on the device.
+ *
+ * coarse_block_gram   : G = U^H W  (Table 6 "ThinQR" shape).
+ *                       Deterministic two-stage reduction; products in `dtype`, partial sums in double.
+ * coarse_small_cholesky: G = S^H S, S upper triangular with positive diagonal (G symmetrised first);
+ *                       optionally S^-1.  info_dev (int32, device) = 0 or COARSE_BREAKDOWN.
+ * coarse_small_hpd_inverse: M = G^-1 through the Cholesky factor (M_k = [D^H Z]^-1).
+ * coarse_block_rotate : W = beta*W + U K, K s x s (the "block rotations" X += D M C, Q - Z M, T S^-1,
+ *                       Q + D S^H of PAPER.md:145-149); beta in {0,1} or any real; W may alias neither U.
+ */
+int coarse_block_gram(coarse_op_t *op, const void *U_dev, const void *W_dev, void *G_dev, int64_t n,
+                      int32_t s, void *stream);
+int coarse_small_cholesky(const void *G_dev, void *S_dev, void *Sinv_dev /* may be NULL */, int32_t s,
+                          int32_t *info_dev, void *stream);
+int coarse_small_hpd_inverse(const void *G_dev, void *M_dev, int32_t s, int32_t *info_dev, void *stream);
+int coarse_block_rotate(coarse_op_t *op, const void *U_dev, const void *K_dev, void *W_dev, double beta,
+                        int64_t n, int32_t s, void *stream);
+
+/*
+ * Bench convenience (input generation, not part of the method): fills A_dev (canonical layout) with the
+ * seeded synthetic Hermitian positive definite operator of DESIGN.md "Synthetic inputs" -- the same
+ * counter-based hash as inputs/synth.py, implemented independently on the device.
+ *   c_factor : diagonal shift c = c_factor * max_x [ ||Hrand(x)||_F + sum_{p != 40} ||A_p(x)||_F ]
+ *   c_out    : host, receives c (float32-exact)
+ * coarse_fill_block fills a [V][nbasis][nrhs] block with complex N(0,1) values of stream `tag`.
+ */
+int coarse_op_fill_synthetic(void *A_dev, const int32_t dims[4], int32_t nbasis, int32_t dtype,
+                             uint64_t seed, double c_factor, double *c_out, void *stream);
+int coarse_fill_block(void *X_dev, const int32_t dims[4], int32_t nbasis, int32_t nrhs, int32_t dtype,
+                      uint64_t seed, int32_t tag, void *stream);
+
+/* Introspection: name of the stencil kernel variant coarse_op_apply would launch for `nrhs`
+ * (static string), bytes of device memory owned by the handle, and the number of kernels this library
+ * has launched in this process so far (monotonic; used for bench.py's gpu_launches). */
+const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs);
+int64_t coarse_op_device_bytes(const coarse_op_t *op);
+int64_t coarse_launch_count(void);
+
+/* Per-launch device timing of the stencil kernel (measurement aid for bench.py's roofline object):
+ * while enabled, every coarse_op_apply -- including those inside block_cg_* -- is bracketed by a CUDA event
+ * pair on its launch stream (at most 64 pairs are kept).  coarse_op_profile_read synchronises on the events,
+ * writes the durations in milliseconds to ms[0..*count) (host) and clears the list. */
+int coarse_op_profile(coarse_op_t *op, int32_t enable);
+int coarse_op_profile_read(coarse_op_t *op, double *ms, int32_t capacity, int32_t *count);
+
+const char *coarse_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COARSE_MRHS_H */

@@ -10,6 +10,7 @@
  *   - oracle_gram        : the s x s block inner product U^H W           (Table 6 "ThinQR")
  *   - oracle_cholesky_upper, oracle_upper_inverse, oracle_hpd_inverse :
  *                          the small dense algebra of BlockCGrQ
+ *   - oracle_block_rotate: the block rotation W = beta W + U K
  *   - oracle_block_cg    : BlockCGrQ, Fig. 2 (left), step by step in the paper's
  *                          order and notation, with the X-update read as X + D M C (reading R1).
  *
@@ -169,6 +170,20 @@ static void block_times_small(int64_t n, int32_t s, const zd *U, const zd *K, zd
             W[k * s + b].re = re;
             W[k * s + b].im = im;
         }
+}
+
+/* Block rotation as one exported call (the "block rotations" of PAPER.md:145-149):
+ * W = beta * W + U . K, U, W : [n][s], K : [s][s].  Same loop nest as block_times_small above. */
+void oracle_block_rotate(int64_t n, int32_t s, const double *U, const double *K, double beta, double *W)
+{
+    zd *tmp = (zd *)malloc(sizeof(zd) * (size_t)n * s);
+    zd *Wz = (zd *)W;
+    block_times_small(n, s, (const zd *)U, (const zd *)K, tmp);
+    for (int64_t e = 0; e < n * s; ++e) {
+        Wz[e].re = beta * Wz[e].re + tmp[e].re;
+        Wz[e].im = beta * Wz[e].im + tmp[e].im;
+    }
+    free(tmp);
 }
 
 static void small_matmul(int32_t s, const zd *P, const zd *Q, zd *R) /* R = P Q */

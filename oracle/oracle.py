@@ -55,6 +55,8 @@ def lib():
         L.oracle_upper_inverse.argtypes = [C.c_int32, C.c_void_p, C.c_void_p]
         L.oracle_hpd_inverse.restype = C.c_int
         L.oracle_hpd_inverse.argtypes = [C.c_int32, C.c_void_p, C.c_void_p]
+        L.oracle_block_rotate.restype = None
+        L.oracle_block_rotate.argtypes = [C.c_int64, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.oracle_block_cg.restype = C.c_int
         L.oracle_block_cg.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                       C.c_void_p, C.c_double, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
@@ -142,6 +144,15 @@ def hpd_inverse(G):
     out = np.empty((s, s), dtype=np.complex128)
     st = lib().oracle_hpd_inverse(s, G.ctypes.data, out.ctypes.data)
     return st, out
+
+
+def block_rotate(U, K, W, beta: float) -> np.ndarray:
+    """returns beta*W + U K (a new array); U, W: [...][s], K: [s][s]."""
+    U, K = _z(U), _z(K)
+    out = _z(W).copy()
+    s = U.shape[-1]
+    lib().oracle_block_rotate(U.size // s, s, U.ctypes.data, K.ctypes.data, float(beta), out.ctypes.data)
+    return out
 
 
 def block_cg(dims, A, B, X0=None, tol: float = 1e-10, maxiter: int = 1000, callback=None):

@@ -1,0 +1,6 @@
+"""B200-native coarse-grid multi-RHS operator and block CG (arXiv:2409.03904 hot path).
+
+The product is the C-ABI library (include/coarse_mrhs.h, csrc/); this package is its ctypes binding.
+"""
+from .binding import (C64, C128, BlockCGResult, CoarseError, CoarseOperator, fill_block, fill_synthetic,  # noqa: F401
+                      launch_count, lib, library_path, small_cholesky, small_hpd_inverse)

@@ -1,0 +1,272 @@
+"""Thin ctypes binding of the C ABI in include/coarse_mrhs.h -- argument marshalling only.
+
+Every step of the path (neighbour table, stencil-GEMM apply, Gram products, s x s algebra, block
+rotations, the BlockCGrQ loop) runs in the CUDA kernels behind the C entry points; nothing here
+computes.  PyTorch is used for device memory and streams only.  There is no CPU fallback: if the shared
+library is missing or a call fails, a CoarseError is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import torch
+
+from . import build as _build
+
+C64, C128 = 0, 1
+OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY, NOT_CONVERGED, BREAKDOWN = 0, -1, -2, -3, -4, -5, -6
+FLAG_FORCE_GENERIC, FLAG_NO_TENSOR = 1, 2
+MAX_NRHS, MAX_HISTORY = 64, 256
+
+EXPORTS = [
+    "coarse_op_create", "coarse_op_destroy", "coarse_op_apply", "coarse_op_apply_host", "block_cg_solve",
+    "block_cg_solve_host", "block_cg_begin", "block_cg_step", "block_cg_end", "coarse_block_gram", "coarse_small_cholesky", "coarse_small_hpd_inverse",
+    "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
+    "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
+]
+
+
+class CoarseError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"coarse_mrhs status {status}: {msg}")
+        self.status = status
+
+
+class BlockCGResult(C.Structure):
+    _fields_ = [("iterations", C.c_int32), ("status", C.c_int32),
+                ("rel_res_recursive", C.c_double * MAX_NRHS), ("rel_res_true", C.c_double * MAX_NRHS),
+                ("history", C.c_double * MAX_HISTORY), ("seconds", C.c_double)]
+
+
+_lib = None
+
+
+def library_path() -> Path:
+    return _build.LIB
+
+
+def lib():
+    """Loads libcoarse_mrhs.so (building it with nvcc when the sources are newer).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(str(path))
+        vp, i32, i64, u32, u64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_double
+        sig = {
+            "coarse_op_create": (C.c_int, [C.POINTER(vp), vp, i32, i32, i32, vp, u32, vp]),
+            "coarse_op_destroy": (C.c_int, [vp]),
+            "coarse_op_apply": (C.c_int, [vp, vp, vp, i32, vp]),
+            "coarse_op_apply_host": (C.c_int, [vp, vp, vp, i32, vp]),
+            "block_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(BlockCGResult), vp]),
+            "block_cg_solve_host": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(BlockCGResult), vp]),
+            "block_cg_begin": (C.c_int, [vp, vp, vp, i32, dbl, C.POINTER(dbl), vp]),
+            "block_cg_step": (C.c_int, [vp, i32, vp]),
+            "block_cg_end": (C.c_int, [vp, C.POINTER(BlockCGResult), vp]),
+            "coarse_block_gram": (C.c_int, [vp, vp, vp, vp, i64, i32, vp]),
+            "coarse_small_cholesky": (C.c_int, [vp, vp, vp, i32, vp, vp]),
+            "coarse_small_hpd_inverse": (C.c_int, [vp, vp, i32, vp, vp]),
+            "coarse_block_rotate": (C.c_int, [vp, vp, vp, vp, dbl, i64, i32, vp]),
+            "coarse_op_fill_synthetic": (C.c_int, [vp, vp, i32, i32, u64, dbl, C.POINTER(dbl), vp]),
+            "coarse_fill_block": (C.c_int, [vp, vp, i32, i32, i32, u64, i32, vp]),
+            "coarse_op_kernel_name": (C.c_char_p, [vp, i32]),
+            "coarse_op_device_bytes": (i64, [vp]),
+            "coarse_launch_count": (i64, []),
+            "coarse_last_error": (C.c_char_p, []),
+            "coarse_op_profile": (C.c_int, [vp, i32]),
+            "coarse_op_profile_read": (C.c_int, [vp, C.POINTER(dbl), i32, C.POINTER(i32)]),
+        }
+        for name, (res, args) in sig.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(st: int, allow=()):
+    if st != OK and st not in allow:
+        raise CoarseError(st, lib().coarse_last_error().decode())
+    return st
+
+
+def _stream(stream=None) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.complex64:
+        return C64
+    if t.dtype == torch.complex128:
+        return C128
+    raise TypeError("tensors must be complex64 or complex128")
+
+
+def _dims(dims):
+    return (C.c_int32 * 4)(*[int(d) for d in dims])
+
+
+def _dev(t: torch.Tensor) -> int:
+    if not (t.is_cuda and t.is_contiguous()):
+        raise ValueError("expected a contiguous CUDA tensor")
+    return t.data_ptr()
+
+
+def launch_count() -> int:
+    return int(lib().coarse_launch_count())
+
+
+class CoarseOperator:
+    """Handle of coarse_op_create.  A: [V][81][nb][nb] complex CUDA tensor (canonical layout; copied)."""
+
+    def __init__(self, dims, A: torch.Tensor, nrhs_max: int, flags: int = 0, stream=None):
+        self.dims = tuple(int(d) for d in dims)
+        V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        if A.dim() != 4 or A.shape[0] != V or A.shape[1] != 81 or A.shape[2] != A.shape[3]:
+            raise ValueError("A must be [V][81][nbasis][nbasis]")
+        self.V, self.nbasis, self.nrhs_max, self.dtype = V, int(A.shape[2]), int(nrhs_max), A.dtype
+        self._h = C.c_void_p()
+        _check(lib().coarse_op_create(C.byref(self._h), _dims(self.dims), self.nbasis, self.nrhs_max, _dtype_code(A),
+                                      _dev(A), flags, _stream(stream)))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().coarse_op_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _block_ok(self, X: torch.Tensor) -> int:
+        if X.dtype != self.dtype or X.dim() != 3 or X.shape[0] != self.V or X.shape[1] != self.nbasis:
+            raise ValueError("blocks must be [V][nbasis][nrhs] in the operator's dtype")
+        return int(X.shape[2])
+
+    def kernel_name(self, nrhs: int) -> str:
+        return lib().coarse_op_kernel_name(self._h, int(nrhs)).decode()
+
+    def device_bytes(self) -> int:
+        return int(lib().coarse_op_device_bytes(self._h))
+
+    def profile(self, enable: bool):
+        _check(lib().coarse_op_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """milliseconds of each stencil-kernel launch since the last read (CUDA events on the launch stream)."""
+        ms = (C.c_double * 64)()
+        n = C.c_int32(0)
+        _check(lib().coarse_op_profile_read(self._h, ms, 64, C.byref(n)))
+        return [ms[i] for i in range(n.value)]
+
+    def apply(self, X: torch.Tensor, Y: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+        """coarse_op_apply: Y(x) = sum_p A_p(x) X(x + delta_p)  (Eq. 19)."""
+        s = self._block_ok(X)
+        if Y is None:
+            Y = torch.empty_like(X)
+        self._block_ok(Y)
+        _check(lib().coarse_op_apply(self._h, _dev(X), _dev(Y), s, _stream(stream)))
+        return Y
+
+    def apply_host(self, X: torch.Tensor, Y: torch.Tensor, stream=None) -> torch.Tensor:
+        """coarse_op_apply_host: X, Y are (pinned) HOST tensors; H2D + apply + D2H + sync."""
+        s = self._block_ok(X)
+        self._block_ok(Y)
+        if X.is_cuda or Y.is_cuda or not X.is_contiguous() or not Y.is_contiguous():
+            raise ValueError("apply_host takes contiguous host tensors")
+        _check(lib().coarse_op_apply_host(self._h, X.data_ptr(), Y.data_ptr(), s, _stream(stream)))
+        return Y
+
+    def _result(self, res: BlockCGResult, s: int, X):
+        k = res.iterations
+        return dict(X=X, iterations=int(k), status=int(res.status), seconds=float(res.seconds),
+                    history=[res.history[i] for i in range(min(k + 1, MAX_HISTORY))],
+                    rel_res_recursive=[res.rel_res_recursive[r] for r in range(s)],
+                    rel_res_true=[res.rel_res_true[r] for r in range(s)])
+
+    def block_cg(self, B: torch.Tensor, X: torch.Tensor | None = None, tol: float = 1e-6, maxiter: int = 1000, stream=None):
+        """block_cg_solve: BlockCGrQ (Fig. 2 left).  X in: X0 (zeros if None), out: solution."""
+        s = self._block_ok(B)
+        if X is None:
+            X = torch.zeros_like(B)
+        self._block_ok(X)
+        res = BlockCGResult()
+        _check(lib().block_cg_solve(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), C.byref(res), _stream(stream)),
+               allow=(NOT_CONVERGED, BREAKDOWN))
+        return self._result(res, s, X)
+
+    def block_cg_begin(self, B: torch.Tensor, X: torch.Tensor, tol: float = 1e-6, stream=None):
+        """block_cg_begin: returns (status, initial max relative residual)."""
+        s = self._block_ok(B)
+        self._block_ok(X)
+        self._bcg_keep = (B, X)
+        r0 = C.c_double(0.0)
+        st = _check(lib().block_cg_begin(self._h, _dev(B), _dev(X), s, float(tol), C.byref(r0), _stream(stream)),
+                    allow=(NOT_CONVERGED, BREAKDOWN))
+        return st, float(r0.value)
+
+    def block_cg_step(self, count: int = 1, stream=None):
+        _check(lib().block_cg_step(self._h, int(count), _stream(stream)))
+
+    def block_cg_end(self, stream=None):
+        res = BlockCGResult()
+        _check(lib().block_cg_end(self._h, C.byref(res), _stream(stream)), allow=(BREAKDOWN,))
+        B, X = self._bcg_keep
+        return self._result(res, int(B.shape[2]), X)
+
+    def block_cg_host(self, B: torch.Tensor, X: torch.Tensor, tol: float = 1e-6, maxiter: int = 1000, stream=None):
+        s = self._block_ok(B)
+        self._block_ok(X)
+        if B.is_cuda or X.is_cuda:
+            raise ValueError("block_cg_host takes host tensors")
+        res = BlockCGResult()
+        _check(lib().block_cg_solve_host(self._h, B.data_ptr(), X.data_ptr(), s, float(tol), int(maxiter), C.byref(res),
+                                         _stream(stream)), allow=(NOT_CONVERGED, BREAKDOWN))
+        return self._result(res, s, X)
+
+    # ---- block-CG building blocks (each parity-tested on its own) ----
+    def gram(self, U: torch.Tensor, W: torch.Tensor, stream=None) -> torch.Tensor:
+        s = int(U.shape[-1])
+        n = U.numel() // s
+        G = torch.empty((s, s), dtype=torch.complex128, device=U.device)
+        _check(lib().coarse_block_gram(self._h, _dev(U), _dev(W), _dev(G), n, s, _stream(stream)))
+        return G
+
+    def rotate(self, U: torch.Tensor, K: torch.Tensor, W: torch.Tensor, beta: float, stream=None) -> torch.Tensor:
+        """W = beta*W + U K, K s x s complex128 on the device."""
+        s = int(U.shape[-1])
+        n = U.numel() // s
+        _check(lib().coarse_block_rotate(self._h, _dev(U), _dev(K), _dev(W), float(beta), n, s, _stream(stream)))
+        return W
+
+
+def small_cholesky(G: torch.Tensor, want_inverse: bool = True, stream=None):
+    s = int(G.shape[0])
+    S = torch.empty_like(G)
+    Sinv = torch.empty_like(G) if want_inverse else None
+    info = torch.zeros(1, dtype=torch.int32, device=G.device)
+    _check(lib().coarse_small_cholesky(_dev(G), _dev(S), _dev(Sinv) if want_inverse else None, s, _dev(info), _stream(stream)))
+    return S, Sinv, int(info.item())
+
+
+def small_hpd_inverse(G: torch.Tensor, stream=None):
+    s = int(G.shape[0])
+    M = torch.empty_like(G)
+    info = torch.zeros(1, dtype=torch.int32, device=G.device)
+    _check(lib().coarse_small_hpd_inverse(_dev(G), _dev(M), s, _dev(info), _stream(stream)))
+    return M, int(info.item())
+
+
+def fill_synthetic(dims, nbasis: int, dtype: torch.dtype, seed: int, c_factor: float, device="cuda", stream=None):
+    """coarse_op_fill_synthetic: device-side seeded HPD operator (input generation).  Returns (A, c)."""
+    V = int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
+    A = torch.empty((V, 81, nbasis, nbasis), dtype=dtype, device=device)
+    c = C.c_double(0.0)
+    _check(lib().coarse_op_fill_synthetic(_dev(A), _dims(dims), nbasis, _dtype_code(A), int(seed), float(c_factor),
+                                          C.byref(c), _stream(stream)))
+    return A, float(c.value)
+
+
+def fill_block(dims, nbasis: int, nrhs: int, dtype: torch.dtype, seed: int, tag: int, device="cuda", stream=None):
+    V = int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
+    X = torch.empty((V, nbasis, nrhs), dtype=dtype, device=device)
+    _check(lib().coarse_fill_block(_dev(X), _dims(dims), nbasis, nrhs, _dtype_code(X), int(seed), int(tag), _stream(stream)))
+    return X

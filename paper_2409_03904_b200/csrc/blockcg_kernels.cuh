@@ -1,0 +1,428 @@
+// Block-CG linear algebra kernels:
+//   Gram products  G = U^H W             ("ThinQR" 12x12x1M shape of Table 6)
+//   block rotations W = beta V + U K
+//   s x s algebra in complex128: Cholesky, triangular / HPD inverse, products, stop scalar.
+// Reductions are deterministic: fixed partition of rows over CTAs, fixed summation order, no float atomics.
+#pragma once
+
+#include "common.cuh"
+
+namespace cmrhs {
+
+constexpr int kLaThreads = 256;
+
+// ------------------------------------------------------------------------------------------------------
+// Gram product, stage 1: each CTA reduces a contiguous chunk of rows to one s x s partial (double).
+// Thread layout: the s x s result is cut into TT x TT sub-blocks (one per thread "tile"); the 256 threads
+// are (row group) x (tile).  Products and short runs in T, flushed to double every row tile.
+// ------------------------------------------------------------------------------------------------------
+template <typename T, int TT>
+__global__ void __launch_bounds__(kLaThreads)
+gram_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W, int64_t n, int s, int rows_per_tile,
+                    zdouble *__restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sU = reinterpret_cast<cplx<T> *>(smem_raw);
+    cplx<T> *sW = sU + (size_t)rows_per_tile * s;
+    const int nt = (s + TT - 1) / TT;          // tiles per dimension
+    const int ntile = nt * nt;
+    const int RG = kLaThreads / ntile;         // row groups (>= 1 because nt <= 16)
+    const int tile = threadIdx.x % ntile, rg = threadIdx.x / ntile;
+    const bool active = rg < RG;
+    const int a0 = (tile / nt) * TT, b0 = (tile % nt) * TT;
+
+    const int64_t chunk = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t r_begin = blockIdx.x * chunk;
+    const int64_t r_end = (r_begin + chunk < n) ? r_begin + chunk : n;
+
+    double accr[TT][TT], acci[TT][TT];
+#pragma unroll
+    for (int a = 0; a < TT; ++a)
+#pragma unroll
+        for (int b = 0; b < TT; ++b) { accr[a][b] = 0.0; acci[a][b] = 0.0; }
+
+    for (int64_t r0 = r_begin; r0 < r_end; r0 += rows_per_tile) {
+        const int nrow = (int)((r_end - r0 < rows_per_tile) ? (r_end - r0) : rows_per_tile);
+        const cplx<T> *gu = U + r0 * s, *gw = W + r0 * s;
+        for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) { sU[e] = gu[e]; sW[e] = gw[e]; }
+        __syncthreads();
+        if (active) {
+            cplx<T> run[TT][TT];
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) { run[a][b].re = 0; run[a][b].im = 0; }
+            for (int k = rg; k < nrow; k += RG) {
+                cplx<T> u[TT], w[TT];
+#pragma unroll
+                for (int a = 0; a < TT; ++a) {
+                    const bool ok = a0 + a < s;
+                    u[a] = ok ? sU[k * s + a0 + a] : cplx<T>{0, 0};
+                }
+#pragma unroll
+                for (int b = 0; b < TT; ++b) {
+                    const bool ok = b0 + b < s;
+                    w[b] = ok ? sW[k * s + b0 + b] : cplx<T>{0, 0};
+                }
+#pragma unroll
+                for (int a = 0; a < TT; ++a)
+#pragma unroll
+                    for (int b = 0; b < TT; ++b) cmac_conj(run[a][b], u[a], w[b]);
+            }
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) { accr[a][b] += (double)run[a][b].re; acci[a][b] += (double)run[a][b].im; }
+        }
+        __syncthreads();
+    }
+
+    // reduce the row groups in a fixed order (group 0, 1, 2, ...) through shared memory; the staging buffer is
+    // reused as s*s complex doubles (it is only needed when RG > 1, i.e. for small s)
+    zdouble *out = partial + (size_t)blockIdx.x * s * s;
+    if (RG == 1) {
+        if (active) {
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b)
+                    if (a0 + a < s && b0 + b < s) out[(a0 + a) * s + b0 + b] = {accr[a][b], acci[a][b]};
+        }
+        return;
+    }
+    double *red = reinterpret_cast<double *>(smem_raw);
+    for (int g = 0; g < RG; ++g) {
+        if (active && rg == g) {
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b)
+                    if (a0 + a < s && b0 + b < s) {
+                        const int e = (a0 + a) * s + b0 + b;
+                        if (g == 0) { red[2 * e] = accr[a][b]; red[2 * e + 1] = acci[a][b]; }
+                        else { red[2 * e] += accr[a][b]; red[2 * e + 1] += acci[a][b]; }
+                    }
+        }
+        __syncthreads();
+    }
+    for (int e = threadIdx.x; e < s * s; e += kLaThreads) { out[e].re = red[2 * e]; out[e].im = red[2 * e + 1]; }
+}
+
+// stage 2: G[e] = sum_b partial[b][e], b in increasing order
+__global__ void gram_reduce_kernel(const zdouble *__restrict__ partial, int nblocks, int ss, zdouble *__restrict__ G)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= ss) return;
+    double re = 0.0, im = 0.0;
+    for (int b = 0; b < nblocks; ++b) { re += partial[(size_t)b * ss + e].re; im += partial[(size_t)b * ss + e].im; }
+    G[e].re = re;
+    G[e].im = im;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Block rotation  out = beta * Vin + U K   (n x s times s x s).  out may alias U and/or Vin: a CTA stages
+// its rows of U in shared memory before it writes them.  K is complex128 on the device, rounded to T at use
+// (reading R11).
+// ------------------------------------------------------------------------------------------------------
+template <typename T, int TC>
+__global__ void __launch_bounds__(kLaThreads)
+rotate_kernel(const cplx<T> *U, const zdouble *__restrict__ K, const cplx<T> *Vin, cplx<T> *out, T beta,
+              int64_t n, int s, int rows_per_tile)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sK = reinterpret_cast<cplx<T> *>(smem_raw);          // [s][s]
+    cplx<T> *sU = sK + (size_t)s * s;                              // [rows_per_tile][s + 1] (padded: row lanes hit different banks)
+    const int su = s + 1;
+    for (int e = threadIdx.x; e < s * s; e += kLaThreads) { sK[e].re = (T)K[e].re; sK[e].im = (T)K[e].im; }
+    const int ncg = (s + TC - 1) / TC;            // column groups (<= 16)
+    const int RL = kLaThreads / ncg;              // row lanes
+    const int cg = threadIdx.x % ncg, rl = threadIdx.x / ncg;
+    const int c0 = cg * TC;
+    const int64_t ntiles = (n + rows_per_tile - 1) / rows_per_tile;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t r0 = t * rows_per_tile;
+        const int nrow = (int)((n - r0 < rows_per_tile) ? (n - r0) : rows_per_tile);
+        __syncthreads();
+        const cplx<T> *gu = U + r0 * s;
+        for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) sU[(e / s) * su + e % s] = gu[e];
+        __syncthreads();
+        if (rl < RL) {
+            for (int k = rl; k < nrow; k += RL) {
+                cplx<T> acc[TC];
+#pragma unroll
+                for (int c = 0; c < TC; ++c) { acc[c].re = 0; acc[c].im = 0; }
+                for (int a = 0; a < s; ++a) {
+                    const cplx<T> u = sU[k * su + a];
+#pragma unroll
+                    for (int c = 0; c < TC; ++c)
+                        if (c0 + c < s) cmac(acc[c], u, sK[a * s + c0 + c]);
+                }
+#pragma unroll
+                for (int c = 0; c < TC; ++c)
+                    if (c0 + c < s) {
+                        const int64_t e = (r0 + k) * s + c0 + c;
+                        cplx<T> v = acc[c];
+                        if (beta != (T)0) { const cplx<T> w = Vin[e]; v.re = fma(beta, w.re, v.re); v.im = fma(beta, w.im, v.im); }
+                        out[e] = v;
+                    }
+            }
+        }
+    }
+}
+
+// out = a*U + b*W elementwise (used for R = B - H X and copies)
+template <typename T>
+__global__ void axpby_kernel(const cplx<T> *U, const cplx<T> *W, cplx<T> *out, T a, T b, int64_t total)
+{
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        cplx<T> v;
+        v.re = a * U[e].re + b * W[e].re;
+        v.im = a * U[e].im + b * W[e].im;
+        out[e] = v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// s x s complex128 algebra, one CTA, matrices in shared memory (row-major, leading dimension s).
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ zdouble zmul(zdouble a, zdouble b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ zdouble zmulc(zdouble a, zdouble b) { return {a.re * b.re + a.im * b.im, a.re * b.im - a.im * b.re}; }   // conj(a)*b
+
+__device__ void sm_load(zdouble *dst, const zdouble *src, int ss)
+{
+    for (int e = threadIdx.x; e < ss; e += blockDim.x) dst[e] = src[e];
+    __syncthreads();
+}
+__device__ void sm_store(zdouble *dst, const zdouble *src, int ss)
+{
+    __syncthreads();
+    for (int e = threadIdx.x; e < ss; e += blockDim.x) dst[e] = src[e];
+}
+
+// In place: G (Hermitian positive definite, symmetrised from its upper triangle and the conjugate of its lower)
+// -> S upper triangular, positive real diagonal, G = S^H S; strict lower part zeroed.  *flag set on a bad pivot.
+__device__ void sm_cholesky_upper(zdouble *G, int s, int *flag)
+{
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) {
+        const int a = e / s, b = e % s;
+        if (a < b) {
+            const zdouble u = G[a * s + b], l = G[b * s + a];
+            G[a * s + b] = {0.5 * (u.re + l.re), 0.5 * (u.im - l.im)};
+        }
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) {
+        const int a = e / s, b = e % s;
+        if (a > b) G[e] = {0.0, 0.0};
+        if (a == b) G[e].im = 0.0;
+    }
+    __syncthreads();
+    for (int a = 0; a < s; ++a) {
+        const double d = G[a * s + a].re;
+        if (!(d > 0.0) || !isfinite(d)) {
+            if (threadIdx.x == 0) *flag = 1;
+            __syncthreads();
+            return;
+        }
+        const double saa = sqrt(d);
+        __syncthreads();
+        for (int b = a + threadIdx.x; b < s; b += blockDim.x) {
+            if (b == a) G[a * s + a] = {saa, 0.0};
+            else { G[a * s + b].re /= saa; G[a * s + b].im /= saa; }
+        }
+        __syncthreads();
+        // trailing update of the upper triangle: G[c][b] -= conj(S[a][c]) S[a][b], a < c <= b
+        const int m = s - a - 1;
+        for (int e = threadIdx.x; e < m * m; e += blockDim.x) {
+            const int c = a + 1 + e / m, b = a + 1 + e % m;
+            if (b >= c) {
+                const zdouble t = zmulc(G[a * s + c], G[a * s + b]);
+                G[c * s + b].re -= t.re;
+                G[c * s + b].im -= t.im;
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Sinv = S^-1 for upper triangular S (thread b does column b by back substitution)
+__device__ void sm_upper_inverse(const zdouble *S, zdouble *Sinv, int s)
+{
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) Sinv[e] = {0.0, 0.0};
+    __syncthreads();
+    for (int b = threadIdx.x; b < s; b += blockDim.x) {
+        for (int a = b; a >= 0; --a) {
+            zdouble acc = {(a == b) ? 1.0 : 0.0, 0.0};
+            for (int c = a + 1; c <= b; ++c) {
+                const zdouble t = zmul(S[a * s + c], Sinv[c * s + b]);
+                acc.re -= t.re;
+                acc.im -= t.im;
+            }
+            const double d = S[a * s + a].re;       // real positive diagonal
+            Sinv[a * s + b] = {acc.re / d, acc.im / d};
+        }
+    }
+    __syncthreads();
+}
+
+// R = op(P) Q with op = identity (adjP = 0) or conjugate transpose (adjP = 1); R must not alias P or Q
+__device__ void sm_matmul(const zdouble *P, const zdouble *Q, zdouble *R, int s, int adjP, int adjQ)
+{
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) {
+        const int a = e / s, b = e % s;
+        double re = 0.0, im = 0.0;
+        for (int c = 0; c < s; ++c) {
+            zdouble p = adjP ? zdouble{P[c * s + a].re, -P[c * s + a].im} : P[a * s + c];
+            zdouble q = adjQ ? zdouble{Q[b * s + c].re, -Q[b * s + c].im} : Q[c * s + b];
+            re += p.re * q.re - p.im * q.im;
+            im += p.re * q.im + p.im * q.re;
+        }
+        R[e] = {re, im};
+    }
+    __syncthreads();
+}
+
+// G -> S (and optionally S^-1).  info: 0 or COARSE_BREAKDOWN.
+__global__ void small_cholesky_kernel(const zdouble *G, zdouble *S, zdouble *Sinv, int s, int32_t *info)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s;
+    __shared__ int flag;
+    if (threadIdx.x == 0) flag = 0;
+    sm_load(m0, G, s * s);
+    sm_cholesky_upper(m0, s, &flag);
+    __syncthreads();
+    if (flag) { if (threadIdx.x == 0) *info = COARSE_BREAKDOWN; return; }
+    sm_store(S, m0, s * s);
+    if (Sinv) { sm_upper_inverse(m0, m1, s); sm_store(Sinv, m1, s * s); }
+    if (threadIdx.x == 0) *info = 0;
+}
+
+// M = G^-1 = S^-1 S^-H
+__global__ void small_hpd_inverse_kernel(const zdouble *G, zdouble *M, int s, int32_t *info)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s;
+    __shared__ int flag;
+    if (threadIdx.x == 0) flag = 0;
+    sm_load(m0, G, s * s);
+    sm_cholesky_upper(m0, s, &flag);
+    __syncthreads();
+    if (flag) { if (threadIdx.x == 0) *info = COARSE_BREAKDOWN; return; }
+    sm_upper_inverse(m0, m1, s);
+    sm_matmul(m1, m1, m0, s, 0, 1);      // Sinv * Sinv^H
+    sm_store(M, m0, s * s);
+    if (threadIdx.x == 0) *info = 0;
+}
+
+// Device-resident scalars/matrices of one block-CG solve (all complex128 / double)
+struct BcgSmall {
+    zdouble *G;       // Gram result (input of every small kernel)
+    zdouble *C;       // C_k
+    zdouble *K1;      // M C    (X update coefficient)   | C_0^-1 at init
+    zdouble *K2;      // -M     (T = Q - Z M)
+    zdouble *K3;      // S^-1
+    zdouble *K4;      // S^H
+    double *bnorm;    // ||B[:,r]||  (1 where the source column is zero)
+    double *relres;   // [s] recursive relative residuals
+    double *stop;     // [0] = max_r relres, [1] = status flag (0 ok, 1 breakdown)
+};
+
+// bnorm[r] = sqrt(G[r][r]) from G = B^H B
+__global__ void bcg_bnorm_kernel(BcgSmall w, int s)
+{
+    for (int r = threadIdx.x; r < s; r += blockDim.x) {
+        const double v = sqrt(fmax(w.G[r * s + r].re, 0.0));
+        w.bnorm[r] = (v == 0.0) ? 1.0 : v;
+    }
+}
+
+// init: G = R^H R.  relres[r] = sqrt(G[r][r])/bnorm[r]; stop[0] = max; if max > tol: C = chol(G), K1 = C^-1
+__global__ void bcg_init_kernel(BcgSmall w, int s, double tol)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s;
+    __shared__ int flag;
+    __shared__ double worst;
+    if (threadIdx.x == 0) {
+        flag = 0;
+        double m = 0.0;
+        for (int r = 0; r < s; ++r) {
+            const double rel = sqrt(fmax(w.G[r * s + r].re, 0.0)) / w.bnorm[r];
+            w.relres[r] = rel;
+            m = fmax(m, rel);
+        }
+        worst = m;
+        w.stop[0] = m;
+        w.stop[1] = 0.0;
+    }
+    sm_load(m0, w.G, s * s);
+    if (worst <= tol) return;
+    sm_cholesky_upper(m0, s, &flag);
+    __syncthreads();
+    if (flag) { if (threadIdx.x == 0) w.stop[1] = 1.0; return; }
+    sm_store(w.C, m0, s * s);
+    sm_upper_inverse(m0, m1, s);
+    sm_store(w.K1, m1, s * s);
+}
+
+// step 1: G = D^H Z.  M = G^-1;  K1 = M C;  K2 = -M.
+__global__ void bcg_step1_kernel(BcgSmall w, int s)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s, *m2 = m1 + s * s;
+    __shared__ int flag;
+    if (threadIdx.x == 0) flag = 0;
+    sm_load(m0, w.G, s * s);
+    sm_cholesky_upper(m0, s, &flag);
+    __syncthreads();
+    if (flag) { if (threadIdx.x == 0) w.stop[1] = 1.0; return; }
+    sm_upper_inverse(m0, m1, s);
+    sm_matmul(m1, m1, m0, s, 0, 1);          // m0 = M
+    sm_load(m2, w.C, s * s);
+    sm_matmul(m0, m2, m1, s, 0, 0);          // m1 = M C
+    sm_store(w.K1, m1, s * s);
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) w.K2[e] = {-m0[e].re, -m0[e].im};
+}
+
+// step 2: G = T^H T.  S = chol(G);  K3 = S^-1;  K4 = S^H;  C <- S C;  relres, stop
+__global__ void bcg_step2_kernel(BcgSmall w, int s)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s, *m2 = m1 + s * s;
+    __shared__ int flag;
+    if (threadIdx.x == 0) flag = 0;
+    sm_load(m0, w.G, s * s);
+    sm_cholesky_upper(m0, s, &flag);
+    __syncthreads();
+    if (flag) { if (threadIdx.x == 0) w.stop[1] = 1.0; return; }
+    sm_upper_inverse(m0, m1, s);
+    sm_store(w.K3, m1, s * s);
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) {
+        const int a = e / s, b = e % s;
+        w.K4[e] = {m0[b * s + a].re, -m0[b * s + a].im};
+    }
+    sm_load(m2, w.C, s * s);
+    sm_matmul(m0, m2, m1, s, 0, 0);          // m1 = S C
+    sm_store(w.C, m1, s * s);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int r = 0; r < s; ++r) {
+            double acc = 0.0;
+            for (int a = 0; a < s; ++a) acc += m1[a * s + r].re * m1[a * s + r].re + m1[a * s + r].im * m1[a * s + r].im;
+            const double rel = sqrt(acc) / w.bnorm[r];
+            w.relres[r] = rel;
+            m = fmax(m, rel);
+        }
+        w.stop[0] = m;
+    }
+}
+
+// column norms of a block from the diagonal of its Gram matrix: out[r] = sqrt(G[r][r]) / bnorm[r]
+__global__ void bcg_truerel_kernel(BcgSmall w, int s, double *out)
+{
+    for (int r = threadIdx.x; r < s; r += blockDim.x) out[r] = sqrt(fmax(w.G[r * s + r].re, 0.0)) / w.bnorm[r];
+}
+
+}  // namespace cmrhs

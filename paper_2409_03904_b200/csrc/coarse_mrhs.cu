@@ -1,0 +1,713 @@
+// C ABI of the B200-native coarse multi-RHS operator and block CG (include/coarse_mrhs.h).
+// Host-side orchestration only: argument checks, kernel selection, launches.  All arithmetic of the
+// path runs in the CUDA kernels of this directory.  No CPU fallback exists.
+#include <chrono>
+#include <cstdarg>
+#include <cstring>
+#include <atomic>
+#include <new>
+
+#include "blockcg_kernels.cuh"
+#include "common.cuh"
+#include "setup_kernels.cuh"
+#include "stencil_generic.cuh"
+#include "stencil_simt.cuh"
+
+namespace cmrhs {
+
+thread_local char g_err[512] = "";
+static std::atomic<int64_t> g_launches{0};
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+// ---- tiled SIMT variants: (dtype, nbasis, nrhs) -> kernel ---------------------------------------------
+//                      T      NB TM TN GC SITES CB KSPLIT STAGES
+using V_f32_s64 = SimtConfig<float, 32, 4, 4, 4, 2, 4, 2, 6>;
+using V_f32_s32 = SimtConfig<float, 32, 4, 4, 4, 4, 2, 2, 5>;
+using V_f32_s16 = SimtConfig<float, 32, 4, 4, 4, 8, 1, 2, 4>;
+using V_f32_s8 = SimtConfig<float, 32, 4, 2, 4, 8, 1, 2, 5>;
+using V_f32_s4 = SimtConfig<float, 32, 4, 1, 4, 8, 1, 2, 5>;
+using V_f32_s1 = SimtConfig<float, 32, 1, 1, 1, 8, 1, 2, 5>;
+using V_f24_s64 = SimtConfig<float, 24, 6, 2, 8, 2, 4, 2, 8>;
+using V_f24_s16 = SimtConfig<float, 24, 6, 2, 8, 8, 1, 2, 6>;
+using V_d24_s8 = SimtConfig<double, 24, 3, 2, 4, 8, 1, 2, 4>;
+using V_d8_s4 = SimtConfig<double, 8, 1, 1, 4, 8, 1, 1, 8>;
+using V_d32_s16 = SimtConfig<double, 32, 4, 2, 4, 4, 2, 2, 4>;
+
+struct SimtVariant {
+    int dtype, nb, s;
+    const char *name;
+    int (*launch)(const void *, const int32_t *, const void *, void *, int64_t, int, cudaStream_t);
+};
+#define CMRHS_VARIANT(DT, CFG) {DT, CFG::NB, CFG::S, "stencil_simt<" #CFG ">", &launch_stencil_simt<CFG>}
+static const SimtVariant kSimtVariants[] = {
+    CMRHS_VARIANT(COARSE_C64, V_f32_s64), CMRHS_VARIANT(COARSE_C64, V_f32_s32), CMRHS_VARIANT(COARSE_C64, V_f32_s16),
+    CMRHS_VARIANT(COARSE_C64, V_f32_s8),  CMRHS_VARIANT(COARSE_C64, V_f32_s4),  CMRHS_VARIANT(COARSE_C64, V_f32_s1),
+    CMRHS_VARIANT(COARSE_C64, V_f24_s64), CMRHS_VARIANT(COARSE_C64, V_f24_s16), CMRHS_VARIANT(COARSE_C128, V_d24_s8),
+    CMRHS_VARIANT(COARSE_C128, V_d8_s4),  CMRHS_VARIANT(COARSE_C128, V_d32_s16),
+};
+
+static const SimtVariant *find_variant(int dtype, int nb, int s)
+{
+    for (const auto &v : kSimtVariants)
+        if (v.dtype == dtype && v.nb == nb && v.s == s) return &v;
+    return nullptr;
+}
+
+}  // namespace cmrhs
+
+using namespace cmrhs;
+
+// ---- the handle ---------------------------------------------------------------------------------------
+struct coarse_op {
+    LatticeDims dims;
+    int nb = 0, nrhs_max = 0, dtype = 0;
+    uint32_t flags = 0;
+    int num_sms = 0;
+    size_t esize = 0;            // bytes per complex element
+    void *At = nullptr;          // [V][81][nb(k)][nb(i)]
+    int32_t *nbr = nullptr;      // [V][81]
+    void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
+    zdouble *gram_partial = nullptr;
+    int gram_blocks = 0;
+    zdouble *small = nullptr;    // 6 s x s matrices
+    double *dscal = nullptr;     // bnorm[64] relres[64] stop[2] truerel[64]
+    int32_t *dinfo = nullptr;
+    double *hpin = nullptr;      // pinned host mirror of relres/stop/truerel
+    const void *bcg_B = nullptr; // state of a begin/step/end solve
+    void *bcg_X = nullptr;
+    int bcg_s = 0, bcg_its = 0;
+    bool bcg_active = false;
+    // optional per-launch timing of the stencil kernel (coarse_op_profile): event pairs recorded on the launch stream
+    bool prof_on = false;
+    int prof_n = 0;
+    cudaEvent_t prof_ev[2 * 64] = {};
+    int64_t device_bytes = 0;
+};
+
+static int alloc_dev(coarse_op *op, void **p, size_t bytes)
+{
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        set_error("cudaMalloc of %zu bytes failed: %s", bytes, cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? COARSE_OUT_OF_MEMORY : COARSE_CUDA_ERROR;
+    }
+    op->device_bytes += (int64_t)bytes;
+    return COARSE_OK;
+}
+
+static BcgSmall small_view(const coarse_op *op)
+{
+    const size_t m = (size_t)COARSE_MAX_NRHS * COARSE_MAX_NRHS;
+    BcgSmall w;
+    w.G = op->small;
+    w.C = op->small + m;
+    w.K1 = op->small + 2 * m;
+    w.K2 = op->small + 3 * m;
+    w.K3 = op->small + 4 * m;
+    w.K4 = op->small + 5 * m;
+    w.bnorm = op->dscal;
+    w.relres = op->dscal + 64;
+    w.stop = op->dscal + 128;
+    return w;
+}
+
+extern "C" const char *coarse_last_error(void) { return g_err; }
+extern "C" int64_t coarse_launch_count(void) { return g_launches.load(); }
+
+static int check_shape(const int32_t dims[4], int nb, int s, int dtype)
+{
+    if (!dims) { set_error("dims is NULL"); return COARSE_INVALID_ARG; }
+    for (int k = 0; k < 4; ++k)
+        if (dims[k] < 1) { set_error("dims[%d] = %d < 1", k, dims[k]); return COARSE_INVALID_ARG; }
+    if (dtype != COARSE_C64 && dtype != COARSE_C128) { set_error("unknown dtype %d", dtype); return COARSE_INVALID_ARG; }
+    if (nb < 1 || s < 1) { set_error("nbasis and nrhs must be >= 1"); return COARSE_INVALID_ARG; }
+    if (nb > COARSE_MAX_NBASIS || s > COARSE_MAX_NRHS) {
+        set_error("nbasis %d / nrhs %d outside the supported range (<= %d / <= %d)", nb, s, COARSE_MAX_NBASIS, COARSE_MAX_NRHS);
+        return COARSE_UNSUPPORTED;
+    }
+    const int64_t V = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
+    if (V > 0x7fffffffLL) { set_error("lattice volume %lld exceeds int32 site indices", (long long)V); return COARSE_UNSUPPORTED; }
+    return COARSE_OK;
+}
+
+extern "C" int coarse_op_destroy(coarse_op_t *op)
+{
+    if (!op) return COARSE_OK;
+    cudaFree(op->At);
+    cudaFree(op->nbr);
+    for (void *b : op->blk) cudaFree(b);
+    cudaFree(op->gram_partial);
+    cudaFree(op->small);
+    cudaFree(op->dscal);
+    cudaFree(op->dinfo);
+    if (op->hpin) cudaFreeHost(op->hpin);
+    for (cudaEvent_t e : op->prof_ev) if (e) cudaEventDestroy(e);
+    delete op;
+    return COARSE_OK;
+}
+
+extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_t nbasis, int32_t nrhs_max, int32_t dtype,
+                                const void *A_dev, uint32_t flags, void *stream_v)
+{
+    if (!out) { set_error("out is NULL"); return COARSE_INVALID_ARG; }
+    *out = nullptr;
+    int st = check_shape(dims, nbasis, nrhs_max, dtype);
+    if (st != COARSE_OK) return st;
+    if (!A_dev) { set_error("A_dev is NULL"); return COARSE_INVALID_ARG; }
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    int dev = 0;
+    CMRHS_CUDA(cudaGetDevice(&dev));
+    coarse_op *op = new (std::nothrow) coarse_op;
+    if (!op) { set_error("host allocation failed"); return COARSE_OUT_OF_MEMORY; }
+    for (int k = 0; k < 4; ++k) op->dims.L[k] = dims[k];
+    op->dims.V = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
+    op->nb = nbasis;
+    op->nrhs_max = nrhs_max;
+    op->dtype = dtype;
+    op->flags = flags;
+    op->esize = dtype == COARSE_C64 ? sizeof(cplx<float>) : sizeof(cplx<double>);
+    cudaError_t ce = cudaDeviceGetAttribute(&op->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (ce != cudaSuccess) { set_error("cudaDeviceGetAttribute: %s", cudaGetErrorString(ce)); delete op; return COARSE_CUDA_ERROR; }
+
+    const int64_t V = op->dims.V;
+    const int64_t ntiles = V * kNPoint;
+    const size_t a_bytes = (size_t)ntiles * nbasis * nbasis * op->esize;
+    const size_t blk_bytes = (size_t)V * nbasis * nrhs_max * op->esize;
+    op->gram_blocks = op->num_sms * 2;
+#define CMRHS_TRY(expr)                      \
+    do {                                     \
+        int _s = (expr);                     \
+        if (_s != COARSE_OK) {               \
+            coarse_op_destroy(op);           \
+            return _s;                       \
+        }                                    \
+    } while (0)
+    CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
+    CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
+    for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
+    CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
+    CMRHS_TRY(alloc_dev(op, (void **)&op->small, (size_t)6 * COARSE_MAX_NRHS * COARSE_MAX_NRHS * sizeof(zdouble)));
+    CMRHS_TRY(alloc_dev(op, (void **)&op->dscal, 256 * sizeof(double)));
+    CMRHS_TRY(alloc_dev(op, (void **)&op->dinfo, 4 * sizeof(int32_t)));
+    ce = cudaMallocHost((void **)&op->hpin, 256 * sizeof(double));
+    if (ce != cudaSuccess) { set_error("cudaMallocHost: %s", cudaGetErrorString(ce)); coarse_op_destroy(op); return COARSE_CUDA_ERROR; }
+#undef CMRHS_TRY
+
+    // a1: neighbour table, once ("The pointers are precomputed")
+    {
+        const int grid = (int)(ceil_div(ntiles, 256) < 65535 ? ceil_div(ntiles, 256) : 65535);
+        neighbour_table_kernel<<<grid, 256, 0, stream>>>(op->dims, op->nbr);
+        count_launch();
+    }
+    // re-layout A into k-major tiles
+    {
+        const int grid = (int)(ntiles < 1048576 ? ntiles : 1048576);
+        if (dtype == COARSE_C64)
+            relayout_transpose_kernel<float><<<grid, 128, 0, stream>>>((const cplx<float> *)A_dev, (cplx<float> *)op->At, ntiles, nbasis);
+        else
+            relayout_transpose_kernel<double><<<grid, 128, 0, stream>>>((const cplx<double> *)A_dev, (cplx<double> *)op->At, ntiles, nbasis);
+        count_launch();
+    }
+    ce = cudaGetLastError();
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(stream);
+    if (ce != cudaSuccess) {
+        set_error("operator setup kernels failed: %s", cudaGetErrorString(ce));
+        coarse_op_destroy(op);
+        return COARSE_CUDA_ERROR;
+    }
+    *out = op;
+    return COARSE_OK;
+}
+
+extern "C" int64_t coarse_op_device_bytes(const coarse_op_t *op) { return op ? op->device_bytes : 0; }
+
+static const SimtVariant *select_variant(const coarse_op *op, int nrhs)
+{
+    if (op->flags & COARSE_FLAG_FORCE_GENERIC) return nullptr;
+    return find_variant(op->dtype, op->nb, nrhs);
+}
+
+extern "C" const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs)
+{
+    if (!op) return "";
+    const SimtVariant *v = select_variant(op, nrhs);
+    return v ? v->name : (op->dtype == COARSE_C64 ? "stencil_generic<float>" : "stencil_generic<double>");
+}
+
+static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream);
+
+static int apply_impl(const coarse_op *op_c, const void *X, void *Y, int nrhs, cudaStream_t stream)
+{
+    coarse_op *op = const_cast<coarse_op *>(op_c);
+    if (!op->prof_on || op->prof_n >= 64) return apply_launch(op, X, Y, nrhs, stream);
+    const int k = op->prof_n;
+    CMRHS_CUDA(cudaEventRecord(op->prof_ev[2 * k], stream));
+    int st = apply_launch(op, X, Y, nrhs, stream);
+    CMRHS_CUDA(cudaEventRecord(op->prof_ev[2 * k + 1], stream));
+    op->prof_n = k + 1;
+    return st;
+}
+
+static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream)
+{
+    const SimtVariant *v = select_variant(op, nrhs);
+    if (v) return v->launch(op->At, op->nbr, X, Y, op->dims.V, op->num_sms, stream);
+    if (op->dtype == COARSE_C64)
+        return launch_stencil_generic<float>((const cplx<float> *)op->At, op->nbr, (const cplx<float> *)X, (cplx<float> *)Y,
+                                             op->dims.V, op->nb, nrhs, op->num_sms, stream);
+    return launch_stencil_generic<double>((const cplx<double> *)op->At, op->nbr, (const cplx<double> *)X, (cplx<double> *)Y,
+                                          op->dims.V, op->nb, nrhs, op->num_sms, stream);
+}
+
+static int check_apply_args(const coarse_op *op, const void *X, const void *Y, int nrhs)
+{
+    if (!op || !X || !Y) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..nrhs_max=%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (X == Y) { set_error("Y must not alias X"); return COARSE_INVALID_ARG; }
+    return COARSE_OK;
+}
+
+extern "C" int coarse_op_apply(const coarse_op_t *op, const void *X_dev, void *Y_dev, int32_t nrhs, void *stream)
+{
+    int st = check_apply_args(op, X_dev, Y_dev, nrhs);
+    if (st != COARSE_OK) return st;
+    return apply_impl(op, X_dev, Y_dev, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int coarse_op_apply_host(coarse_op_t *op, const void *X_host, void *Y_host, int32_t nrhs, void *stream_v)
+{
+    int st = check_apply_args(op, X_host, Y_host, nrhs);
+    if (st != COARSE_OK) return st;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    const size_t bytes = (size_t)op->dims.V * op->nb * nrhs * op->esize;
+    CMRHS_CUDA(cudaMemcpyAsync(op->blk[4], X_host, bytes, cudaMemcpyHostToDevice, stream));
+    st = apply_impl(op, op->blk[4], op->blk[5], nrhs, stream);
+    if (st != COARSE_OK) return st;
+    CMRHS_CUDA(cudaMemcpyAsync(Y_host, op->blk[5], bytes, cudaMemcpyDeviceToHost, stream));
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    return COARSE_OK;
+}
+
+// ---- block-CG building blocks --------------------------------------------------------------------------
+template <typename T>
+static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble *G, int64_t n, int s, cudaStream_t stream)
+{
+    const int TT = (s + 15) / 16;
+    const int nt = (s + TT - 1) / TT;
+    const int RG = kLaThreads / (nt * nt);
+    int rows = (int)(40960 / (2 * (size_t)s * sizeof(cplx<T>)));
+    rows = rows / RG * RG;
+    if (rows < RG) rows = RG;
+    size_t smem = (size_t)rows * s * 2 * sizeof(cplx<T>);
+    if (RG > 1 && smem < (size_t)s * s * sizeof(zdouble)) smem = (size_t)s * s * sizeof(zdouble);
+    int blocks = op->gram_blocks;
+    if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
+    if (blocks < 1) blocks = 1;
+    const cplx<T> *u = (const cplx<T> *)U, *w = (const cplx<T> *)W;
+#define CMRHS_GRAM_CASE(TTV)                                                                                     \
+    {                                                                                                            \
+        auto kern = gram_partial_kernel<T, TTV>;                                                                 \
+        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152))); \
+        kern<<<blocks, kLaThreads, smem, stream>>>(u, w, n, s, rows, op->gram_partial);                          \
+    }
+    switch (TT) {
+    case 1: CMRHS_GRAM_CASE(1) break;
+    case 2: CMRHS_GRAM_CASE(2) break;
+    case 3: CMRHS_GRAM_CASE(3) break;
+    default: CMRHS_GRAM_CASE(4) break;
+    }
+#undef CMRHS_GRAM_CASE
+    CMRHS_LAUNCH_CHECK();
+    gram_reduce_kernel<<<(s * s + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, s * s, G);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+static int gram_dispatch(const coarse_op *op, const void *U, const void *W, zdouble *G, int64_t n, int s, cudaStream_t stream)
+{
+    return op->dtype == COARSE_C64 ? gram_impl<float>(op, U, W, G, n, s, stream) : gram_impl<double>(op, U, W, G, n, s, stream);
+}
+
+template <typename T>
+static int rotate_impl(const coarse_op *op, const void *U, const zdouble *K, const void *Vin, void *out, double beta, int64_t n,
+                       int s, cudaStream_t stream)
+{
+    const int TC = (s + 15) / 16;
+    const int ncg = (s + TC - 1) / TC;
+    const int RL = kLaThreads / ncg;
+    int rows = RL * 4;
+    const size_t smem = ((size_t)s * s + (size_t)rows * (s + 1)) * sizeof(cplx<T>);
+    const int64_t ntiles = ceil_div(n, rows);
+    const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
+#define CMRHS_ROT_CASE(TCV)                                                                                      \
+    {                                                                                                            \
+        auto kern = rotate_kernel<T, TCV>;                                                                       \
+        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152))); \
+        kern<<<grid, kLaThreads, smem, stream>>>((const cplx<T> *)U, K, (const cplx<T> *)Vin, (cplx<T> *)out, (T)beta, n, s, rows); \
+    }
+    switch (TC) {
+    case 1: CMRHS_ROT_CASE(1) break;
+    case 2: CMRHS_ROT_CASE(2) break;
+    case 3: CMRHS_ROT_CASE(3) break;
+    default: CMRHS_ROT_CASE(4) break;
+    }
+#undef CMRHS_ROT_CASE
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+static int rotate_dispatch(const coarse_op *op, const void *U, const zdouble *K, const void *Vin, void *out, double beta, int64_t n,
+                           int s, cudaStream_t stream)
+{
+    return op->dtype == COARSE_C64 ? rotate_impl<float>(op, U, K, Vin, out, beta, n, s, stream)
+                                   : rotate_impl<double>(op, U, K, Vin, out, beta, n, s, stream);
+}
+
+static int axpby_dispatch(const coarse_op *op, const void *U, const void *W, void *out, double a, double b, int64_t total,
+                          cudaStream_t stream)
+{
+    const int grid = (int)(ceil_div(total, 256) < (int64_t)op->num_sms * 16 ? ceil_div(total, 256) : (int64_t)op->num_sms * 16);
+    if (op->dtype == COARSE_C64)
+        axpby_kernel<float><<<grid, 256, 0, stream>>>((const cplx<float> *)U, (const cplx<float> *)W, (cplx<float> *)out, (float)a, (float)b, total);
+    else
+        axpby_kernel<double><<<grid, 256, 0, stream>>>((const cplx<double> *)U, (const cplx<double> *)W, (cplx<double> *)out, a, b, total);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+static int small_smem_attr(const void *kern, int s, int nmat, size_t *smem)
+{
+    *smem = (size_t)nmat * s * s * sizeof(zdouble);
+    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(*smem > 49152 ? *smem : 49152)));
+    return COARSE_OK;
+}
+
+extern "C" int coarse_block_gram(coarse_op_t *op, const void *U_dev, const void *W_dev, void *G_dev, int64_t n, int32_t s, void *stream)
+{
+    if (!op || !U_dev || !W_dev || !G_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (s < 1 || s > op->nrhs_max || n < 1) { set_error("bad n/s"); return COARSE_INVALID_ARG; }
+    return gram_dispatch(op, U_dev, W_dev, (zdouble *)G_dev, n, s, (cudaStream_t)stream);
+}
+
+extern "C" int coarse_block_rotate(coarse_op_t *op, const void *U_dev, const void *K_dev, void *W_dev, double beta, int64_t n, int32_t s,
+                                   void *stream)
+{
+    if (!op || !U_dev || !K_dev || !W_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (s < 1 || s > COARSE_MAX_NRHS || n < 1) { set_error("bad n/s"); return COARSE_INVALID_ARG; }
+    if (U_dev == W_dev) { set_error("W must not alias U"); return COARSE_INVALID_ARG; }
+    return rotate_dispatch(op, U_dev, (const zdouble *)K_dev, W_dev, W_dev, beta, n, s, (cudaStream_t)stream);
+}
+
+extern "C" int coarse_small_cholesky(const void *G_dev, void *S_dev, void *Sinv_dev, int32_t s, int32_t *info_dev, void *stream)
+{
+    if (!G_dev || !S_dev || !info_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (s < 1 || s > COARSE_MAX_NRHS) { set_error("bad s"); return COARSE_INVALID_ARG; }
+    size_t smem;
+    int st = small_smem_attr((const void *)small_cholesky_kernel, s, 2, &smem);
+    if (st != COARSE_OK) return st;
+    small_cholesky_kernel<<<1, kLaThreads, smem, (cudaStream_t)stream>>>((const zdouble *)G_dev, (zdouble *)S_dev, (zdouble *)Sinv_dev, s, info_dev);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+extern "C" int coarse_small_hpd_inverse(const void *G_dev, void *M_dev, int32_t s, int32_t *info_dev, void *stream)
+{
+    if (!G_dev || !M_dev || !info_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (s < 1 || s > COARSE_MAX_NRHS) { set_error("bad s"); return COARSE_INVALID_ARG; }
+    size_t smem;
+    int st = small_smem_attr((const void *)small_hpd_inverse_kernel, s, 2, &smem);
+    if (st != COARSE_OK) return st;
+    small_hpd_inverse_kernel<<<1, kLaThreads, smem, (cudaStream_t)stream>>>((const zdouble *)G_dev, (zdouble *)M_dev, s, info_dev);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+// ---- BlockCGrQ (Fig. 2 left) ----------------------------------------------------------
+static int small_launch(void (*kern)(BcgSmall, int), const coarse_op *op, int s, int nmat, cudaStream_t stream)
+{
+    size_t smem;
+    int st = small_smem_attr((const void *)kern, s, nmat, &smem);
+    if (st != COARSE_OK) return st;
+    kern<<<1, kLaThreads, smem, stream>>>(small_view(op), s);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+// copies relres[64] | stop[2] | truerel[64] (device doubles 64..193) to the pinned mirror and synchronises
+static int fetch_scalars(const coarse_op *op, cudaStream_t stream)
+{
+    CMRHS_CUDA(cudaMemcpyAsync(op->hpin, op->dscal + 64, 130 * sizeof(double), cudaMemcpyDeviceToHost, stream));
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    return COARSE_OK;
+}
+
+#define CMRHS_STEP(expr)                   \
+    do {                                   \
+        int _s = (expr);                   \
+        if (_s != COARSE_OK) return _s;    \
+    } while (0)
+
+// The solve is split into begin / step / poll / end so that a caller (bench.py) can time exactly K iterations
+// on the device without the per-iteration host read of block_cg_solve.  State lives in the handle.
+static int bcg_begin(coarse_op *op, const void *B, void *X, int s, double tol, cudaStream_t stream)
+{
+    const int64_t n = op->dims.V * op->nb, total = n * s;
+    const size_t blk_bytes = (size_t)total * op->esize;
+    void *Q = op->blk[0], *D = op->blk[1], *Z = op->blk[2], *T = op->blk[3];
+    BcgSmall w = small_view(op);
+    op->bcg_B = B; op->bcg_X = X; op->bcg_s = s; op->bcg_its = 0; op->bcg_active = false;
+    // ||B[:,r]||
+    CMRHS_STEP(gram_dispatch(op, B, B, w.G, n, s, stream));
+    bcg_bnorm_kernel<<<1, 64, 0, stream>>>(w, s);
+    CMRHS_LAUNCH_CHECK();
+    // R_0 = B - H X_0  (held in T)
+    CMRHS_STEP(apply_impl(op, X, Z, s, stream));
+    CMRHS_STEP(axpby_dispatch(op, B, Z, T, 1.0, -1.0, total, stream));
+    // Q_0 C_0 = R_0 by Cholesky of R^H R
+    CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));
+    {
+        size_t smem;
+        CMRHS_STEP(small_smem_attr((const void *)bcg_init_kernel, s, 2, &smem));
+        bcg_init_kernel<<<1, kLaThreads, smem, stream>>>(w, s, tol);
+        CMRHS_LAUNCH_CHECK();
+    }
+    CMRHS_STEP(fetch_scalars(op, stream));
+    const double *h_stop = op->hpin + 64;
+    if (h_stop[1] != 0.0) return COARSE_BREAKDOWN;
+    if (h_stop[0] <= tol) return COARSE_OK;                                             // X_0 already solves the system
+    CMRHS_STEP(rotate_dispatch(op, T, w.K1, nullptr, Q, 0.0, n, s, stream));           // Q_0 = R_0 C_0^-1
+    CMRHS_CUDA(cudaMemcpyAsync(D, Q, blk_bytes, cudaMemcpyDeviceToDevice, stream));    // D_0 = Q_0
+    op->bcg_active = true;
+    return COARSE_NOT_CONVERGED;
+}
+
+// one iteration k -> k+1 of Fig. 2 (left), statements 8-13; asynchronous, no host read
+static int bcg_step(coarse_op *op, cudaStream_t stream)
+{
+    const int s = op->bcg_s;
+    const int64_t n = op->dims.V * op->nb;
+    void *Q = op->blk[0], *D = op->blk[1], *Z = op->blk[2], *T = op->blk[3], *X = op->bcg_X;
+    BcgSmall w = small_view(op);
+    CMRHS_STEP(apply_impl(op, D, Z, s, stream));                                   // Z_k = H D_k
+    CMRHS_STEP(gram_dispatch(op, D, Z, w.G, n, s, stream));                        // D^H Z
+    CMRHS_STEP(small_launch(bcg_step1_kernel, op, s, 3, stream));                  // M, K1 = M C, K2 = -M
+    CMRHS_STEP(rotate_dispatch(op, D, w.K1, X, X, 1.0, n, s, stream));             // X += D M C
+    CMRHS_STEP(rotate_dispatch(op, Z, w.K2, Q, T, 1.0, n, s, stream));             // T = Q - Z M
+    CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));                        // T^H T
+    CMRHS_STEP(small_launch(bcg_step2_kernel, op, s, 3, stream));                  // S, K3 = S^-1, K4 = S^H, C = S C
+    CMRHS_STEP(rotate_dispatch(op, T, w.K3, nullptr, Q, 0.0, n, s, stream));       // Q = T S^-1
+    CMRHS_STEP(rotate_dispatch(op, D, w.K4, Q, D, 1.0, n, s, stream));             // D = Q + D S^H
+    op->bcg_its += 1;
+    return COARSE_OK;
+}
+
+// true residual from one extra apply; fills res (iterations, residuals); synchronises
+static int bcg_end(coarse_op *op, block_cg_result *res, cudaStream_t stream)
+{
+    const int s = op->bcg_s;
+    const int64_t n = op->dims.V * op->nb, total = n * s;
+    void *Z = op->blk[2], *T = op->blk[3];
+    BcgSmall w = small_view(op);
+    CMRHS_STEP(apply_impl(op, op->bcg_X, Z, s, stream));
+    CMRHS_STEP(axpby_dispatch(op, op->bcg_B, Z, T, 1.0, -1.0, total, stream));
+    CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));
+    bcg_truerel_kernel<<<1, 64, 0, stream>>>(w, s, op->dscal + 130);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(fetch_scalars(op, stream));
+    for (int r = 0; r < s; ++r) {
+        res->rel_res_recursive[r] = op->hpin[r];
+        res->rel_res_true[r] = op->hpin[66 + r];
+    }
+    res->iterations = op->bcg_its;
+    op->bcg_active = false;
+    return COARSE_OK;
+}
+
+static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double tol, int maxiter, block_cg_result *res,
+                         cudaStream_t stream)
+{
+    const double *h_stop = op->hpin + 64;
+    memset(res, 0, sizeof(*res));
+    for (int k = 0; k < COARSE_MAX_HISTORY; ++k) res->history[k] = -1.0;
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    const auto t0 = std::chrono::steady_clock::now();
+    int status = bcg_begin(op, B, X, s, tol, stream);
+    if (status != COARSE_OK && status != COARSE_NOT_CONVERGED && status != COARSE_BREAKDOWN) return status;
+    res->history[0] = h_stop[0];
+    if (status == COARSE_NOT_CONVERGED) {
+        for (int k = 0; k < maxiter; ++k) {
+            CMRHS_STEP(bcg_step(op, stream));
+            CMRHS_STEP(fetch_scalars(op, stream));                                         // stop scalar -> host
+            if (h_stop[1] != 0.0) { status = COARSE_BREAKDOWN; break; }
+            if (op->bcg_its < COARSE_MAX_HISTORY) res->history[op->bcg_its] = h_stop[0];
+            if (h_stop[0] <= tol) { status = COARSE_OK; break; }
+        }
+    }
+    CMRHS_STEP(bcg_end(op, res, stream));
+    res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    res->status = status;
+    return status;
+}
+
+static int check_solve_args(const coarse_op *op, const void *B, const void *X, int nrhs, double tol, int maxiter,
+                            const block_cg_result *res)
+{
+    if (!op || !B || !X || !res) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..nrhs_max=%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (!(tol > 0.0) || maxiter < 0) { set_error("tol must be > 0 and maxiter >= 0"); return COARSE_INVALID_ARG; }
+    if (B == X) { set_error("X must not alias B"); return COARSE_INVALID_ARG; }
+    return COARSE_OK;
+}
+
+extern "C" int block_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
+                              block_cg_result *res, void *stream)
+{
+    int st = check_solve_args(op, B_dev, X_dev, nrhs, tol, maxiter, res);
+    if (st != COARSE_OK) return st;
+    return block_cg_impl(op, B_dev, X_dev, nrhs, tol, maxiter, res, (cudaStream_t)stream);
+}
+
+extern "C" int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
+                                   int32_t maxiter, block_cg_result *res, void *stream_v)
+{
+    int st = check_solve_args(op, B_host, X_host, nrhs, tol, maxiter, res);
+    if (st != COARSE_OK) return st;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    const size_t bytes = (size_t)op->dims.V * op->nb * nrhs * op->esize;
+    CMRHS_CUDA(cudaMemcpyAsync(op->blk[4], B_host, bytes, cudaMemcpyHostToDevice, stream));
+    CMRHS_CUDA(cudaMemcpyAsync(op->blk[5], X_host, bytes, cudaMemcpyHostToDevice, stream));
+    st = block_cg_impl(op, op->blk[4], op->blk[5], nrhs, tol, maxiter, res, stream);
+    if (st != COARSE_OK && st != COARSE_NOT_CONVERGED) return st;
+    CMRHS_CUDA(cudaMemcpyAsync(X_host, op->blk[5], bytes, cudaMemcpyDeviceToHost, stream));
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    return st;
+}
+
+// ---- synthetic inputs (bench convenience) --------------------------------
+template <typename T>
+static int fill_synthetic_impl(void *A_dev, const LatticeDims &d, int nb, uint64_t seed, double c_factor, double *c_out,
+                               cudaStream_t stream)
+{
+    const int64_t total = d.V * kNPoint * nb * nb;
+    const int grid = (int)(ceil_div(total, 256) < 148 * 32 ? ceil_div(total, 256) : 148 * 32);
+    synth_fill_kernel<T><<<grid, 256, 0, stream>>>((cplx<T> *)A_dev, d, nb, synth_key(seed, SYNTH_TAG_A), synth_key(seed, SYNTH_TAG_G));
+    CMRHS_LAUNCH_CHECK();
+    double c = 0.0;
+    if (c_factor != 0.0) {
+        double *bound = nullptr;
+        CMRHS_CUDA(cudaMalloc((void **)&bound, (size_t)(d.V + 1) * sizeof(double)));
+        const int bgrid = (int)(ceil_div(d.V * 32, 256) < 148 * 16 ? ceil_div(d.V * 32, 256) : 148 * 16);
+        synth_bound_kernel<T><<<bgrid, 256, 0, stream>>>((const cplx<T> *)A_dev, d.V, nb, bound);
+        count_launch();
+        max_reduce_kernel<<<1, 256, 0, stream>>>(bound, d.V, bound + d.V);
+        count_launch();
+        double best = 0.0;
+        cudaError_t e = cudaMemcpyAsync(&best, bound + d.V, sizeof(double), cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        cudaFree(bound);
+        if (e != cudaSuccess) { set_error("synthetic bound pass failed: %s", cudaGetErrorString(e)); return COARSE_CUDA_ERROR; }
+        c = (double)(float)(c_factor * best);
+        const int sgrid = (int)ceil_div(d.V * nb, 256);
+        synth_shift_kernel<T><<<sgrid, 256, 0, stream>>>((cplx<T> *)A_dev, d.V, nb, (float)c);
+        CMRHS_LAUNCH_CHECK();
+    }
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    if (c_out) *c_out = c;
+    return COARSE_OK;
+}
+
+extern "C" int coarse_op_fill_synthetic(void *A_dev, const int32_t dims[4], int32_t nbasis, int32_t dtype, uint64_t seed,
+                                        double c_factor, double *c_out, void *stream)
+{
+    int st = check_shape(dims, nbasis, 1, dtype);
+    if (st != COARSE_OK) return st;
+    if (!A_dev) { set_error("A_dev is NULL"); return COARSE_INVALID_ARG; }
+    LatticeDims d;
+    for (int k = 0; k < 4; ++k) d.L[k] = dims[k];
+    d.V = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
+    return dtype == COARSE_C64 ? fill_synthetic_impl<float>(A_dev, d, nbasis, seed, c_factor, c_out, (cudaStream_t)stream)
+                               : fill_synthetic_impl<double>(A_dev, d, nbasis, seed, c_factor, c_out, (cudaStream_t)stream);
+}
+
+extern "C" int coarse_fill_block(void *X_dev, const int32_t dims[4], int32_t nbasis, int32_t nrhs, int32_t dtype, uint64_t seed,
+                                 int32_t tag, void *stream_v)
+{
+    int st = check_shape(dims, nbasis, nrhs, dtype);
+    if (st != COARSE_OK) return st;
+    if (!X_dev) { set_error("X_dev is NULL"); return COARSE_INVALID_ARG; }
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    const int64_t total = (int64_t)dims[0] * dims[1] * dims[2] * dims[3] * nbasis * nrhs;
+    const int grid = (int)(ceil_div(total, 256) < 148 * 32 ? ceil_div(total, 256) : 148 * 32);
+    const uint64_t key = synth_key(seed, (uint64_t)tag);
+    if (dtype == COARSE_C64) synth_block_kernel<float><<<grid, 256, 0, stream>>>((cplx<float> *)X_dev, total, key);
+    else synth_block_kernel<double><<<grid, 256, 0, stream>>>((cplx<double> *)X_dev, total, key);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+extern "C" int block_cg_begin(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, double *rel_res0,
+                              void *stream)
+{
+    block_cg_result dummy;
+    int st = check_solve_args(op, B_dev, X_dev, nrhs, tol, 0, &dummy);
+    if (st != COARSE_OK) return st;
+    st = bcg_begin(op, B_dev, X_dev, nrhs, tol, (cudaStream_t)stream);
+    if (rel_res0 && (st == COARSE_OK || st == COARSE_NOT_CONVERGED)) *rel_res0 = op->hpin[64];
+    return st;
+}
+
+extern "C" int block_cg_step(coarse_op_t *op, int32_t count, void *stream)
+{
+    if (!op || count < 0) { set_error("bad argument"); return COARSE_INVALID_ARG; }
+    if (!op->bcg_active) { set_error("block_cg_step without an active block_cg_begin"); return COARSE_INVALID_ARG; }
+    for (int k = 0; k < count; ++k) CMRHS_STEP(bcg_step(op, (cudaStream_t)stream));
+    return COARSE_OK;
+}
+
+extern "C" int block_cg_end(coarse_op_t *op, block_cg_result *res, void *stream)
+{
+    if (!op || !res) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (!op->bcg_B) { set_error("block_cg_end without block_cg_begin"); return COARSE_INVALID_ARG; }
+    memset(res, 0, sizeof(*res));
+    for (int k = 0; k < COARSE_MAX_HISTORY; ++k) res->history[k] = -1.0;
+    CMRHS_STEP(bcg_end(op, res, (cudaStream_t)stream));
+    double worst = 0.0;
+    for (int r = 0; r < op->bcg_s; ++r) worst = worst > res->rel_res_recursive[r] ? worst : res->rel_res_recursive[r];
+    if (op->bcg_its < COARSE_MAX_HISTORY) res->history[op->bcg_its] = worst;
+    res->status = op->hpin[65] != 0.0 ? COARSE_BREAKDOWN : COARSE_OK;
+    return res->status;
+}
+
+// ---- per-launch timing of the stencil kernel, for bench.py's roofline object --------------------------------
+extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)
+{
+    if (!op) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (enable && !op->prof_ev[0])
+        for (cudaEvent_t &e : op->prof_ev) CMRHS_CUDA(cudaEventCreate(&e));
+    op->prof_on = enable != 0;
+    op->prof_n = 0;
+    return COARSE_OK;
+}
+
+extern "C" int coarse_op_profile_read(coarse_op_t *op, double *ms, int32_t capacity, int32_t *count)
+{
+    if (!op || !ms || !count) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    int n = op->prof_n < capacity ? op->prof_n : capacity;
+    for (int k = 0; k < n; ++k) {
+        CMRHS_CUDA(cudaEventSynchronize(op->prof_ev[2 * k + 1]));
+        float t = 0.f;
+        CMRHS_CUDA(cudaEventElapsedTime(&t, op->prof_ev[2 * k], op->prof_ev[2 * k + 1]));
+        ms[k] = (double)t;
+    }
+    *count = n;
+    op->prof_n = 0;
+    return COARSE_OK;
+}

@@ -1,0 +1,68 @@
+// Shared device/host helpers of the CUDA path (no code is shared with oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/coarse_mrhs.h"
+
+namespace cmrhs {
+
+constexpr int kNPoint = 81;   // all relative shifts (-1..1)^4
+constexpr int kCentre = 40;
+
+// ---- error plumbing -------------------------------------------------------------------------------
+void set_error(const char *fmt, ...);
+extern thread_local char g_err[512];
+void count_launch(int n = 1);
+
+#define CMRHS_CUDA(expr)                                                                         \
+    do {                                                                                         \
+        cudaError_t _e = (expr);                                                                 \
+        if (_e != cudaSuccess) {                                                                 \
+            cmrhs::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__,   \
+                             __LINE__);                                                          \
+            return (_e == cudaErrorMemoryAllocation) ? COARSE_OUT_OF_MEMORY : COARSE_CUDA_ERROR; \
+        }                                                                                        \
+    } while (0)
+
+#define CMRHS_LAUNCH_CHECK()                                                                     \
+    do {                                                                                         \
+        cmrhs::count_launch();                                                                   \
+        cudaError_t _e = cudaGetLastError();                                                     \
+        if (_e != cudaSuccess) {                                                                 \
+            cmrhs::set_error("kernel launch failed: %s (%s:%d)", cudaGetErrorString(_e),         \
+                             __FILE__, __LINE__);                                                \
+            return COARSE_CUDA_ERROR;                                                            \
+        }                                                                                        \
+    } while (0)
+
+// ---- complex scalar helpers -------------------------------------------------------------------------
+template <typename T> struct cplx;           // T = float / double
+template <> struct __align__(8) cplx<float> { float re, im; };
+template <> struct __align__(16) cplx<double> { double re, im; };
+
+template <typename T>
+__device__ __forceinline__ void cmac(cplx<T> &acc, const cplx<T> &a, const cplx<T> &b)
+{   // acc += a * b   (4 fused multiply-adds)
+    acc.re = fma(a.re, b.re, acc.re);
+    acc.re = fma(-a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im);
+    acc.im = fma(a.im, b.re, acc.im);
+}
+
+template <typename T>
+__device__ __forceinline__ void cmac_conj(cplx<T> &acc, const cplx<T> &a, const cplx<T> &b)
+{   // acc += conj(a) * b
+    acc.re = fma(a.re, b.re, acc.re);
+    acc.re = fma(a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im);
+    acc.im = fma(-a.im, b.re, acc.im);
+}
+
+struct zdouble { double re, im; };   // s x s matrices are always complex128
+
+__host__ __device__ __forceinline__ int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+}  // namespace cmrhs

@@ -51,6 +51,19 @@ def test_gram_matches_numpy():
 
 
 # --- the solve against a dense direct solve (BASELINE.json configs[0]) -------------------------------------
+def test_block_rotate_matches_numpy_matmul():
+    # pin: library routine (numpy matmul) for W = beta W + U K
+    rng = np.random.default_rng(11)
+    n, s = 301, 5
+    U = rng.standard_normal((n, s)) + 1j * rng.standard_normal((n, s))
+    W = rng.standard_normal((n, s)) + 1j * rng.standard_normal((n, s))
+    K = rng.standard_normal((s, s)) + 1j * rng.standard_normal((s, s))
+    for beta in (0.0, 1.0, -0.5):
+        out = oracle.block_rotate(U, K, W, beta)
+        ref = beta * W + U @ K
+        assert np.linalg.norm(out - ref) <= 1e-14 * np.linalg.norm(ref)
+
+
 def test_block_cg_matches_dense_solve(cfg1, cfg1_dense):
     dims, A, B = cfg1["dims"], cfg1["A"], cfg1["B"]
     V, nb, s = B.shape
