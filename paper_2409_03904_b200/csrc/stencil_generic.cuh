@@ -35,7 +35,8 @@ stencil_generic_kernel(const cplx<T> *__restrict__ At, const int32_t *__restrict
         cplx<T> acc[MAXOUT];
 #pragma unroll
         for (int o = 0; o < MAXOUT; ++o) { acc[o].re = 0; acc[o].im = 0; }
-        for (int p = 0; p < kNPoint; ++p) {
+        for (int q = 0; q < kNPoint; ++q) {
+            const int p = stencil_point_in_order(q);
             const int64_t y = nbr[x * kNPoint + p];
             const cplx<T> *a = At + (x * kNPoint + p) * (int64_t)nn;
             const cplx<T> *xin = X + y * (int64_t)ns;

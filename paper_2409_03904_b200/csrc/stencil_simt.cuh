@@ -174,10 +174,11 @@ stencil_simt_kernel(const cplx<typename C::real> *__restrict__ At, const int32_t
                 if (x >= V) x = V - 1;                       // tail group: duplicate the last site (its Y store is skipped)
                 const int32_t *nrow = nbr + x * kNPoint;
                 const Z *arow = At + x * (int64_t)kNPoint * NN;
-                int32_t ynext = nrow[0];
-                for (int p = 0; p < kNPoint; ++p) {
+                int32_t ynext = nrow[stencil_point_in_order(0)];
+                for (int q = 0; q < kNPoint; ++q) {
+                    const int p = stencil_point_in_order(q);
                     const int64_t y = ynext;
-                    if (p + 1 < kNPoint) ynext = nrow[p + 1];
+                    if (q + 1 < kNPoint) ynext = nrow[stencil_point_in_order(q + 1)];
 #pragma unroll
                     for (int h = 0; h < C::KSPLIT; ++h, ++it) {
                         const uint32_t st = it % C::STAGES, round = it / C::STAGES;
