@@ -28,18 +28,18 @@ void set_error(const char *fmt, ...)
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 // ---- tiled SIMT variants: (dtype, nbasis, nrhs) -> kernel ---------------------------------------------
-//                      T      NB TM TN GC SITES CB KSPLIT STAGES
-using V_f32_s64 = SimtConfig<float, 32, 4, 4, 4, 2, 4, 2, 6>;
-using V_f32_s32 = SimtConfig<float, 32, 4, 4, 4, 4, 2, 2, 5>;
-using V_f32_s16 = SimtConfig<float, 32, 4, 4, 4, 8, 1, 2, 4>;
-using V_f32_s8 = SimtConfig<float, 32, 4, 2, 4, 8, 1, 2, 5>;
-using V_f32_s4 = SimtConfig<float, 32, 4, 1, 4, 8, 1, 2, 5>;
-using V_f32_s1 = SimtConfig<float, 32, 1, 1, 1, 8, 1, 2, 5>;
-using V_f24_s64 = SimtConfig<float, 24, 6, 2, 8, 2, 4, 2, 8>;
-using V_f24_s16 = SimtConfig<float, 24, 6, 2, 8, 8, 1, 2, 6>;
-using V_d24_s8 = SimtConfig<double, 24, 3, 2, 4, 8, 1, 2, 4>;
-using V_d8_s4 = SimtConfig<double, 8, 1, 1, 4, 8, 1, 1, 8>;
-using V_d32_s16 = SimtConfig<double, 32, 4, 2, 4, 4, 2, 2, 4>;
+//                      T      NB TM TN GC KSPLIT STAGES WARPS
+using V_f32_s64 = SimtConfig<float, 32, 8, 8, 8, 4, 4, 8>;
+using V_f32_s32 = SimtConfig<float, 32, 8, 4, 8, 4, 4, 12>;
+using V_f32_s16 = SimtConfig<float, 32, 4, 4, 4, 4, 4, 16>;
+using V_f32_s8 = SimtConfig<float, 32, 4, 2, 4, 4, 5, 16>;
+using V_f32_s4 = SimtConfig<float, 32, 4, 1, 4, 4, 5, 16>;
+using V_f32_s1 = SimtConfig<float, 32, 1, 1, 1, 4, 6, 16>;
+using V_f24_s64 = SimtConfig<float, 24, 6, 8, 8, 3, 5, 8>;
+using V_f24_s16 = SimtConfig<float, 24, 6, 2, 8, 3, 5, 16>;
+using V_d24_s8 = SimtConfig<double, 24, 3, 2, 4, 3, 3, 16>;
+using V_d8_s4 = SimtConfig<double, 8, 1, 1, 4, 1, 8, 16>;
+using V_d32_s16 = SimtConfig<double, 32, 4, 4, 4, 4, 4, 8>;
 
 struct SimtVariant {
     int dtype, nb, s;

@@ -2,15 +2,20 @@
 //   Y(x) = sum_{p=0}^{80} A^p(x) . X(x + delta_p)                       (Eq. 19)
 //
 // B200 design:
-//  * persistent CTAs, one per SM; a CTA works on groups of SITES consecutive lattice sites at a time;
-//  * a producer warp streams the stencil matrices A^p(x) (k-major tiles, the dominant HBM stream) and the
-//    neighbours' X tiles into a STAGES-deep shared-memory ring with 1-D bulk TMA copies
-//    (cp.async.bulk + mbarrier complete_tx), A with an L2 evict-first policy, X with evict-last;
-//  * SITES*CB consumer warps: warp (site, column block) owns the NB x CT block of Y(site) in registers
-//    (TM x TN complex accumulators per thread) for all 81 stencil points -- every A element fetched from
-//    HBM is reused across all nrhs columns on chip and Y is written exactly once (the paper's formulation
-//    does 81 read-modify-writes of C);
-//  * full/empty mbarriers per stage, no __syncthreads in the main loop.
+//  * persistent CTAs, one per SM, WARPS warps each; every WARP owns whole lattice sites: warp w of the grid
+//    handles sites w, w + W_total, w + 2 W_total, ...  and keeps the full NB x S block Y(x) in registers
+//    (TM x TN complex accumulators per thread) while it walks the 81 stencil points, so every A element
+//    fetched from HBM is reused across all nrhs columns on chip and Y is written exactly once (the paper's
+//    formulation does 81 read-modify-writes of C, one per batched-GEMM launch: PAPER.md:320, 587);
+//  * every warp runs its OWN STAGES-deep shared-memory ring, filled by 1-D bulk TMA copies
+//    (cp.async.bulk + mbarrier complete_tx) that its lane 0 issues: a stage carries KCH = NB/KSPLIT
+//    contraction indices of one stencil matrix (k-major tile, the dominant HBM stream, L2 evict-first)
+//    and the matching rows of the neighbour's X tile (L2 evict-last).  A warp is the only consumer of its
+//    ring, so a stage is re-armed by the warp itself right after it has been consumed: no producer warp,
+//    no empty barriers, no cross-warp synchronisation anywhere in the main loop;
+//  * the chunk stream of a warp is continuous across its sites, so the ring never drains at a site boundary;
+//  * neighbour indices come from the periodic neighbour table (a1): the 81 entries of a site sit in three
+//    registers per lane and are broadcast with a shuffle.
 #pragma once
 
 #include "common.cuh"
@@ -32,10 +37,6 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t by
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
 {
     uint32_t ok;
@@ -54,6 +55,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
     while (!mbar_try_wait(bar, parity)) {}
 }
+// orders this thread's earlier generic-proxy accesses to shared memory before later async-proxy (TMA) accesses
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ uint64_t l2_policy_evict_first()
 {
     uint64_t pol;
@@ -79,32 +82,31 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
 // ---- compile-time configuration -------------------------------------------------------------------------
 // NB     : nbasis
 // TM, TN : per-thread register tile (rows x columns of Y, complex)
-// GC     : thread columns per warp (thread rows GR = 32 / GC);  NB = GR*TM,  CT = GC*TN columns per warp
-// SITES  : lattice sites per CTA group;  CB : column blocks per site;  nrhs = CB*CT exactly
-// KSPLIT : a pipeline stage carries NB/KSPLIT contraction indices of every site of the group
-template <typename T, int NB_, int TM_, int TN_, int GC_, int SITES_, int CB_, int KSPLIT_, int STAGES_>
+// GC     : thread columns per warp (thread rows GR = 32 / GC);  NB = GR*TM,  nrhs = S = GC*TN exactly
+// KSPLIT : a pipeline stage carries KCH = NB/KSPLIT contraction indices of one stencil point
+// STAGES : depth of each warp's ring;  WARPS : warps per CTA (one CTA per SM)
+template <typename T, int NB_, int TM_, int TN_, int GC_, int KSPLIT_, int STAGES_, int WARPS_>
 struct SimtConfig {
     using real = T;
-    static constexpr int NB = NB_, TM = TM_, TN = TN_, GC = GC_, SITES = SITES_, CB = CB_, KSPLIT = KSPLIT_, STAGES = STAGES_;
+    static constexpr int NB = NB_, TM = TM_, TN = TN_, GC = GC_, KSPLIT = KSPLIT_, STAGES = STAGES_, WARPS = WARPS_;
     static constexpr int GR = 32 / GC;
-    static constexpr int CT = GC * TN;
-    static constexpr int S = CB * CT;
-    static constexpr int NWARP = SITES * CB;
-    static constexpr int THREADS = (NWARP + 1) * 32;
+    static constexpr int S = GC * TN;
+    static constexpr int THREADS = WARPS * 32;
     static constexpr int KCH = NB / KSPLIT;
+    static constexpr int CPS = kNPoint * KSPLIT;                                // chunks (stages) per site
     static constexpr int VEC16 = 16 / (int)sizeof(cplx<T>);                    // complex elements per 16-byte vector
     static constexpr int VA = (TM % VEC16 == 0) ? VEC16 : 1;                    // vector width of the A (row) loads
     static constexpr int VX = (TN % VEC16 == 0) ? VEC16 : 1;                    // vector width of the X (column) loads
-    static constexpr int A_ELEMS = KCH * NB;                                    // per site per stage
+    static constexpr int A_ELEMS = KCH * NB;
     static constexpr int X_ELEMS = KCH * S;
     static constexpr uint32_t A_BYTES = A_ELEMS * sizeof(cplx<T>);
     static constexpr uint32_t X_BYTES = X_ELEMS * sizeof(cplx<T>);
-    static constexpr uint32_t STAGE_BYTES = SITES * (A_BYTES + X_BYTES);
-    static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 2 * STAGES * sizeof(uint64_t) + 16;
+    static constexpr uint32_t STAGE_BYTES = A_BYTES + X_BYTES;
+    static constexpr size_t SMEM_BYTES = (size_t)WARPS * STAGES * STAGE_BYTES + (size_t)WARPS * STAGES * sizeof(uint64_t) + 16;
     static_assert(GR * GC == 32 && GR * TM == NB, "thread grid must tile NB rows");
     static_assert(NB % KSPLIT == 0, "KSPLIT must divide NB");
     static_assert(A_BYTES % 16 == 0 && X_BYTES % 16 == 0, "bulk copies need 16-byte multiples");
-    static_assert(SITES <= 32, "one producer lane per site");
+    static_assert(SMEM_BYTES <= 227 * 1024, "shared memory ring does not fit");
 };
 
 // row r (0..TM-1) of a thread -> matrix row; chosen so that one warp-wide vector load touches a
@@ -145,102 +147,111 @@ stencil_simt_kernel(const cplx<typename C::real> *__restrict__ At, const int32_t
     using T = typename C::real;
     using Z = cplx<T>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    unsigned char *stage_base = smem_raw;
-    uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem_raw + (size_t)C::STAGES * C::STAGE_BYTES);
-    uint64_t *empty_bar = full_bar + C::STAGES;
-
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) {
-        for (int st = 0; st < C::STAGES; ++st) {
-            mbar_init(&full_bar[st], 1);
-            mbar_init(&empty_bar[st], C::NWARP);
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
+    unsigned char *ring = smem_raw + (size_t)warp * C::STAGES * C::STAGE_BYTES;
+    uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem_raw + (size_t)C::WARPS * C::STAGES * C::STAGE_BYTES) + warp * C::STAGES;
 
-    const int64_t ngroups = (V + C::SITES - 1) / C::SITES;
     constexpr int NN = C::NB * C::NB;        // elements per stencil matrix
     constexpr int NS = C::NB * C::S;         // elements per site of a vector block
+    constexpr unsigned FULL = 0xffffffffu;
 
-    if (warp == C::NWARP) {
-        // ===================== producer warp: lane l streams site l of the group =====================
-        if (lane < C::SITES) {
-            const uint64_t pol_a = l2_policy_evict_first();
-            const uint64_t pol_x = l2_policy_evict_last();
-            uint32_t it = 0;
-            for (int64_t g = blockIdx.x; g < ngroups; g += gridDim.x) {
-                int64_t x = g * C::SITES + lane;
-                if (x >= V) x = V - 1;                       // tail group: duplicate the last site (its Y store is skipped)
-                const int32_t *nrow = nbr + x * kNPoint;
-                const Z *arow = At + x * (int64_t)kNPoint * NN;
-                int32_t ynext = nrow[stencil_point_in_order(0)];
-                for (int q = 0; q < kNPoint; ++q) {
-                    const int p = stencil_point_in_order(q);
-                    const int64_t y = ynext;
-                    if (q + 1 < kNPoint) ynext = nrow[stencil_point_in_order(q + 1)];
-#pragma unroll
-                    for (int h = 0; h < C::KSPLIT; ++h, ++it) {
-                        const uint32_t st = it % C::STAGES, round = it / C::STAGES;
-                        mbar_wait(&empty_bar[st], (round & 1) ^ 1);
-                        if (lane == 0) mbar_arrive_expect_tx(&full_bar[st], C::STAGE_BYTES);
-                        __syncwarp(C::SITES >= 32 ? 0xffffffffu : ((1u << (C::SITES & 31)) - 1u));
-                        unsigned char *sb = stage_base + (size_t)st * C::STAGE_BYTES;
-                        Z *sA = reinterpret_cast<Z *>(sb) + lane * C::A_ELEMS;
-                        Z *sX = reinterpret_cast<Z *>(sb + C::SITES * C::A_BYTES) + lane * C::X_ELEMS;
-                        bulk_g2s(sA, arow + (int64_t)p * NN + h * C::A_ELEMS, C::A_BYTES, &full_bar[st], pol_a);
-                        bulk_g2s(sX, X + y * (int64_t)NS + h * C::X_ELEMS, C::X_BYTES, &full_bar[st], pol_x);
-                    }
-                }
-            }
+    // sites of this warp: first, first + stride, ...
+    const int64_t stride = (int64_t)gridDim.x * C::WARPS;
+    const int64_t first = (int64_t)blockIdx.x * C::WARPS + warp;
+    if (first >= V) return;
+    const int64_t nsites = (V - first + stride - 1) / stride;
+    const int64_t nchunks = nsites * C::CPS;
+
+    if (lane == 0) {
+        for (int st = 0; st < C::STAGES; ++st) mbar_init(&full_bar[st], 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+
+    uint64_t pol_a = 0, pol_x = 0;
+    if (lane == 0) { pol_a = l2_policy_evict_first(); pol_x = l2_policy_evict_last(); }
+
+    // ---- issue side: chunk (site, q, h) of the continuous stream, neighbour row of the site in registers ----
+    int64_t ix = first;                       // site whose chunks are being issued
+    int iw = 0;                               // chunk index within that site (q * KSPLIT + h)
+    int32_t n0, n1, n2;
+    auto load_nbr_row = [&](int64_t x) {
+        const int32_t *row = nbr + x * kNPoint;
+        n0 = row[lane];
+        n1 = row[lane + 32];
+        n2 = (lane + 64 < kNPoint) ? row[lane + 64] : 0;
+    };
+    load_nbr_row(ix);
+    auto issue = [&](int st) {                // all lanes call; lane 0 issues the two bulk copies of one chunk
+        const int q = iw / C::KSPLIT, h = iw % C::KSPLIT;
+        const int p = stencil_point_in_order(q);
+        const int32_t v = p < 32 ? n0 : (p < 64 ? n1 : n2);
+        const int64_t y = __shfl_sync(FULL, v, p & 31);
+        if (lane == 0) {
+            unsigned char *sb = ring + (size_t)st * C::STAGE_BYTES;
+            fence_proxy_async_smem();
+            mbar_arrive_expect_tx(&full_bar[st], C::STAGE_BYTES);
+            bulk_g2s(sb, At + (ix * kNPoint + p) * (int64_t)NN + h * C::A_ELEMS, C::A_BYTES, &full_bar[st], pol_a);
+            bulk_g2s(sb + C::A_BYTES, X + y * (int64_t)NS + h * C::X_ELEMS, C::X_BYTES, &full_bar[st], pol_x);
         }
-    } else {
-        // ===================== consumer warps: register-tiled complex MAC =====================
-        const int site_l = warp / C::CB, cb = warp % C::CB;
-        const int gr = lane / C::GC, gc = lane % C::GC;
-        const int row0 = gr * C::VA;                       // first row of this thread within a vector group
-        const int col0 = cb * C::CT + gc * C::VX;
-        uint32_t it = 0;
-        for (int64_t g = blockIdx.x; g < ngroups; g += gridDim.x) {
-            Z acc[C::TM][C::TN];
-#pragma unroll
-            for (int a = 0; a < C::TM; ++a)
-#pragma unroll
-                for (int b = 0; b < C::TN; ++b) { acc[a][b].re = 0; acc[a][b].im = 0; }
+        if (++iw == C::CPS) {
+            iw = 0;
+            ix += stride;
+            if (ix < V) load_nbr_row(ix);
+        }
+    };
 
-            for (int ph = 0; ph < kNPoint * C::KSPLIT; ++ph, ++it) {
-                const uint32_t st = it % C::STAGES, round = it / C::STAGES;
-                mbar_wait(&full_bar[st], round & 1);
-                const unsigned char *sb = stage_base + (size_t)st * C::STAGE_BYTES;
-                const Z *sA = reinterpret_cast<const Z *>(sb) + site_l * C::A_ELEMS + row0;
-                const Z *sX = reinterpret_cast<const Z *>(sb + C::SITES * C::A_BYTES) + site_l * C::X_ELEMS + col0;
+    // prologue: fill the ring
+    int64_t issued = 0;
+    for (; issued < C::STAGES && issued < nchunks; ++issued) issue((int)issued);
+
+    // ---- compute side ----
+    const int gr = lane / C::GC, gc = lane % C::GC;
+    const int row0 = gr * C::VA;
+    const int col0 = gc * C::VX;
+    Z acc[C::TM][C::TN];
+#pragma unroll
+    for (int a = 0; a < C::TM; ++a)
+#pragma unroll
+        for (int b = 0; b < C::TN; ++b) { acc[a][b].re = 0; acc[a][b].im = 0; }
+
+    int64_t cx = first;                       // site being computed
+    int cw = 0;                               // chunk index within it
+    int st = 0;
+    uint32_t parity = 0;
+    for (int64_t c = 0; c < nchunks; ++c) {
+        mbar_wait(&full_bar[st], parity);
+        const unsigned char *sb = ring + (size_t)st * C::STAGE_BYTES;
+        const Z *sA = reinterpret_cast<const Z *>(sb) + row0;
+        const Z *sX = reinterpret_cast<const Z *>(sb + C::A_BYTES) + col0;
 #pragma unroll 4
-                for (int k = 0; k < C::KCH; ++k) {
-                    Z a[C::TM], b[C::TN];
-                    VecLoad<T, C::TM, C::VA>::run(sA + k * C::NB, C::GR * C::VA, a);
-                    VecLoad<T, C::TN, C::VX>::run(sX + k * C::S, C::GC * C::VX, b);
+        for (int k = 0; k < C::KCH; ++k) {
+            Z a[C::TM], b[C::TN];
+            VecLoad<T, C::TM, C::VA>::run(sA + k * C::NB, C::GR * C::VA, a);
+            VecLoad<T, C::TN, C::VX>::run(sX + k * C::S, C::GC * C::VX, b);
 #pragma unroll
-                    for (int i = 0; i < C::TM; ++i)
+            for (int i = 0; i < C::TM; ++i)
 #pragma unroll
-                        for (int j = 0; j < C::TN; ++j) cmac(acc[i][j], a[i], b[j]);
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty_bar[st]);
-            }
+                for (int j = 0; j < C::TN; ++j) cmac(acc[i][j], a[i], b[j]);
+        }
+        __syncwarp();
+        if (issued < nchunks) { issue(st); ++issued; }      // re-arm the stage just consumed
+        if (++st == C::STAGES) { st = 0; parity ^= 1u; }
 
-            const int64_t x = g * C::SITES + site_l;
-            if (x < V) {
-                Z *yout = Y + x * (int64_t)NS;
+        if (++cw == C::CPS) {                 // site finished: write Y(x) once, start the next site
+            Z *yout = Y + cx * (int64_t)NS;
 #pragma unroll
-                for (int i = 0; i < C::TM; ++i) {
-                    const int row = simt_row<C>(gr, i);
+            for (int i = 0; i < C::TM; ++i) {
+                const int row = simt_row<C>(gr, i);
 #pragma unroll
-                    for (int j = 0; j < C::TN; ++j) {
-                        const int col = cb * C::CT + simt_col<C>(gc, j);
-                        yout[row * C::S + col] = acc[i][j];
-                    }
+                for (int j = 0; j < C::TN; ++j) {
+                    yout[row * C::S + simt_col<C>(gc, j)] = acc[i][j];
+                    acc[i][j].re = 0;
+                    acc[i][j].im = 0;
                 }
             }
+            cw = 0;
+            cx += stride;
         }
     }
 }
@@ -255,8 +266,8 @@ int launch_stencil_simt(const void *At, const int32_t *nbr, const void *X, void 
         CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
         attr_set = true;
     }
-    const int64_t ngroups = (V + C::SITES - 1) / C::SITES;
-    const int grid = (int)(ngroups < num_sms ? ngroups : num_sms);
+    const int64_t nctas = (V + C::WARPS - 1) / C::WARPS;
+    const int grid = (int)(nctas < num_sms ? nctas : num_sms);
     kern<<<grid, C::THREADS, C::SMEM_BYTES, stream>>>(static_cast<const Z *>(At), nbr, static_cast<const Z *>(X),
                                                        static_cast<Z *>(Y), V);
     CMRHS_LAUNCH_CHECK();
