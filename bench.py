@@ -186,6 +186,23 @@ def run_reference(args, cfg):
     return 0
 
 
+# ---- multi-rank plumbing (replicas only: DESIGN.md section 9) ---------------------------------------------------
+def max_over_ranks(ms: float, world: int, device: str) -> float:
+    """device time of the slowest rank (all_reduce MAX over the default process group)"""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, steps: int, flops_per_step_per_rank: float, ms_max: float) -> float:
+    """TFLOP/s of the whole job: every rank does the same work on its own replica (weak scaling)"""
+    return world * steps * flops_per_step_per_rank / (ms_max * 1e-3) / 1e12
+
+
 # ---- our arm ---------------------------------------------------------------------------------------------------
 def load_traffic(kernel_name):
     """dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture, or None."""
@@ -261,11 +278,8 @@ def run_ours(args, cfg):
     clk = clocks.stop() if rank == 0 else None
     out = op.block_cg_end()
     assert out["status"] == 0, "block CG broke down inside the timed region"
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * K * step_flops(V, nb, s) / (ms * 1e-3) / 1e12
+    ms = max_over_ranks(ms, world, "cuda")
+    value = whole_job_value(world, K, step_flops(V, nb, s), ms)
 
     if rank != 0:
         if world > 1:
