@@ -12,6 +12,7 @@
 #include "setup_kernels.cuh"
 #include "stencil_generic.cuh"
 #include "stencil_simt.cuh"
+#include "stencil_tc.cuh"
 
 namespace cmrhs {
 
@@ -73,6 +74,9 @@ struct coarse_op {
     int num_sms = 0;
     size_t esize = 0;            // bytes per complex element
     void *At = nullptr;          // [V][81][nb(k)][nb(i)]
+    void *Ac = nullptr;          // canonical copy [V][81][nb(i)][nb(k)] for the tensor path (complex64 only)
+    CUtensorMap tmA;             // TMA descriptor of Ac
+    bool tc_ok = false;
     int32_t *nbr = nullptr;      // [V][81]
     void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
     zdouble *gram_partial = nullptr;
@@ -142,6 +146,7 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
 {
     if (!op) return COARSE_OK;
     cudaFree(op->At);
+    cudaFree(op->Ac);
     cudaFree(op->nbr);
     for (void *b : op->blk) cudaFree(b);
     cudaFree(op->gram_partial);
@@ -192,6 +197,8 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
     } while (0)
     CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
+    const bool want_tc = dtype == COARSE_C64 && !(flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) && tc_supported(nbasis, 8);
+    if (want_tc) CMRHS_TRY(alloc_dev(op, &op->Ac, a_bytes));
     for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
     CMRHS_TRY(alloc_dev(op, (void **)&op->small, (size_t)6 * COARSE_MAX_NRHS * COARSE_MAX_NRHS * sizeof(zdouble)));
@@ -216,6 +223,20 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
             relayout_transpose_kernel<double><<<grid, 128, 0, stream>>>((const cplx<double> *)A_dev, (cplx<double> *)op->At, ntiles, nbasis);
         count_launch();
     }
+    if (want_tc) {
+        ce = cudaMemcpyAsync(op->Ac, A_dev, a_bytes, cudaMemcpyDeviceToDevice, stream);
+        int ts = COARSE_CUDA_ERROR;
+        if (ce == cudaSuccess) {
+            switch (nbasis) {
+            case 8: ts = tc_make_tmap_A<8>(&op->tmA, op->Ac, V); break;
+            case 16: ts = tc_make_tmap_A<16>(&op->tmA, op->Ac, V); break;
+            case 24: ts = tc_make_tmap_A<24>(&op->tmA, op->Ac, V); break;
+            default: ts = tc_make_tmap_A<32>(&op->tmA, op->Ac, V); break;
+            }
+        } else set_error("copy of A failed: %s", cudaGetErrorString(ce));
+        if (ts != COARSE_OK) { coarse_op_destroy(op); return ts; }
+        op->tc_ok = true;
+    }
     ce = cudaGetLastError();
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(stream);
     if (ce != cudaSuccess) {
@@ -235,9 +256,12 @@ static const SimtVariant *select_variant(const coarse_op *op, int nrhs)
     return find_variant(op->dtype, op->nb, nrhs);
 }
 
+static bool use_tc(const coarse_op *op, int nrhs) { return op->tc_ok && tc_supported(op->nb, nrhs); }
+
 extern "C" const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs)
 {
     if (!op) return "";
+    if (use_tc(op, nrhs)) return "stencil_tc<tf32x3>";
     const SimtVariant *v = select_variant(op, nrhs);
     return v ? v->name : (op->dtype == COARSE_C64 ? "stencil_generic<float>" : "stencil_generic<double>");
 }
@@ -258,6 +282,14 @@ static int apply_impl(const coarse_op *op_c, const void *X, void *Y, int nrhs, c
 
 static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream)
 {
+    if (use_tc(op, nrhs)) {
+        switch (op->nb) {
+        case 8: return launch_stencil_tc<8>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
+        case 16: return launch_stencil_tc<16>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
+        case 24: return launch_stencil_tc<24>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
+        default: return launch_stencil_tc<32>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
+        }
+    }
     const SimtVariant *v = select_variant(op, nrhs);
     if (v) return v->launch(op->At, op->nbr, X, Y, op->dims.V, op->num_sms, stream);
     if (op->dtype == COARSE_C64)
