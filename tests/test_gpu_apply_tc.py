@@ -5,11 +5,11 @@ diagonally dominant operators of BASELINE.json the measured error is asserted ag
 block CG to 1e-6 needs the apply to be that accurate.
 
 Two properties of the tensor core shape the assertions:
- * x = hi + lo with both parts rounded to TF32 loses the last bit of x in about a quarter of the cases, and the
-   FP32 accumulator adds with truncation: "exact" cases (pure shifts, multiplication by i) are exact to ONE float32
-   ulp per real component, not bit for bit (the SIMT kernels are bit exact, test_gpu_apply.py);
- * without a dominant diagonal (c = 0) the truncated accumulation is the leading error: <= 1e-5 where the correction
-   products have their own accumulators (nrhs <= 32), <= 3e-5 for nrhs > 32 (tensor memory has no room for them).
+ * x = hi + lo with hi rounded to TF32 and lo = x - hi cut to TF32 by the tensor core loses the last bits of x, and
+   the FP32 accumulator adds with truncation: "exact" cases (pure shifts, multiplication by i) are exact to ONE
+   float32 ulp per real component, not bit for bit (the SIMT kernels are bit exact, test_gpu_apply.py);
+ * without a dominant diagonal (c = 0) the truncated accumulation is the leading error; the correction products have
+   their own accumulators for every nrhs, which keeps it below the 1e-5 bar (measured ~6e-6).
 """
 import numpy as np
 import pytest
@@ -36,7 +36,7 @@ def _apply_tc(dims, A, X, nrhs_max=None):
     return Y
 
 
-# lattices: x extent 3 (one ragged group of 3), 4 (one full group), 5 (4 + 1), 6 (4 + 2), 9 (4 + 4 + 1); wrap in every direction
+# lattices: x extent 3 (one pair + a single site), 4 (two pairs), 5 (2 + 2 + 1); wrap in every direction
 @pytest.mark.parametrize("nb,s", [(32, 16), (32, 8), (32, 32), (32, 64), (32, 24), (32, 40), (24, 16), (24, 64), (16, 16), (8, 8), (8, 48)])
 @pytest.mark.parametrize("dims", [(3, 3, 3, 5), (4, 4, 4, 6), (5, 2, 3, 3)])
 def test_tensor_kernel_matches_oracle(nb, s, dims):
@@ -57,7 +57,7 @@ def test_tensor_kernel_small_extents_alias_and_add(dims):
 
 def test_tensor_kernel_without_diagonal_shift():
     dims = (3, 4, 3, 4)
-    for nb, s, bar in [(32, 16, 1e-5), (32, 32, 1e-5), (24, 64, 3e-5)]:
+    for nb, s, bar in [(32, 16, 1e-5), (32, 32, 1e-5), (32, 64, 1e-5), (24, 64, 1e-5)]:
         A, c, X, _ = host_case(dims, nb, s, seed=7, factor=0.0)
         assert c == 0.0
         Y = _apply_tc(dims, A, X)
