@@ -147,7 +147,7 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     using C = TcCfg<NB>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // carve: [A ring][X ring (hi|lo per stage)][epilogue exchange][schedule tables][barriers][tmem slot]
-    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);     // keeps the shared address space
     unsigned char *ringA = smem;
     unsigned char *ringX = ringA + (size_t)P.sa * C::STAGE_BYTES;
     float4 *exch = reinterpret_cast<float4 *>(ringX + (size_t)P.sx * 2 * P.xt_bytes);      // [pair 2][buf 2][part 2][j 2][lane 32]
@@ -257,12 +257,22 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 mbar_wait(&x_full[rx.stage], rx.phase);
                 unsigned char *hi_t = ringX + (size_t)rx.stage * 2 * P.xt_bytes;
                 unsigned char *lo_t = hi_t + P.xt_bytes;
-                for (int c = tid; c < nchunks; c += 128) {
+                int c = tid;
+                for (; c + 128 < nchunks; c += 256) {          // two chunks per trip: both loads in flight
+                    const float4 v0 = *reinterpret_cast<const float4 *>(hi_t + 16 * c);
+                    const float4 v1 = *reinterpret_cast<const float4 *>(hi_t + 16 * (c + 128));
+                    const float4 h0 = make_float4(tf32_rn(v0.x), tf32_rn(v0.y), tf32_rn(v0.z), tf32_rn(v0.w));
+                    const float4 h1 = make_float4(tf32_rn(v1.x), tf32_rn(v1.y), tf32_rn(v1.z), tf32_rn(v1.w));
+                    *reinterpret_cast<float4 *>(hi_t + 16 * c) = h0;
+                    *reinterpret_cast<float4 *>(lo_t + 16 * c) = make_float4(v0.x - h0.x, v0.y - h0.y, v0.z - h0.z, v0.w - h0.w);
+                    *reinterpret_cast<float4 *>(hi_t + 16 * (c + 128)) = h1;
+                    *reinterpret_cast<float4 *>(lo_t + 16 * (c + 128)) = make_float4(v1.x - h1.x, v1.y - h1.y, v1.z - h1.z, v1.w - h1.w);
+                }
+                if (c < nchunks) {
                     const float4 v = *reinterpret_cast<const float4 *>(hi_t + 16 * c);
                     const float4 h = make_float4(tf32_rn(v.x), tf32_rn(v.y), tf32_rn(v.z), tf32_rn(v.w));
-                    const float4 l = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
                     *reinterpret_cast<float4 *>(hi_t + 16 * c) = h;
-                    *reinterpret_cast<float4 *>(lo_t + 16 * c) = l;
+                    *reinterpret_cast<float4 *>(lo_t + 16 * c) = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
                 }
                 fence_proxy_async_smem();       // generic-proxy writes -> visible to the tensor core's async-proxy reads
                 __syncwarp();
@@ -328,62 +338,67 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
     } else if (warp == 16) {
         // ================= A producer: one canonical stencil matrix per stage =================
-        if (lane == 0) {
-            const uint64_t pol = l2_policy_evict_first();
-            TcRing ra;
-            for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-                const TcGroup grp = tc_group(P, g, tab2, tab1);
-                const int64_t site0 = tc_site(P, grp.x0, grp.y, grp.z, grp.t);
-                for (int step = 0; step < grp.nsteps; ++step) {
-                    const uint32_t e = grp.tab[step];
-                    const int off3 = (int)(e & 31u);
+        // (the whole warp walks the schedule so that every address stays warp-uniform; one elected lane issues)
+        const uint64_t pol = l2_policy_evict_first();
+        TcRing ra;
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const TcGroup grp = tc_group(P, g, tab2, tab1);
+            const int64_t site0 = tc_site(P, grp.x0, grp.y, grp.z, grp.t);
+            for (int step = 0; step < grp.nsteps; ++step) {
+                const uint32_t e = grp.tab[step];
+                const int off3 = (int)(e & 31u);
 #pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        if (!((e >> (8 + i)) & 1u)) continue;
-                        const int p = (int)((e >> (10 + 2 * i)) & 3u) + 3 * off3;
-                        const int64_t row0 = ((site0 + i) * kNPoint + p) * NB;
-                        mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u);
+                for (int i = 0; i < 2; ++i) {
+                    if (!((e >> (8 + i)) & 1u)) continue;
+                    const int p = (int)((e >> (10 + 2 * i)) & 3u) + 3 * off3;
+                    const int64_t row0 = ((site0 + i) * kNPoint + p) * NB;
+                    mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u);
+                    if (elect_one_sync()) {
                         mbar_arrive_expect_tx(&a_full[ra.stage], C::TILE_BYTES);
                         unsigned char *dst = ringA + (size_t)ra.stage * C::STAGE_BYTES;
 #pragma unroll
                         for (int h = 0; h < C::PIECES; ++h)
                             tma_load_2d(dst + h * C::PIECE_BYTES, &tmA, h * C::KW, (int32_t)row0, &a_full[ra.stage], pol);
-                        ra.advance(P.sa);
                     }
+                    __syncwarp();
+                    ra.advance(P.sa);
                 }
             }
         }
     } else if (warp == 17) {
         // ================= X producer: the neighbour's X tile, once per step =================
-        if (lane == 0) {
-            const uint64_t pol = l2_policy_evict_last();
-            TcRing rx;
-            for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-                const TcGroup grp = tc_group(P, g, tab2, tab1);
-                for (int step = 0; step < grp.nsteps; ++step) {
-                    const int64_t row0 = tc_x_site(P, grp, grp.tab[step]) * NB;
-                    mbar_wait(&x_empty[rx.stage], rx.phase ^ 1u);
+        const uint64_t pol = l2_policy_evict_last();
+        TcRing rx;
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const TcGroup grp = tc_group(P, g, tab2, tab1);
+            for (int step = 0; step < grp.nsteps; ++step) {
+                const int64_t row0 = tc_x_site(P, grp, grp.tab[step]) * NB;
+                mbar_wait(&x_empty[rx.stage], rx.phase ^ 1u);
+                if (elect_one_sync()) {
                     mbar_arrive_expect_tx(&x_full[rx.stage], (uint32_t)P.x_tile_tx);
                     unsigned char *dst = ringX + (size_t)rx.stage * 2 * P.xt_bytes;
                     for (int b = 0; b < P.nxb; ++b)
                         tma_load_2d(dst + (size_t)b * NB * 128, &tmX, b * 32, (int32_t)row0, &x_full[rx.stage], pol);
-                    rx.advance(P.sx);
                 }
+                __syncwarp();
+                rx.advance(P.sx);
             }
         }
     } else if (warp == 18) {
         // ================= MMA issuer =================
-        if (lane == 0) {
-            TcRing rx, rs, rc;
-            for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-                const int nsteps = (min(2, P.L[0] - (g % P.ng0) * 2) == 2) ? 110 : 81;
-                mbar_wait(&acc_empty[rc.stage], rc.phase ^ 1u);
+        // The whole warp runs the loop (all operands stay warp-uniform: no per-instruction broadcast loops in SASS);
+        // one elected lane -- the same one every time -- issues the MMAs and the commits.
+        TcRing rx, rs, rc;
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const int nsteps = (min(2, P.L[0] - (g % P.ng0) * 2) == 2) ? 110 : 81;
+            mbar_wait(&acc_empty[rc.stage], rc.phase ^ 1u);
+            tc_fence_after_sync();
+            const uint32_t d = tmem + (uint32_t)(rc.stage * P.acc_stride), cacc = d + (uint32_t)P.N;
+            for (int step = 0; step < nsteps; ++step) {
+                mbar_wait(&set_full[rs.stage], rs.phase);
+                mbar_wait(&xlo_full[rx.stage], rx.phase);
                 tc_fence_after_sync();
-                const uint32_t d = tmem + (uint32_t)(rc.stage * P.acc_stride), cacc = d + (uint32_t)P.N;
-                for (int step = 0; step < nsteps; ++step) {
-                    mbar_wait(&set_full[rs.stage], rs.phase);
-                    mbar_wait(&xlo_full[rx.stage], rx.phase);
-                    tc_fence_after_sync();
+                if (elect_one_sync()) {
                     const uint32_t a_hi = tmem + acc_cols + (uint32_t)rs.stage * kTcSetCols, a_lo = a_hi + 32u;
                     const uint32_t xhi = smem_u32(ringX + (size_t)rx.stage * 2 * P.xt_bytes), xlo = xhi + (uint32_t)P.xt_bytes;
 #pragma unroll
@@ -398,11 +413,12 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     umma_commit(&set_empty[rs.stage]);
                     umma_commit(&x_empty[rx.stage]);
                     if (step == nsteps - 1) umma_commit(&acc_full[rc.stage]);
-                    rs.advance(P.nset);
-                    rx.advance(P.sx);
                 }
-                rc.advance(P.nacc);
+                __syncwarp();
+                rs.advance(P.nset);
+                rx.advance(P.sx);
             }
+            rc.advance(P.nacc);
         }
     }
     // ---- teardown ----

@@ -9,6 +9,20 @@
 
 namespace cmrhs {
 
+// ---- one lane of a converged warp (the same one every time for a full mask) --------------------------------
+__device__ __forceinline__ bool elect_one_sync()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 // ---- mbarrier: plain arrive -----------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
