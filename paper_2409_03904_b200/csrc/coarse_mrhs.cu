@@ -75,6 +75,7 @@ struct coarse_op {
     size_t esize = 0;            // bytes per complex element
     void *At = nullptr;          // [V][81][nb(k)][nb(i)]
     void *Ac = nullptr;          // canonical copy [V][81][nb(i)][nb(k)] for the tensor path (complex64 only)
+    bool Ac_owned = false;       // false: Ac is the caller's A_dev (COARSE_FLAG_BORROW_A)
     CUtensorMap tmA;             // TMA descriptor of Ac
     bool tc_ok = false;
     int32_t *nbr = nullptr;      // [V][81]
@@ -146,7 +147,7 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
 {
     if (!op) return COARSE_OK;
     cudaFree(op->At);
-    cudaFree(op->Ac);
+    if (op->Ac_owned) cudaFree(op->Ac);
     cudaFree(op->nbr);
     for (void *b : op->blk) cudaFree(b);
     cudaFree(op->gram_partial);
@@ -198,7 +199,9 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
     CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
     const bool want_tc = dtype == COARSE_C64 && !(flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) && tc_supported(nbasis, 8);
-    if (want_tc) CMRHS_TRY(alloc_dev(op, &op->Ac, a_bytes));
+    const bool borrow = want_tc && (flags & COARSE_FLAG_BORROW_A) && (reinterpret_cast<uintptr_t>(A_dev) & 15u) == 0;
+    if (want_tc && !borrow) { CMRHS_TRY(alloc_dev(op, &op->Ac, a_bytes)); op->Ac_owned = true; }
+    if (borrow) op->Ac = const_cast<void *>(A_dev);
     for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
     CMRHS_TRY(alloc_dev(op, (void **)&op->small, (size_t)6 * COARSE_MAX_NRHS * COARSE_MAX_NRHS * sizeof(zdouble)));
@@ -224,7 +227,7 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
         count_launch();
     }
     if (want_tc) {
-        ce = cudaMemcpyAsync(op->Ac, A_dev, a_bytes, cudaMemcpyDeviceToDevice, stream);
+        ce = borrow ? cudaSuccess : cudaMemcpyAsync(op->Ac, A_dev, a_bytes, cudaMemcpyDeviceToDevice, stream);
         int ts = COARSE_CUDA_ERROR;
         if (ce == cudaSuccess) {
             switch (nbasis) {

@@ -122,3 +122,17 @@ def test_tensor_and_simt_kernels_agree():
     ref = oracle.apply(dims, A, X)
     assert rel_err_cols(Yt, ref) <= 1e-6 and rel_err_cols(Ys, ref) <= 1e-6
     assert rel_err_cols(Yt, Ys) <= 2e-6
+
+
+def test_borrowed_and_copied_operator_give_identical_results():
+    # COARSE_FLAG_BORROW_A: the tensor kernel reads the caller's canonical A instead of an internal copy
+    dims, nb, s = (4, 3, 3, 4), 24, 16
+    A, c, X, _ = host_case(dims, nb, s, seed=17, factor=1.02)
+    Ad, Xd = to_dev(A, "c64"), to_dev(X, "c64")
+    outs = []
+    for flags in (0, cm.binding.FLAG_BORROW_A):
+        op = cm.CoarseOperator(dims, Ad, s, flags=flags)
+        assert op.kernel_name(s).startswith("stencil_tc")
+        outs.append(to_np(op.apply(Xd)))
+        op.close()
+    assert np.array_equal(outs[0], outs[1])
