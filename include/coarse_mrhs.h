@@ -56,10 +56,9 @@ enum {
 enum {
     COARSE_FLAG_FORCE_GENERIC = 1u << 0, /* always use the generic (untiled) stencil kernel: test / debugging aid */
     COARSE_FLAG_NO_TENSOR = 1u << 1,     /* never select a tensor-core kernel variant */
-    COARSE_FLAG_BORROW_A = 1u << 2       /* the tensor-core kernels read the canonical layout: let them read A_dev itself
-                                            instead of a second internal copy.  The caller keeps A_dev alive and
-                                            unmodified until coarse_op_destroy.  (The SIMT kernels' re-laid-out copy is
-                                            always internal.) */
+    COARSE_FLAG_TENSOR_ONLY = 1u << 2    /* complex64 shapes the tensor-core kernel covers: keep only its layout of A (one
+                                            internal copy instead of two); apply / solve with an nrhs that kernel does not
+                                            cover (not a multiple of 8) then return COARSE_UNSUPPORTED */
 };
 
 #define COARSE_MAX_NRHS 64
@@ -74,10 +73,9 @@ enum {
  *   nrhs_max  : 1..64, largest nrhs later passed to apply / solve; sizes the block-CG workspace
  *   dtype     : COARSE_C64 or COARSE_C128 (storage and multiply precision of A, X, Y)
  *   A_dev     : device, canonical layout; COPIED (re-laid-out for the kernels) -- may be freed after return
- *               unless COARSE_FLAG_BORROW_A is set
  *   flags     : COARSE_FLAG_*
  * Allocates device memory: one internal copy of A (two for complex64 shapes the tensor-core kernel covers, unless
- * COARSE_FLAG_BORROW_A), V*81 int32 neighbour table, 6 vector blocks of
+ * COARSE_FLAG_TENSOR_ONLY or COARSE_FLAG_NO_TENSOR), V*81 int32 neighbour table, 6 vector blocks of
  * V*nbasis*nrhs_max elements plus O(grid * nrhs_max^2) reduction scratch.  Synchronises `stream`.
  */
 int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_t nbasis, int32_t nrhs_max,

@@ -16,7 +16,7 @@ from . import build as _build
 
 C64, C128 = 0, 1
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY, NOT_CONVERGED, BREAKDOWN = 0, -1, -2, -3, -4, -5, -6
-FLAG_FORCE_GENERIC, FLAG_NO_TENSOR, FLAG_BORROW_A = 1, 2, 4
+FLAG_FORCE_GENERIC, FLAG_NO_TENSOR, FLAG_TENSOR_ONLY = 1, 2, 4
 MAX_NRHS, MAX_HISTORY = 64, 256
 
 EXPORTS = [
@@ -117,11 +117,10 @@ def launch_count() -> int:
 
 
 class CoarseOperator:
-    """Handle of coarse_op_create.  A: [V][81][nb][nb] complex CUDA tensor (canonical layout).  The library keeps its
-    own re-laid-out copy for the SIMT kernels; with FLAG_BORROW_A (the default here) the tensor-core kernels read A
-    itself, and this object keeps the tensor alive."""
+    """Handle of coarse_op_create.  A: [V][81][nb][nb] complex CUDA tensor (canonical layout; copied into the
+    kernels' own layouts, so the caller may release it afterwards)."""
 
-    def __init__(self, dims, A: torch.Tensor, nrhs_max: int, flags: int = FLAG_BORROW_A, stream=None):
+    def __init__(self, dims, A: torch.Tensor, nrhs_max: int, flags: int = 0, stream=None):
         self.dims = tuple(int(d) for d in dims)
         V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
         if A.dim() != 4 or A.shape[0] != V or A.shape[1] != 81 or A.shape[2] != A.shape[3]:
@@ -130,13 +129,11 @@ class CoarseOperator:
         self._h = C.c_void_p()
         _check(lib().coarse_op_create(C.byref(self._h), _dims(self.dims), self.nbasis, self.nrhs_max, _dtype_code(A),
                                       _dev(A), flags, _stream(stream)))
-        self._A = A if (flags & FLAG_BORROW_A) else None
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h:
             lib().coarse_op_destroy(self._h)
             self._h = None
-            self._A = None
 
     __del__ = close
 

@@ -74,9 +74,7 @@ struct coarse_op {
     int num_sms = 0;
     size_t esize = 0;            // bytes per complex element
     void *At = nullptr;          // [V][81][nb(k)][nb(i)]
-    void *Ac = nullptr;          // canonical copy [V][81][nb(i)][nb(k)] for the tensor path (complex64 only)
-    bool Ac_owned = false;       // false: Ac is the caller's A_dev (COARSE_FLAG_BORROW_A)
-    CUtensorMap tmA;             // TMA descriptor of Ac
+    float *Ak = nullptr;         // planar k-major [V][81][part][nb(k)][nb(i)] for the tensor path (complex64 only)
     bool tc_ok = false;
     int32_t *nbr = nullptr;      // [V][81]
     void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
@@ -147,7 +145,7 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
 {
     if (!op) return COARSE_OK;
     cudaFree(op->At);
-    if (op->Ac_owned) cudaFree(op->Ac);
+    cudaFree(op->Ak);
     cudaFree(op->nbr);
     for (void *b : op->blk) cudaFree(b);
     cudaFree(op->gram_partial);
@@ -196,12 +194,11 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
             return _s;                       \
         }                                    \
     } while (0)
-    CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
-    CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
     const bool want_tc = dtype == COARSE_C64 && !(flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) && tc_supported(nbasis, 8);
-    const bool borrow = want_tc && (flags & COARSE_FLAG_BORROW_A) && (reinterpret_cast<uintptr_t>(A_dev) & 15u) == 0;
-    if (want_tc && !borrow) { CMRHS_TRY(alloc_dev(op, &op->Ac, a_bytes)); op->Ac_owned = true; }
-    if (borrow) op->Ac = const_cast<void *>(A_dev);
+    const bool want_simt = !(want_tc && (flags & COARSE_FLAG_TENSOR_ONLY));
+    if (want_simt) CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
+    CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
+    if (want_tc) CMRHS_TRY(alloc_dev(op, (void **)&op->Ak, a_bytes));
     for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
     CMRHS_TRY(alloc_dev(op, (void **)&op->small, (size_t)6 * COARSE_MAX_NRHS * COARSE_MAX_NRHS * sizeof(zdouble)));
@@ -217,27 +214,18 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
         neighbour_table_kernel<<<grid, 256, 0, stream>>>(op->dims, op->nbr);
         count_launch();
     }
-    // re-layout A into k-major tiles
-    {
-        const int grid = (int)(ntiles < 1048576 ? ntiles : 1048576);
+    // re-layout A into k-major tiles (SIMT kernels: interleaved complex; tensor kernel: planar float32)
+    const int rgrid = (int)(ntiles < 1048576 ? ntiles : 1048576);
+    if (want_simt) {
         if (dtype == COARSE_C64)
-            relayout_transpose_kernel<float><<<grid, 128, 0, stream>>>((const cplx<float> *)A_dev, (cplx<float> *)op->At, ntiles, nbasis);
+            relayout_transpose_kernel<float><<<rgrid, 128, 0, stream>>>((const cplx<float> *)A_dev, (cplx<float> *)op->At, ntiles, nbasis);
         else
-            relayout_transpose_kernel<double><<<grid, 128, 0, stream>>>((const cplx<double> *)A_dev, (cplx<double> *)op->At, ntiles, nbasis);
+            relayout_transpose_kernel<double><<<rgrid, 128, 0, stream>>>((const cplx<double> *)A_dev, (cplx<double> *)op->At, ntiles, nbasis);
         count_launch();
     }
     if (want_tc) {
-        ce = borrow ? cudaSuccess : cudaMemcpyAsync(op->Ac, A_dev, a_bytes, cudaMemcpyDeviceToDevice, stream);
-        int ts = COARSE_CUDA_ERROR;
-        if (ce == cudaSuccess) {
-            switch (nbasis) {
-            case 8: ts = tc_make_tmap_A<8>(&op->tmA, op->Ac, V); break;
-            case 16: ts = tc_make_tmap_A<16>(&op->tmA, op->Ac, V); break;
-            case 24: ts = tc_make_tmap_A<24>(&op->tmA, op->Ac, V); break;
-            default: ts = tc_make_tmap_A<32>(&op->tmA, op->Ac, V); break;
-            }
-        } else set_error("copy of A failed: %s", cudaGetErrorString(ce));
-        if (ts != COARSE_OK) { coarse_op_destroy(op); return ts; }
+        relayout_planar_kernel<<<rgrid, 128, 0, stream>>>((const cplx<float> *)A_dev, op->Ak, ntiles, nbasis);
+        count_launch();
         op->tc_ok = true;
     }
     ce = cudaGetLastError();
@@ -265,6 +253,7 @@ extern "C" const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs
 {
     if (!op) return "";
     if (use_tc(op, nrhs)) return "stencil_tc<tf32x3>";
+    if (!op->At) return "unsupported";
     const SimtVariant *v = select_variant(op, nrhs);
     return v ? v->name : (op->dtype == COARSE_C64 ? "stencil_generic<float>" : "stencil_generic<double>");
 }
@@ -287,11 +276,15 @@ static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, c
 {
     if (use_tc(op, nrhs)) {
         switch (op->nb) {
-        case 8: return launch_stencil_tc<8>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
-        case 16: return launch_stencil_tc<16>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
-        case 24: return launch_stencil_tc<24>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
-        default: return launch_stencil_tc<32>(op->tmA, op->dims, X, Y, nrhs, op->num_sms, stream);
+        case 8: return launch_stencil_tc<8>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);
+        case 16: return launch_stencil_tc<16>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);
+        case 24: return launch_stencil_tc<24>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);
+        default: return launch_stencil_tc<32>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);
         }
+    }
+    if (!op->At) {
+        set_error("COARSE_FLAG_TENSOR_ONLY: nrhs %d is not covered by the tensor-core kernel (multiples of 8)", nrhs);
+        return COARSE_UNSUPPORTED;
     }
     const SimtVariant *v = select_variant(op, nrhs);
     if (v) return v->launch(op->At, op->nbr, X, Y, op->dims.V, op->num_sms, stream);
@@ -746,3 +739,11 @@ extern "C" int coarse_op_profile_read(coarse_op_t *op, double *ms, int32_t capac
     op->prof_n = 0;
     return COARSE_OK;
 }
+
+#ifdef CMRHS_TC_TRACE
+// developer diagnostic (not part of the ABI): per-CTA, per-warp cycle counters of the last tensor-kernel launch
+extern "C" int coarse_debug_trace_read(long long *out)
+{
+    return (int)cudaMemcpyFromSymbol(out, cmrhs::g_tc_trace, sizeof(cmrhs::g_tc_trace));
+}
+#endif

@@ -8,11 +8,12 @@
 //   (lane quarter q: site slot q/2, part q%2): one accumulator of N = 2 nrhs columns serves both parts, an X tile
 //   X(y) is shared by the x-neighbours, so a group of two sites takes 110 MMA steps instead of 162 (26 x 4 columns
 //   of neighbours + the centre offset swept so that each site's centre point comes last).
-// * The stencil matrices (the HBM stream: 81 nb^2 complex per site) arrive by 2-D TMA in the caller's canonical
-//   layout, 128B/64B-swizzled so that "one thread = one matrix row" reads are bank-conflict free; the converter
-//   warps split every element into TF32 hi (round to nearest) + lo = x - hi (exact; the tensor core keeps its
-//   leading 11 bits), de-interleave re/im and write the operand panels (hi | lo) into TMEM with tcgen05.st.
-//   A is never re-written to shared memory.
+// * The stencil matrices (the HBM stream: 81 nb^2 complex per site) are kept in a planar, k-major internal layout
+//   Ak[x][p][part][k][i] (part 0 = Re, 1 = Im; written once by coarse_op_create): a whole matrix is one contiguous
+//   1-D bulk copy, and "one thread = one matrix row i" reads of a column k are 32 consecutive floats (conflict free,
+//   no swizzle, any nbasis).  The converter warps (three per TMEM lane quarter, taking turns step by step) split
+//   every element into TF32 hi (round to nearest) + lo = x - hi (exact; the tensor core keeps its leading 11 bits)
+//   and write the operand panels (hi | lo) into TMEM with tcgen05.st.  A is never re-written to shared memory.
 // * N side = the neighbour's X tile exactly as it lies in memory ([j][r][re,im] = K x N, N contiguous: an
 //   MN-major UMMA operand, layout SWIZZLE_128B_BASE32B), loaded by TMA with the matching swizzle (128B_ATOM_32B);
 //   four warps round it to TF32 in place and write the lo tile beside it.
@@ -20,9 +21,9 @@
 //   into its FP32 accumulator with truncation: keeping the small products apart spares D two thirds of the
 //   additions); Y = D + C is formed with a round-to-nearest add in the epilogue.
 // * Accumulation order: the 80 off-centre points first, the centre point (which carries c*I) last.
-// * Warp roles (640 threads, one persistent CTA per SM): 0-7 A converters (two per lane quarter, alternating
-//   steps), 8-11 X converters, 12-15 epilogue, 16 A producer (TMA), 17 X producer (TMA), 18 MMA issuer,
-//   19 TMEM allocator.  All hand-offs are mbarriers; the step schedule is a table in shared memory.
+// * Warp roles (768 threads, one persistent CTA per SM): 0-11 A converters (three per lane quarter, taking turns),
+//   12-15 X converters, 16-19 epilogue, 20 A producer (bulk copies), 21 X producer (TMA), 22 MMA issuer,
+//   23 TMEM allocator.  All hand-offs are mbarriers; the step schedule is a table in shared memory.
 #pragma once
 
 #include "setup_kernels.cuh"
@@ -30,8 +31,9 @@
 
 namespace cmrhs {
 
-constexpr int kTcThreads = 640;
-constexpr int kTcMaxStagesA = 24;
+constexpr int kTcThreads = 768;
+constexpr int kTcConvTurns = 3;        // A converter warps per TMEM lane quarter
+constexpr int kTcMaxStagesA = 32;
 constexpr int kTcMaxStagesX = 4;
 constexpr int kTcMaxSets = 6;
 constexpr int kTcSetCols = 64;          // TMEM columns of one operand panel set: hi at +0, lo at +32
@@ -57,14 +59,9 @@ struct TcParams {
 
 template <int NB> struct TcCfg {
     static_assert(NB % 8 == 0 && NB >= 8 && NB <= 32, "tensor path: nbasis in {8,16,24,32}");
-    static constexpr int KW = (2 * NB % 32 == 0) ? 32 : 16;         // floats per swizzle row of an A piece
-    static constexpr int PIECES = 2 * NB / KW;
-    static constexpr uint32_t SWZ_MASK = KW == 32 ? 7u : 3u;         // Swizzle<3,4,3> / Swizzle<2,4,3>
-    static constexpr int JP = KW / 2;                                // complex columns per piece
-    static constexpr int CH = KW / 4;                                // 16-byte chunks per piece row
-    static constexpr uint32_t PIECE_BYTES = NB * KW * 4;
-    static constexpr uint32_t TILE_BYTES = NB * 2 * NB * 4;
-    static constexpr uint32_t STAGE_BYTES = (TILE_BYTES + 1023u) / 1024u * 1024u;
+    static constexpr uint32_t PART_FLOATS = NB * NB;                 // one part (Re or Im) of a tile: [k][i]
+    static constexpr uint32_t TILE_BYTES = 2 * NB * NB * 4;
+    static constexpr uint32_t STAGE_BYTES = (TILE_BYTES + 127u) / 128u * 128u;
     static constexpr int KSTEPS = NB / 8;
 };
 
@@ -139,18 +136,31 @@ __device__ __forceinline__ void tc_named_barrier(int id, int nthreads)
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// Optional per-role cycle accounting (compile with -DCMRHS_TC_TRACE; read back with coarse_debug_trace_read):
+// TW(k, wait) adds the cycles spent in `wait` to slot k of the warp's counters; slot 7 is the warp's total.
+#ifdef CMRHS_TC_TRACE
+__device__ long long g_tc_trace[160][32][8];
+#define TW(k, ...) do { const long long _t0 = clock64(); __VA_ARGS__; wt[k] += clock64() - _t0; } while (0)
+#define TW_BEGIN() const long long _tw = clock64()
+#define TW_END(k) wt[k] += clock64() - _tw
+#else
+#define TW(k, ...) do { __VA_ARGS__; } while (0)
+#define TW_BEGIN() do {} while (0)
+#define TW_END(k) do {} while (0)
+#endif
+
 template <int NB>
 __global__ void __launch_bounds__(kTcThreads, 1)
-stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmX, float2 *__restrict__ Y,
+stencil_tc_kernel(const float *__restrict__ Ak, const __grid_constant__ CUtensorMap tmX, float2 *__restrict__ Y,
                   const TcParams P)
 {
     using C = TcCfg<NB>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    // carve: [A ring][X ring (hi|lo per stage)][epilogue exchange][schedule tables][barriers][tmem slot]
+    // carve: [X ring (hi|lo per stage), 1024-byte aligned for the swizzle][A ring][epilogue exchange][schedule tables][barriers][tmem slot]
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);     // keeps the shared address space
-    unsigned char *ringA = smem;
-    unsigned char *ringX = ringA + (size_t)P.sa * C::STAGE_BYTES;
-    float4 *exch = reinterpret_cast<float4 *>(ringX + (size_t)P.sx * 2 * P.xt_bytes);      // [pair 2][buf 2][part 2][j 2][lane 32]
+    unsigned char *ringX = smem;
+    unsigned char *ringA = ringX + (size_t)P.sx * 2 * P.xt_bytes;
+    float4 *exch = reinterpret_cast<float4 *>(ringA + (size_t)P.sa * C::STAGE_BYTES);      // [pair 2][buf 2][part 2][j 2][lane 32]
     uint32_t *tab2 = reinterpret_cast<uint32_t *>(exch + 2 * 2 * 2 * 2 * 32);
     uint32_t *tab1 = tab2 + kTcMaxSteps;
     uint64_t *bars = reinterpret_cast<uint64_t *>(tab1 + kTcMaxSteps);
@@ -161,6 +171,10 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_empty + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#ifdef CMRHS_TC_TRACE
+    long long wt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long t_begin = clock64();
+#endif
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 2); }
@@ -171,90 +185,88 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
     if (threadIdx.x == 32) tc_build_schedule(2, tab2);
     if (threadIdx.x == 64) tc_build_schedule(1, tab1);
-    if (warp == 19) tmem_alloc_512(tmem_slot);
-    if (warp == 16 && lane == 0) tma_prefetch_desc(&tmA);
-    if (warp == 17 && lane == 0) tma_prefetch_desc(&tmX);
+    if (warp == 4 * kTcConvTurns + 11) tmem_alloc_512(tmem_slot);
+    if (warp == 4 * kTcConvTurns + 9 && lane == 0) tma_prefetch_desc(&tmX);
     tc_fence_before_sync();
     __syncthreads();
     tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
     const uint32_t acc_cols = (uint32_t)(P.nacc * P.acc_stride);
 
-    if (warp < 8) {
-        // ================= A converters: smem tile row -> TF32 hi/lo of the Re or Im panel -> TMEM =================
-        const int q = warp & 3, par = warp >> 2;
-        const int slot = q >> 1;
-        const bool im_part = (q & 1) != 0;
+    if (warp < 4 * kTcConvTurns) {
+        // ================= A converters: smem tile column k, row = lane -> TF32 hi/lo of the Re or Im panel -> TMEM =================
+        const int q = warp & 3, turn_mine = warp >> 2;
+        const int slot = q >> 1, part = q & 1;
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
-        const int i = lane;
-        const bool row_ok = i < NB;
-        const uint32_t row_off = (uint32_t)(row_ok ? i : 0) * (C::KW * 4);
+        const bool row_ok = lane < NB;
+        const uint32_t row_off = (uint32_t)part * C::PART_FLOATS + (uint32_t)(row_ok ? lane : 0);
         TcRing ra, rs;                  // ra: position of the NEXT tile of the tile sequence; rs: panel set of this step
-        uint32_t zero_sets = 0;         // panel sets whose lanes of this quarter currently hold zeros (only this warp writes them)
-        uint32_t gs = 0;                // global step counter: this warp converts the steps with gs % 2 == par
+        uint32_t zero_sets = 0;         // panel sets whose lanes of this quarter hold zeros (every warp of the quarter tracks all sets)
+        int turn = 0;                   // running step counter mod kTcConvTurns: the warp whose turn it is fills this step's set
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const TcGroup grp = tc_group(P, g, tab2, tab1);
-            for (int step = 0; step < grp.nsteps; ++step, ++gs) {
+            for (int step = 0; step < grp.nsteps; ++step) {
                 const uint32_t e = grp.tab[step];
                 const uint32_t um = (e >> 8) & 3u;
-                if ((gs & 1u) == (uint32_t)par) {
-                    const bool mine = (um >> slot) & 1u;
-                    mbar_wait(&set_empty[rs.stage], rs.phase ^ 1u);
+                const bool mine = (um >> slot) & 1u;
+                if (turn == turn_mine) {
+                    TW(0, mbar_wait(&set_empty[rs.stage], rs.phase ^ 1u));
                     tc_fence_after_sync();
+                    TW_BEGIN();
                     const uint32_t set_col = acc_cols + (uint32_t)rs.stage * kTcSetCols;
                     if (mine) {
                         TcRing mt = ra;                                   // my tile: sequence position + rank among the users
                         if (slot == 1 && (um & 1u)) mt.advance(P.sa);
-                        mbar_wait(&a_full[mt.stage], mt.phase);
-                        const unsigned char *tile = ringA + (size_t)mt.stage * C::STAGE_BYTES;
+                        TW(1, mbar_wait(&a_full[mt.stage], mt.phase));
+                        const float *col = reinterpret_cast<const float *>(ringA + (size_t)mt.stage * C::STAGE_BYTES) + row_off;
 #pragma unroll
-                        for (int h = 0; h < C::PIECES; ++h) {
-                            uint32_t hi[C::JP], lo[C::JP];
+                        for (int kc = 0; kc < NB / 8; ++kc) {
+                            float x[8];
 #pragma unroll
-                            for (int c = 0; c < C::CH; ++c) {
-                                const uint32_t off = (uint32_t)h * C::PIECE_BYTES + row_off + (uint32_t)c * 16u;
-                                const uint32_t phys = off ^ (((off >> 7) & C::SWZ_MASK) << 4);
-                                const float4 v = *reinterpret_cast<const float4 *>(tile + phys);
-                                float e0 = im_part ? v.y : v.x, e1 = im_part ? v.w : v.z;
-                                if (!row_ok) { e0 = 0.f; e1 = 0.f; }
-                                const float h0 = tf32_rn(e0), h1 = tf32_rn(e1);
-                                hi[2 * c] = __float_as_uint(h0); hi[2 * c + 1] = __float_as_uint(h1);
-                                lo[2 * c] = __float_as_uint(e0 - h0); lo[2 * c + 1] = __float_as_uint(e1 - h1);
+                            for (int u = 0; u < 8; ++u) x[u] = col[(kc * 8 + u) * NB];
+                            uint32_t hi[8], lo[8];
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                const float v = row_ok ? x[u] : 0.f;
+                                const float h = tf32_rn(v);
+                                hi[u] = __float_as_uint(h);
+                                lo[u] = __float_as_uint(v - h);
                             }
-                            const uint32_t col = set_col + (uint32_t)(h * C::JP);
-                            tmem_st<C::JP>(lane_base + col, hi);
-                            tmem_st<C::JP>(lane_base + col + 32u, lo);
+                            tmem_st_x8(lane_base + set_col + (uint32_t)(kc * 8), hi);
+                            tmem_st_x8(lane_base + set_col + 32u + (uint32_t)(kc * 8), lo);
                         }
                         __syncwarp();
                         if (lane == 0) mbar_arrive(&a_empty[mt.stage]);      // all lanes have read the tile
-                        zero_sets &= ~(1u << rs.stage);
                     } else if (!((zero_sets >> rs.stage) & 1u)) {
                         uint32_t zz[16];
 #pragma unroll
                         for (int k = 0; k < 16; ++k) zz[k] = 0u;
 #pragma unroll
                         for (int b = 0; b < kTcSetCols / 16; ++b) tmem_st_x16(lane_base + set_col + 16u * b, zz);
-                        zero_sets |= 1u << rs.stage;
                     }
                     tmem_wait_st();
                     tc_fence_before_sync();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&set_full[rs.stage]);
+                    TW_END(2);
                 }
+                zero_sets = mine ? (zero_sets & ~(1u << rs.stage)) : (zero_sets | (1u << rs.stage));
                 rs.advance(P.nset);
                 ra.advance(P.sa);
                 if (um == 3u) ra.advance(P.sa);
+                turn = (turn + 1 == kTcConvTurns) ? 0 : turn + 1;
             }
         }
-    } else if (warp < 12) {
+    } else if (warp < 4 * kTcConvTurns + 4) {
         // ================= X converters: round the tile to TF32 in place (hi), write the lo tile =================
-        const int tid = threadIdx.x - 256;
+        const int tid = threadIdx.x - 32 * 4 * kTcConvTurns;
         const int nchunks = P.nxb * NB * 8;     // 16-byte chunks per X tile (whole 128-byte rows, zero padded by TMA)
         TcRing rx;
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const int nsteps = (min(2, P.L[0] - (g % P.ng0) * 2) == 2) ? 110 : 81;
             for (int step = 0; step < nsteps; ++step) {
-                mbar_wait(&x_full[rx.stage], rx.phase);
+                TW(0, mbar_wait(&x_full[rx.stage], rx.phase));
+                TW_BEGIN();
                 unsigned char *hi_t = ringX + (size_t)rx.stage * 2 * P.xt_bytes;
                 unsigned char *lo_t = hi_t + P.xt_bytes;
                 int c = tid;
@@ -277,12 +289,13 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 fence_proxy_async_smem();       // generic-proxy writes -> visible to the tensor core's async-proxy reads
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&xlo_full[rx.stage]);
+                TW_END(1);
                 rx.advance(P.sx);
             }
         }
-    } else if (warp < 16) {
+    } else if (warp < 4 * kTcConvTurns + 8) {
         // ================= epilogue: Y = combine(D + C) -> global =================
-        const int q = warp - 12;
+        const int q = warp - (4 * kTcConvTurns + 4);      // = warp % 4: the TMEM lane quarter this warp may access
         const int slot = q >> 1, part = q & 1;
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
         float4 *xb = exch + slot * (2 * 2 * 2 * 32);
@@ -290,8 +303,9 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         uint32_t chunk_no = 0;          // running chunk counter: selects the exchange buffer
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const TcGroup grp = tc_group(P, g, tab2, tab1);
-            mbar_wait(&acc_full[rc.stage], rc.phase);
+            TW(0, mbar_wait(&acc_full[rc.stage], rc.phase));
             tc_fence_after_sync();
+            TW_BEGIN();
             if (slot < grp.G) {
                 const uint32_t d = lane_base + (uint32_t)(rc.stage * P.acc_stride), cacc = d + (uint32_t)P.N;
                 const int64_t site = tc_site(P, grp.x0 + slot, grp.y, grp.z, grp.t);
@@ -334,10 +348,11 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             tc_fence_before_sync();
             __syncwarp();
             if (lane == 0) mbar_arrive(&acc_empty[rc.stage]);
+            TW_END(1);
             rc.advance(P.nacc);
         }
-    } else if (warp == 16) {
-        // ================= A producer: one canonical stencil matrix per stage =================
+    } else if (warp == 4 * kTcConvTurns + 8) {
+        // ================= A producer: one stencil matrix (planar k-major tile, contiguous) per stage =================
         // (the whole warp walks the schedule so that every address stays warp-uniform; one elected lane issues)
         const uint64_t pol = l2_policy_evict_first();
         TcRing ra;
@@ -351,21 +366,18 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 for (int i = 0; i < 2; ++i) {
                     if (!((e >> (8 + i)) & 1u)) continue;
                     const int p = (int)((e >> (10 + 2 * i)) & 3u) + 3 * off3;
-                    const int64_t row0 = ((site0 + i) * kNPoint + p) * NB;
-                    mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u);
+                    const float *src = Ak + ((site0 + i) * kNPoint + p) * (int64_t)(2 * C::PART_FLOATS);
+                    TW(0, mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u));
                     if (elect_one_sync()) {
                         mbar_arrive_expect_tx(&a_full[ra.stage], C::TILE_BYTES);
-                        unsigned char *dst = ringA + (size_t)ra.stage * C::STAGE_BYTES;
-#pragma unroll
-                        for (int h = 0; h < C::PIECES; ++h)
-                            tma_load_2d(dst + h * C::PIECE_BYTES, &tmA, h * C::KW, (int32_t)row0, &a_full[ra.stage], pol);
+                        bulk_g2s(ringA + (size_t)ra.stage * C::STAGE_BYTES, src, C::TILE_BYTES, &a_full[ra.stage], pol);
                     }
                     __syncwarp();
                     ra.advance(P.sa);
                 }
             }
         }
-    } else if (warp == 17) {
+    } else if (warp == 4 * kTcConvTurns + 9) {
         // ================= X producer: the neighbour's X tile, once per step =================
         const uint64_t pol = l2_policy_evict_last();
         TcRing rx;
@@ -373,7 +385,7 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const TcGroup grp = tc_group(P, g, tab2, tab1);
             for (int step = 0; step < grp.nsteps; ++step) {
                 const int64_t row0 = tc_x_site(P, grp, grp.tab[step]) * NB;
-                mbar_wait(&x_empty[rx.stage], rx.phase ^ 1u);
+                TW(0, mbar_wait(&x_empty[rx.stage], rx.phase ^ 1u));
                 if (elect_one_sync()) {
                     mbar_arrive_expect_tx(&x_full[rx.stage], (uint32_t)P.x_tile_tx);
                     unsigned char *dst = ringX + (size_t)rx.stage * 2 * P.xt_bytes;
@@ -384,20 +396,21 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 rx.advance(P.sx);
             }
         }
-    } else if (warp == 18) {
+    } else if (warp == 4 * kTcConvTurns + 10) {
         // ================= MMA issuer =================
         // The whole warp runs the loop (all operands stay warp-uniform: no per-instruction broadcast loops in SASS);
         // one elected lane -- the same one every time -- issues the MMAs and the commits.
         TcRing rx, rs, rc;
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const int nsteps = (min(2, P.L[0] - (g % P.ng0) * 2) == 2) ? 110 : 81;
-            mbar_wait(&acc_empty[rc.stage], rc.phase ^ 1u);
+            TW(0, mbar_wait(&acc_empty[rc.stage], rc.phase ^ 1u));
             tc_fence_after_sync();
             const uint32_t d = tmem + (uint32_t)(rc.stage * P.acc_stride), cacc = d + (uint32_t)P.N;
             for (int step = 0; step < nsteps; ++step) {
-                mbar_wait(&set_full[rs.stage], rs.phase);
-                mbar_wait(&xlo_full[rx.stage], rx.phase);
+                TW(1, mbar_wait(&set_full[rs.stage], rs.phase));
+                TW(2, mbar_wait(&xlo_full[rx.stage], rx.phase));
                 tc_fence_after_sync();
+                TW_BEGIN();
                 if (elect_one_sync()) {
                     const uint32_t a_hi = tmem + acc_cols + (uint32_t)rs.stage * kTcSetCols, a_lo = a_hi + 32u;
                     const uint32_t xhi = smem_u32(ringX + (size_t)rx.stage * 2 * P.xt_bytes), xlo = xhi + (uint32_t)P.xt_bytes;
@@ -415,17 +428,24 @@ stencil_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     if (step == nsteps - 1) umma_commit(&acc_full[rc.stage]);
                 }
                 __syncwarp();
+                TW_END(3);
                 rs.advance(P.nset);
                 rx.advance(P.sx);
             }
             rc.advance(P.nacc);
         }
     }
+#ifdef CMRHS_TC_TRACE
+    if (lane == 0 && blockIdx.x < 160) {
+        wt[7] = clock64() - t_begin;
+        for (int k = 0; k < 8; ++k) g_tc_trace[blockIdx.x][warp][k] = wt[k];
+    }
+#endif
     // ---- teardown ----
     tc_fence_before_sync();
     __syncthreads();
     tc_fence_after_sync();
-    if (warp == 19) tmem_dealloc_512(tmem);
+    if (warp == 4 * kTcConvTurns + 11) tmem_dealloc_512(tmem);
 }
 
 // ---- host side ------------------------------------------------------------------------------------------------
@@ -466,7 +486,7 @@ inline int tc_make_tmap(CUtensorMap *out, const void *base, uint64_t width, uint
 inline bool tc_supported(int nb, int s) { return (nb == 8 || nb == 16 || nb == 24 || nb == 32) && s >= 8 && s <= 64 && s % 8 == 0; }
 
 template <int NB>
-int launch_stencil_tc(const CUtensorMap &tmA, const LatticeDims &d, const void *X, void *Y, int s, int num_sms, cudaStream_t stream)
+int launch_stencil_tc(const float *Ak, const LatticeDims &d, const void *X, void *Y, int s, int num_sms, cudaStream_t stream)
 {
     using C = TcCfg<NB>;
     if ((reinterpret_cast<uintptr_t>(X) & 15u) || (reinterpret_cast<uintptr_t>(Y) & 15u)) {
@@ -489,7 +509,7 @@ int launch_stencil_tc(const CUtensorMap &tmA, const LatticeDims &d, const void *
     if (P.nset > kTcMaxSets) P.nset = kTcMaxSets;
     P.nset &= ~1;                              // even: a converter warp owns the sets of its step parity
     P.sx = (2 * P.xt_bytes * 4 <= 96 * 1024) ? 4 : 3;
-    const int64_t fixed = 1024 /* alignment */ + 2 * 2 * 2 * 2 * 32 * 16 /* exchange */ + 2 * kTcMaxSteps * 4 + 1024 /* barriers */;
+    const int64_t fixed = 1024 /* alignment */ + 2 * 2 * 2 * 2 * 32 * 16 /* exchange */ + 2 * kTcMaxSteps * 4 + 1024 /* barriers */ + 128 /* A ring alignment */;
     const int64_t budget = 225 * 1024 - fixed - (int64_t)P.sx * 2 * P.xt_bytes;
     P.sa = (int32_t)(budget / C::STAGE_BYTES);
     if (P.sa > kTcMaxStagesA) P.sa = kTcMaxStagesA;
@@ -510,16 +530,26 @@ int launch_stencil_tc(const CUtensorMap &tmA, const LatticeDims &d, const void *
         attr_set = true;
     }
     const int grid = P.ngroups < num_sms ? P.ngroups : num_sms;
-    kern<<<grid, kTcThreads, smem, stream>>>(tmA, tmX, static_cast<float2 *>(Y), P);
+    kern<<<grid, kTcThreads, smem, stream>>>(Ak, tmX, static_cast<float2 *>(Y), P);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
 
-template <int NB> int tc_make_tmap_A(CUtensorMap *out, const void *A, int64_t V)
+// create-time re-layout for the tensor kernel: canonical A[t][i][k] (complex64, interleaved) -> planar k-major
+// Ak[t][part][k][i] (float32; part 0 = Re, 1 = Im).  One CTA per tile, coalesced writes.
+__global__ void relayout_planar_kernel(const cplx<float> *__restrict__ A, float *__restrict__ Ak, int64_t ntiles, int nb)
 {
-    using C = TcCfg<NB>;
-    return tc_make_tmap(out, A, (uint64_t)2 * NB, (uint64_t)V * kNPoint * NB, (uint32_t)C::KW, NB,
-                        C::KW == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B);
+    const int nn = nb * nb;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const cplx<float> *src = A + t * nn;
+        float *dst = Ak + t * 2 * nn;
+        for (int e = threadIdx.x; e < nn; e += blockDim.x) {
+            const int k = e / nb, i = e % nb;
+            const cplx<float> v = src[i * nb + k];
+            dst[e] = v.re;
+            dst[nn + e] = v.im;
+        }
+    }
 }
 
 }  // namespace cmrhs

@@ -124,15 +124,21 @@ def test_tensor_and_simt_kernels_agree():
     assert rel_err_cols(Yt, Ys) <= 2e-6
 
 
-def test_borrowed_and_copied_operator_give_identical_results():
-    # COARSE_FLAG_BORROW_A: the tensor kernel reads the caller's canonical A instead of an internal copy
+def test_tensor_only_operator_keeps_one_copy_and_rejects_uncovered_nrhs():
+    # COARSE_FLAG_TENSOR_ONLY: only the tensor kernel's layout of A is kept; nrhs it does not cover -> UNSUPPORTED
     dims, nb, s = (4, 3, 3, 4), 24, 16
     A, c, X, _ = host_case(dims, nb, s, seed=17, factor=1.02)
     Ad, Xd = to_dev(A, "c64"), to_dev(X, "c64")
-    outs = []
-    for flags in (0, cm.binding.FLAG_BORROW_A):
+    outs, sizes = [], []
+    for flags in (0, cm.binding.FLAG_TENSOR_ONLY):
         op = cm.CoarseOperator(dims, Ad, s, flags=flags)
         assert op.kernel_name(s).startswith("stencil_tc")
         outs.append(to_np(op.apply(Xd)))
+        sizes.append(op.device_bytes())
+        if flags:
+            with pytest.raises(cm.binding.CoarseError) as ei:
+                op.apply(Xd[:, :, :4].contiguous())
+            assert ei.value.status == cm.binding.UNSUPPORTED
         op.close()
     assert np.array_equal(outs[0], outs[1])
+    assert sizes[0] - sizes[1] == Ad.numel() * 8

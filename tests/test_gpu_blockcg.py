@@ -171,7 +171,7 @@ def test_block_cg_full_size_properties(index, nrhs):
         pytest.skip("not enough free device memory")
     A, c = cm.fill_synthetic(dims, nb, TORCH_DTYPE[dtype], cfg["seed"], cfg["factor"])
     B = cm.fill_block(dims, nb, nrhs, TORCH_DTYPE[dtype], cfg["seed"], synth.TAG_B)
-    op = cm.CoarseOperator(dims, A, nrhs)
+    op = cm.CoarseOperator(dims, A, nrhs, flags=cm.binding.FLAG_TENSOR_ONLY if index == 4 else 0)
     out = op.block_cg(B, tol=tol, maxiter=100)
     assert out["status"] == 0 and max(out["rel_res_true"]) <= tol * 1.001 + 2e-7
     # sampled true residual through the oracle
