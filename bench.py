@@ -66,8 +66,11 @@ def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         p = json.load(open(path))
-        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
-    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")        # B200_PROFILING.md fallback
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)),
+                    bf16_tflops=float(p.get("bf16_tflops", 1590.0)),
+                    bf16_tflops_sustained=float(p.get("bf16_tflops_sustained", p.get("bf16_tflops", 1400.0))), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0,
+                source="fallback")                                           # B200_PROFILING.md fallback
 
 
 def alu_peak_tflops(dtype, sm_mhz):
@@ -75,13 +78,29 @@ def alu_peak_tflops(dtype, sm_mhz):
     return SM_COUNT * lanes * 2.0 * sm_mhz * 1e6 / 1e12
 
 
-def roofline_tflops(V, nb, s, dtype, peaks):
+TF32_OVER_BF16 = 1.1 / 2.25     # nominal dense peaks (B200_PROFILING.md): the TF32 peak is the measured bf16 peak x this ratio
+TF32_SPLIT = 3                   # tcgen05 kind::tf32 products per algorithmic product (hi.hi + lo.hi + hi.lo)
+
+
+def tensor_peak_tflops(peaks, sustained):
+    """ALGORITHMIC TFLOP/s the split-TF32 tensor kernel could reach if the tensor pipe were the only limit:
+    measured bf16 GEMM peak (sustained figure for a kernel timed inside a long step) x nominal TF32/bf16 ratio / 3."""
+    bf16 = peaks["bf16_tflops_sustained"] if sustained else peaks["bf16_tflops"]
+    return bf16 * TF32_OVER_BF16 / TF32_SPLIT
+
+
+def roofline_tflops(V, nb, s, dtype, peaks, kernel="", sustained=True):
+    """min(pipe peak, intensity x HBM bandwidth) for the apply; the pipe is the tensor pipe for the tcgen05 kernel
+    (complex64, nrhs multiple of 8) and the FP32 / FP64 FMA pipe for the SIMT kernels."""
     esize = 8 if dtype == "c64" else 16
     intensity = apply_flops(V, nb, s) / apply_bytes(V, nb, s, esize)
     hbm = intensity * peaks["hbm_gbs"] / 1e3
-    alu = alu_peak_tflops(dtype, peaks["sm_max_mhz"])
-    return dict(intensity=intensity, hbm_tflops=hbm, alu_tflops=alu, roof_tflops=min(hbm, alu),
-                bound="hbm" if hbm <= alu else "alu")
+    if kernel.startswith("stencil_tc"):
+        pipe, pipe_name = tensor_peak_tflops(peaks, sustained), "tensor"
+    else:
+        pipe, pipe_name = alu_peak_tflops(dtype, peaks["sm_max_mhz"]), "alu"
+    return dict(intensity=intensity, hbm_tflops=hbm, pipe_tflops=pipe, roof_tflops=min(hbm, pipe),
+                bound="hbm" if hbm <= pipe else pipe_name)
 
 
 # ---- clocks during the timed region (B200_PROFILING.md "clocks line") ----------------------------------------
@@ -288,15 +307,17 @@ def run_ours(args, cfg):
         return 0
 
     # ---- roofline object: the stencil-GEMM apply, timed per launch inside the timed region -----------------
-    rf = roofline_tflops(V, nb, s, dtype, peaks)
+    rf = roofline_tflops(V, nb, s, dtype, peaks, kernel_name, sustained=True)
     a_ms = float(np.mean(apply_ms)) if apply_ms else float("nan")
     a_tflops = apply_flops(V, nb, s) / (a_ms * 1e-3) / 1e12
     a_gbs = apply_bytes(V, nb, s, esize) / (a_ms * 1e-3) / 1e9
     if rf["bound"] == "hbm":
         roofline = dict(bound="hbm", achieved=a_gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=a_gbs / peaks["hbm_gbs"])
     else:
-        roofline = dict(bound="alu", achieved=a_tflops, peak=rf["alu_tflops"], unit="TFLOP/s", frac=a_tflops / rf["alu_tflops"])
-    roofline.update(traffic=load_traffic(kernel_name), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
+        roofline = dict(bound=rf["bound"], achieved=a_tflops, peak=rf["pipe_tflops"], unit="TFLOP/s", frac=a_tflops / rf["pipe_tflops"],
+                        peak_note=("measured sustained bf16 GEMM x nominal TF32/bf16 (1.1/2.25) / 3 products per algorithmic product"
+                                   if rf["bound"] == "tensor" else "148 SMs x FMA lanes x 2 x max SM clock"))
+    roofline.update(traffic=load_traffic(f"{kernel_name}@nrhs{s}"), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
                     share_of_step=a_ms * len(apply_ms) / ms if apply_ms else None, peak_source=peaks["source"],
                     intensity_flop_per_byte=rf["intensity"], hbm_gbs_achieved=a_gbs,
                     frac_of_min_peak_IxBW=a_tflops / rf["roof_tflops"])
@@ -310,7 +331,7 @@ def run_ours(args, cfg):
             for _ in range(3):
                 op.apply(Xs, Ys)
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-            reps = 5
+            reps = 20
             torch.cuda.synchronize()
             ev[0].record()
             for _ in range(reps):
@@ -318,7 +339,7 @@ def run_ours(args, cfg):
             ev[1].record()
             torch.cuda.synchronize()
             t_ms = ev[0].elapsed_time(ev[1]) / reps
-            r = roofline_tflops(V, nb, sv, dtype, peaks)
+            r = roofline_tflops(V, nb, sv, dtype, peaks, op.kernel_name(sv), sustained=True)
             tf = apply_flops(V, nb, sv) / (t_ms * 1e-3) / 1e12
             sweep.append(dict(nrhs=sv, ms=t_ms, tflops=tf, hbm_gbs=apply_bytes(V, nb, sv, esize) / (t_ms * 1e-3) / 1e9,
                               roof_tflops=r["roof_tflops"], bound=r["bound"], frac=tf / r["roof_tflops"],
