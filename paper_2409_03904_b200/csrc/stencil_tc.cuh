@@ -34,7 +34,7 @@ namespace cmrhs {
 constexpr int kTcThreads = 768;
 constexpr int kTcConvTurns = 3;        // A converter warps per TMEM lane quarter
 constexpr int kTcMaxStagesA = 32;
-constexpr int kTcMaxStagesX = 4;
+constexpr int kTcMaxStagesX = 8;
 constexpr int kTcMaxSets = 6;
 constexpr int kTcSetCols = 64;          // TMEM columns of one operand panel set: hi at +0, lo at +32
 constexpr int kTcMaxSteps = 112;
@@ -51,8 +51,10 @@ struct TcParams {
     int32_t x_tile_tx;    // bytes TMA delivers per X tile
     int32_t sa, sx;       // ring depths
     int32_t nacc, nset;   // accumulator buffers, operand panel sets (even)
-    int32_t acc_stride;   // TMEM columns per accumulator buffer: D at +0, C at +N
+    int32_t acc_stride;   // TMEM columns per accumulator buffer: D at +0, C at +N (wide: D | C' | C'' at +0, +32, +64)
+    int32_t wide;         // 1: N <= 32, the X hi and lo tiles form one 64-column operand and A_hi meets both in ONE MMA
     uint32_t idesc;
+    uint32_t idesc_wide;  // M 128, N 64
     uint64_t xdesc_base;  // shared-memory descriptor of an X tile without the address
     uint32_t x_kadv;      // bytes between consecutive K = 8 steps of an X tile
 };
@@ -307,17 +309,25 @@ stencil_tc_kernel(const float *__restrict__ Ak, const __grid_constant__ CUtensor
             tc_fence_after_sync();
             TW_BEGIN();
             if (slot < grp.G) {
-                const uint32_t d = lane_base + (uint32_t)(rc.stage * P.acc_stride), cacc = d + (uint32_t)P.N;
+                const uint32_t d = lane_base + (uint32_t)(rc.stage * P.acc_stride), cacc = d + (uint32_t)(P.wide ? 32 : P.N);
                 const int64_t site = tc_site(P, grp.x0 + slot, grp.y, grp.z, grp.t);
                 float2 *yrow = Y + (site * NB + (lane < NB ? lane : 0)) * (int64_t)P.s;
                 for (int c = 0; c < P.N / 16; ++c, ++chunk_no) {
                     uint32_t a[16], b[16];
                     tmem_ld_x16(d + 16u * c, a);
                     tmem_ld_x16(cacc + 16u * c, b);
-                    tmem_wait_ld();
                     float v[16];
+                    if (P.wide) {
+                        uint32_t b2[16];
+                        tmem_ld_x16(d + 64u + 16u * c, b2);
+                        tmem_wait_ld();
 #pragma unroll
-                    for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(a[k]) + __uint_as_float(b[k]);
+                        for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(a[k]) + (__uint_as_float(b[k]) + __uint_as_float(b2[k]));
+                    } else {
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(a[k]) + __uint_as_float(b[k]);
+                    }
                     // the Re-panel warp finishes right-hand sides 8c..8c+3 and needs the partner's columns 0-7;
                     // the Im-panel warp finishes 8c+4..8c+7 and needs the partner's columns 8-15
                     float4 *buf = xb + (chunk_no & 1u) * (2 * 2 * 32);
@@ -419,9 +429,14 @@ stencil_tc_kernel(const float *__restrict__ Ak, const __grid_constant__ CUtensor
                         const uint64_t bh = umma_smem_desc(P.xdesc_base, xhi + ks * P.x_kadv);
                         const uint64_t bl = umma_smem_desc(P.xdesc_base, xlo + ks * P.x_kadv);
                         const uint32_t acc = (step | ks) != 0 ? 1u : 0u;
-                        umma_tf32_ts(d, a_hi + 8u * ks, bh, P.idesc, acc);       // A hi . X hi
-                        umma_tf32_ts(cacc, a_lo + 8u * ks, bh, P.idesc, acc);    // A lo . X hi
-                        umma_tf32_ts(cacc, a_hi + 8u * ks, bl, P.idesc, 1u);     // A hi . X lo
+                        if (P.wide) {
+                            umma_tf32_ts(d, a_hi + 8u * ks, bh, P.idesc_wide, acc);      // A hi . [X hi | X lo] -> D | C'
+                            umma_tf32_ts(d + 64u, a_lo + 8u * ks, bh, P.idesc, acc);     // A lo . X hi -> C''
+                        } else {
+                            umma_tf32_ts(d, a_hi + 8u * ks, bh, P.idesc, acc);       // A hi . X hi
+                            umma_tf32_ts(cacc, a_lo + 8u * ks, bh, P.idesc, acc);    // A lo . X hi
+                            umma_tf32_ts(cacc, a_hi + 8u * ks, bl, P.idesc, 1u);     // A hi . X lo
+                        }
                     }
                     umma_commit(&set_empty[rs.stage]);
                     umma_commit(&x_empty[rx.stage]);
@@ -503,18 +518,22 @@ int launch_stencil_tc(const float *Ak, const LatticeDims &d, const void *X, void
     P.x_tile_tx = P.nxb * NB * 128;           // TMA counts the whole box, out-of-range columns are zero filled
     P.xt_bytes = (P.x_tile_tx + 1023) / 1024 * 1024;
     // tensor memory: accumulator buffers of 2 N columns (main D | correction C), the rest in panel sets of 64 columns
-    P.acc_stride = 2 * P.N;
+    P.wide = (P.nxb == 1) ? 1 : 0;
+    P.acc_stride = P.wide ? 96 : 2 * P.N;
     P.nacc = (2 * P.acc_stride <= 256) ? 2 : 1;
     P.nset = (512 - P.nacc * P.acc_stride) / kTcSetCols;
     if (P.nset > kTcMaxSets) P.nset = kTcMaxSets;
-    P.nset &= ~1;                              // even: a converter warp owns the sets of its step parity
-    P.sx = (2 * P.xt_bytes * 4 <= 96 * 1024) ? 4 : 3;
+    // (any converter warp may fill any set: turns go by step mod 3, sets by step mod nset)
+    P.sx = 64 * 1024 / (2 * P.xt_bytes);
+    if (P.sx > kTcMaxStagesX) P.sx = kTcMaxStagesX;
+    if (P.sx < 3) P.sx = 3;
     const int64_t fixed = 1024 /* alignment */ + 2 * 2 * 2 * 2 * 32 * 16 /* exchange */ + 2 * kTcMaxSteps * 4 + 1024 /* barriers */ + 128 /* A ring alignment */;
     const int64_t budget = 225 * 1024 - fixed - (int64_t)P.sx * 2 * P.xt_bytes;
     P.sa = (int32_t)(budget / C::STAGE_BYTES);
     if (P.sa > kTcMaxStagesA) P.sa = kTcMaxStagesA;
     if (P.sa < 4 || P.nset < 2) { set_error("tensor path: shared/tensor memory plan does not fit (nb %d, nrhs %d)", NB, s); return COARSE_UNSUPPORTED; }
     P.idesc = umma_idesc_tf32(128, P.N, true);
+    P.idesc_wide = umma_idesc_tf32(128, 64, true);
     P.xdesc_base = umma_smem_desc_base((uint32_t)(NB * 128), 512u, 1u);     // LBO: next 32 columns, SBO: next 4 K rows
     P.x_kadv = 1024u;                                                         // 8 K rows
     const size_t smem = (size_t)fixed + (size_t)P.sa * C::STAGE_BYTES + (size_t)P.sx * 2 * P.xt_bytes;
