@@ -56,9 +56,13 @@ enum {
 enum {
     COARSE_FLAG_FORCE_GENERIC = 1u << 0, /* always use the generic (untiled) stencil kernel: test / debugging aid */
     COARSE_FLAG_NO_TENSOR = 1u << 1,     /* never select a tensor-core kernel variant */
-    COARSE_FLAG_TENSOR_ONLY = 1u << 2    /* complex64 shapes the tensor-core kernel covers: keep only its layout of A (one
+    COARSE_FLAG_TENSOR_ONLY = 1u << 2,   /* complex64 shapes the tensor-core kernel covers: keep only its layout of A (one
                                             internal copy instead of two); apply / solve with an nrhs that kernel does not
                                             cover (not a multiple of 8) then return COARSE_UNSUPPORTED */
+    COARSE_FLAG_TF32 = 1u << 3           /* complex64, nbasis 32: use the split-TF32 tensor kernel (operator kept as float32)
+                                            instead of the default split-FP16 kernel (operator stored pre-split as two
+                                            binary16 numbers per real: 22-23 significant bits, elements below 2^-29 of the
+                                            operator's largest element lose relative precision) */
 };
 
 #define COARSE_MAX_NRHS 64

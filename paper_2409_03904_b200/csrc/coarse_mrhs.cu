@@ -13,6 +13,7 @@
 #include "stencil_generic.cuh"
 #include "stencil_simt.cuh"
 #include "stencil_tc.cuh"
+#include "stencil_h16.cuh"
 
 namespace cmrhs {
 
@@ -76,6 +77,10 @@ struct coarse_op {
     void *At = nullptr;          // [V][81][nb(k)][nb(i)]
     float *Ak = nullptr;         // planar k-major [V][81][part][nb(k)][nb(i)] for the tensor path (complex64 only)
     bool tc_ok = false;
+    unsigned char *Ah = nullptr; // pre-split FP16 tiles [V][81][hi 4 KB | lo 4 KB] for the FP16-split tensor kernel (complex64, nbasis 32)
+    bool h16_ok = false;
+    float inv_sA = 1.0f;         // 1 / (power-of-two operator scale of Ah)
+    uint32_t *amax = nullptr;    // [64] per-column max |x| bit patterns (pre-pass of the FP16-split kernel) + [64] scratch
     int32_t *nbr = nullptr;      // [V][81]
     void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
     zdouble *gram_partial = nullptr;
@@ -146,6 +151,8 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     if (!op) return COARSE_OK;
     cudaFree(op->At);
     cudaFree(op->Ak);
+    cudaFree(op->Ah);
+    cudaFree(op->amax);
     cudaFree(op->nbr);
     for (void *b : op->blk) cudaFree(b);
     cudaFree(op->gram_partial);
@@ -195,10 +202,15 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
         }                                    \
     } while (0)
     const bool want_tc = dtype == COARSE_C64 && !(flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) && tc_supported(nbasis, 8);
+    const bool want_h16 = want_tc && !(flags & COARSE_FLAG_TF32) && h16_supported(nbasis, 8);
     const bool want_simt = !(want_tc && (flags & COARSE_FLAG_TENSOR_ONLY));
     if (want_simt) CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
-    if (want_tc) CMRHS_TRY(alloc_dev(op, (void **)&op->Ak, a_bytes));
+    if (want_tc && !want_h16) CMRHS_TRY(alloc_dev(op, (void **)&op->Ak, a_bytes));
+    if (want_h16) {
+        CMRHS_TRY(alloc_dev(op, (void **)&op->Ah, a_bytes));
+        CMRHS_TRY(alloc_dev(op, (void **)&op->amax, 128 * sizeof(uint32_t)));
+    }
     for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
     CMRHS_TRY(alloc_dev(op, (void **)&op->small, (size_t)6 * COARSE_MAX_NRHS * COARSE_MAX_NRHS * sizeof(zdouble)));
@@ -223,10 +235,31 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
             relayout_transpose_kernel<double><<<rgrid, 128, 0, stream>>>((const cplx<double> *)A_dev, (cplx<double> *)op->At, ntiles, nbasis);
         count_launch();
     }
-    if (want_tc) {
+    if (want_tc && !want_h16) {
         relayout_planar_kernel<<<rgrid, 128, 0, stream>>>((const cplx<float> *)A_dev, op->Ak, ntiles, nbasis);
         count_launch();
         op->tc_ok = true;
+    }
+    if (want_h16) {
+        // operator scale: the power of two that maps max |Re a|, |Im a| into [2^14, 2^15) (stencil_h16.cuh)
+        uint32_t bits = 0;
+        ce = cudaMemsetAsync(op->amax, 0, 128 * sizeof(uint32_t), stream);
+        if (ce == cudaSuccess) {
+            absmax_kernel<<<op->num_sms * 8, 256, 0, stream>>>((const float *)A_dev, (int64_t)ntiles * nbasis * nbasis * 2, op->amax + 64);
+            count_launch();
+            ce = cudaMemcpyAsync(&bits, op->amax + 64, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream);
+        }
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(stream);
+        if (ce != cudaSuccess) {
+            set_error("operator scale pass failed: %s", cudaGetErrorString(ce));
+            coarse_op_destroy(op);
+            return COARSE_CUDA_ERROR;
+        }
+        const float sA = h_scale_from_bits(bits);
+        op->inv_sA = 1.0f / sA;
+        relayout_h16_kernel<<<rgrid, 256, 0, stream>>>((const cplx<float> *)A_dev, op->Ah, ntiles, sA);
+        count_launch();
+        op->h16_ok = true;
     }
     ce = cudaGetLastError();
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(stream);
@@ -248,10 +281,12 @@ static const SimtVariant *select_variant(const coarse_op *op, int nrhs)
 }
 
 static bool use_tc(const coarse_op *op, int nrhs) { return op->tc_ok && tc_supported(op->nb, nrhs); }
+static bool use_h16(const coarse_op *op, int nrhs) { return op->h16_ok && h16_supported(op->nb, nrhs); }
 
 extern "C" const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs)
 {
     if (!op) return "";
+    if (use_h16(op, nrhs)) return "stencil_h16<fp16x3>";
     if (use_tc(op, nrhs)) return "stencil_tc<tf32x3>";
     if (!op->At) return "unsupported";
     const SimtVariant *v = select_variant(op, nrhs);
@@ -274,6 +309,7 @@ static int apply_impl(const coarse_op *op_c, const void *X, void *Y, int nrhs, c
 
 static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream)
 {
+    if (use_h16(op, nrhs)) return launch_stencil_h16(op->Ah, op->inv_sA, op->amax, op->dims, X, Y, nrhs, op->num_sms, stream);
     if (use_tc(op, nrhs)) {
         switch (op->nb) {
         case 8: return launch_stencil_tc<8>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);

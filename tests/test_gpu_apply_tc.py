@@ -27,7 +27,7 @@ import paper_2409_03904_b200 as cm  # noqa: E402
 
 def _apply_tc(dims, A, X, nrhs_max=None):
     s = X.shape[-1]
-    op = cm.CoarseOperator(dims, to_dev(A, "c64"), nrhs_max or s)
+    op = cm.CoarseOperator(dims, to_dev(A, "c64"), nrhs_max or s, flags=cm.binding.FLAG_TF32)    # nbasis 32 defaults to the FP16-split kernel
     name = op.kernel_name(s)
     assert name.startswith("stencil_tc"), name
     Y = to_np(op.apply(to_dev(X, "c64")))
