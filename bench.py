@@ -79,14 +79,16 @@ def alu_peak_tflops(dtype, sm_mhz):
 
 
 TF32_OVER_BF16 = 1.1 / 2.25     # nominal dense peaks (B200_PROFILING.md): the TF32 peak is the measured bf16 peak x this ratio
-TF32_SPLIT = 3                   # tcgen05 kind::tf32 products per algorithmic product (hi.hi + lo.hi + hi.lo)
+SPLIT_PRODUCTS = 3               # tensor-core products per algorithmic product (hi.hi + lo.hi + hi.lo, DESIGN.md 5.3 / 5.4)
 
 
-def tensor_peak_tflops(peaks, sustained):
-    """ALGORITHMIC TFLOP/s the split-TF32 tensor kernel could reach if the tensor pipe were the only limit:
-    measured bf16 GEMM peak (sustained figure for a kernel timed inside a long step) x nominal TF32/bf16 ratio / 3."""
+def tensor_peak_tflops(peaks, sustained, kernel):
+    """ALGORITHMIC TFLOP/s a split-precision tensor kernel could reach if the tensor pipe were the only limit:
+    measured bf16 GEMM peak (sustained figure for a kernel timed inside a long step; binary16 runs at the bf16 rate)
+    [x nominal TF32/bf16 ratio for the TF32 kernel] / 3 products."""
     bf16 = peaks["bf16_tflops_sustained"] if sustained else peaks["bf16_tflops"]
-    return bf16 * TF32_OVER_BF16 / TF32_SPLIT
+    ratio = TF32_OVER_BF16 if kernel.startswith("stencil_tc") else 1.0
+    return bf16 * ratio / SPLIT_PRODUCTS
 
 
 def roofline_tflops(V, nb, s, dtype, peaks, kernel="", sustained=True):
@@ -95,8 +97,8 @@ def roofline_tflops(V, nb, s, dtype, peaks, kernel="", sustained=True):
     esize = 8 if dtype == "c64" else 16
     intensity = apply_flops(V, nb, s) / apply_bytes(V, nb, s, esize)
     hbm = intensity * peaks["hbm_gbs"] / 1e3
-    if kernel.startswith("stencil_tc"):
-        pipe, pipe_name = tensor_peak_tflops(peaks, sustained), "tensor"
+    if kernel.startswith(("stencil_tc", "stencil_h16")):
+        pipe, pipe_name = tensor_peak_tflops(peaks, sustained, kernel), "tensor"
     else:
         pipe, pipe_name = alu_peak_tflops(dtype, peaks["sm_max_mhz"]), "alu"
     return dict(intensity=intensity, hbm_tflops=hbm, pipe_tflops=pipe, roof_tflops=min(hbm, pipe),
@@ -315,7 +317,7 @@ def run_ours(args, cfg):
         roofline = dict(bound="hbm", achieved=a_gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=a_gbs / peaks["hbm_gbs"])
     else:
         roofline = dict(bound=rf["bound"], achieved=a_tflops, peak=rf["pipe_tflops"], unit="TFLOP/s", frac=a_tflops / rf["pipe_tflops"],
-                        peak_note=("measured sustained bf16 GEMM x nominal TF32/bf16 (1.1/2.25) / 3 products per algorithmic product"
+                        peak_note=("measured sustained bf16 GEMM [x nominal TF32/bf16 (1.1/2.25) for the TF32 kernel] / 3 products per algorithmic product"
                                    if rf["bound"] == "tensor" else "148 SMs x FMA lanes x 2 x max SM clock"))
     roofline.update(traffic=load_traffic(f"{kernel_name}@nrhs{s}"), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
                     share_of_step=a_ms * len(apply_ms) / ms if apply_ms else None, peak_source=peaks["source"],

@@ -80,6 +80,7 @@ struct coarse_op {
     unsigned char *Ah = nullptr; // pre-split FP16 tiles [V][81][hi 4 KB | lo 4 KB] for the FP16-split tensor kernel (complex64, nbasis 32)
     bool h16_ok = false;
     float inv_sA = 1.0f;         // 1 / (power-of-two operator scale of Ah)
+    unsigned char *Xh = nullptr; // [V] split operand tiles of the current X (pre-pass of the FP16-split kernel)
     uint32_t *amax = nullptr;    // [64] per-column max |x| bit patterns (pre-pass of the FP16-split kernel) + [64] scratch
     int32_t *nbr = nullptr;      // [V][81]
     void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
@@ -152,6 +153,7 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     cudaFree(op->At);
     cudaFree(op->Ak);
     cudaFree(op->Ah);
+    cudaFree(op->Xh);
     cudaFree(op->amax);
     cudaFree(op->nbr);
     for (void *b : op->blk) cudaFree(b);
@@ -210,6 +212,9 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
     if (want_h16) {
         CMRHS_TRY(alloc_dev(op, (void **)&op->Ah, a_bytes));
         CMRHS_TRY(alloc_dev(op, (void **)&op->amax, 128 * sizeof(uint32_t)));
+        const size_t xh_bytes = (size_t)V * h16_xo_bytes(nrhs_max < 8 ? 8 : nrhs_max);
+        CMRHS_TRY(alloc_dev(op, (void **)&op->Xh, xh_bytes));
+        CMRHS_CUDA(cudaMemsetAsync(op->Xh, 0, xh_bytes, stream));       // padding columns of the tiles are never written again
     }
     for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
@@ -309,7 +314,7 @@ static int apply_impl(const coarse_op *op_c, const void *X, void *Y, int nrhs, c
 
 static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream)
 {
-    if (use_h16(op, nrhs)) return launch_stencil_h16(op->Ah, op->inv_sA, op->amax, op->dims, X, Y, nrhs, op->num_sms, stream);
+    if (use_h16(op, nrhs)) return launch_stencil_h16(op->Ah, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream);
     if (use_tc(op, nrhs)) {
         switch (op->nb) {
         case 8: return launch_stencil_tc<8>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);

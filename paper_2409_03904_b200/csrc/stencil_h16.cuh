@@ -23,13 +23,14 @@
 #pragma once
 
 #include <cuda_fp16.h>
+#include <stdlib.h>
 
 #include "stencil_tc.cuh"
 
 namespace cmrhs {
 
-// warp roles: XW X converters | 4 epilogue | A producer | X producer | MMA issuer | TMEM allocator.  Two shapes:
-// <8 converter warps, 1 CTA per SM> for wide X tiles, <4, 2> (two independent pipelines per SM) for narrow ones.
+// warp roles: 4 epilogue | A producer | X producer | MMA issuer | TMEM allocator; 1-3 CTAs (independent pipelines) per SM
+constexpr int kHThreads = 256;
 constexpr int kHMaxStagesA = 24;
 constexpr int kHMaxStagesX = 8;
 constexpr int kHMaxAcc = 4;
@@ -42,13 +43,11 @@ struct HParams {
     int32_t s;            // nrhs (multiple of 8)
     int32_t N2;           // 2 s: real columns of an X tile
     int32_t LO;           // operand column of the lo half: 2 s if 4 s <= 64 (hi | lo share one 64-column atom), else a multiple of 64
-    int32_t wideN;        // LO + 2 s: N of the A_hi MMA ([X_hi | X_lo]); C'' sits at TMEM column wideN
+    int32_t wideN;        // LO + 2 s: N of the A_hi MMA ([X_hi | X_lo] -> D | C); the A_lo . X_hi MMA adds into C (TMEM column LO)
     int32_t acc_stride, nacc;
     int32_t tmem_cols;    // 512 (one CTA per SM) or 256 (two)
-    int32_t sa, sxs, sxo; // ring depths: A tiles, X fp32 staging, X fp16 operand
-    int32_t xs_bytes;     // fp32 X tile: 32 * s * 8
-    int32_t xo_bytes;     // fp16 operand stage: atoms * 4096
-    int32_t nchunks;      // 8-column chunks per X tile: 32 * (2 s / 8)
+    int32_t sa, sxo;      // ring depths: A tiles, X operand tiles
+    int32_t xo_bytes;     // fp16 X operand tile: atoms * 4096
     uint32_t idesc_wide, idesc_lo;
     float inv_sA;         // 1 / sA
     const uint32_t *amax; // [s] bit patterns of max |Re|, |Im| per column of X (pre-pass)
@@ -121,29 +120,26 @@ __device__ __forceinline__ int64_t h_x_site(const HParams &P, const TcGroup &g, 
     return h_site(P, tc_wrap(g.x0 + j - 1, P.L[0]), tc_wrap(g.y + dy, P.L[1]), tc_wrap(g.z + dz, P.L[2]), tc_wrap(g.t + dt, P.L[3]));
 }
 
-template <int kHXconvWarps, int kCtasPerSm>
-__global__ void __launch_bounds__(32 * (kHXconvWarps + 8), kCtasPerSm)
-stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict__ X, float2 *__restrict__ Y, const HParams P)
+template <int kCtasPerSm>
+__global__ void __launch_bounds__(kHThreads, kCtasPerSm)
+stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__restrict__ Xh, float2 *__restrict__ Y, const HParams P)
 {
     constexpr int NB = 32;
-    constexpr int kHThreads = 32 * (kHXconvWarps + 8);
+    constexpr int kHXconvWarps = 0;          // (role offsets: the X operand arrives ready-made, nothing converts on chip)
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    // carve: [zeros 2 KB][A ring][zeros 2 KB][X operand ring][X staging ring][epilogue exchange][tables][scales][barriers][tmem slot]
+    // carve: [zeros 2 KB][A ring][zeros 2 KB][X operand ring][epilogue exchange][tables][scales][barriers][tmem slot]
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     unsigned char *zero0 = smem;
     unsigned char *ringA = zero0 + kHZero;
     unsigned char *zero1 = ringA + (size_t)P.sa * kHTile;
     unsigned char *ringXo = zero1 + kHZero;
-    unsigned char *ringXs = ringXo + (size_t)P.sxo * P.xo_bytes;
-    float4 *exch = reinterpret_cast<float4 *>(ringXs + (size_t)P.sxs * P.xs_bytes);         // [pair 2][buf 2][part 2][j 2][lane 32]
+    float4 *exch = reinterpret_cast<float4 *>(ringXo + (size_t)P.sxo * P.xo_bytes);         // [pair 2][buf 2][part 2][j 2][lane 32]
     uint32_t *tab2 = reinterpret_cast<uint32_t *>(exch + 2 * 2 * 2 * 2 * 32);
     uint32_t *tab1 = tab2 + kTcMaxSteps;
-    float *scl = reinterpret_cast<float *>(tab1 + kTcMaxSteps);      // [128] per real column: sX_r
-    float *inv = scl + 128;                                           // [128] 1 / (sA sX_r)
+    float *inv = reinterpret_cast<float *>(tab1 + kTcMaxSteps);      // [128] per real column: 1 / (sA sX_r)
     uint64_t *bars = reinterpret_cast<uint64_t *>(inv + 128);
     uint64_t *a_full = bars, *a_empty = a_full + kHMaxStagesA;
-    uint64_t *xs_full = a_empty + kHMaxStagesA, *xs_empty = xs_full + kHMaxStagesX;
-    uint64_t *xo_full = xs_empty + kHMaxStagesX, *xo_empty = xo_full + kHMaxStagesX;
+    uint64_t *xo_full = a_empty + kHMaxStagesA, *xo_empty = xo_full + kHMaxStagesX;
     uint64_t *acc_full = xo_empty + kHMaxStagesX, *acc_empty = acc_full + kHMaxAcc;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_empty + kHMaxAcc);
 
@@ -155,8 +151,7 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
-        for (int i = 0; i < P.sxs; ++i) { mbar_init(&xs_full[i], 1); mbar_init(&xs_empty[i], kHXconvWarps / 2); }
-        for (int i = 0; i < P.sxo; ++i) { mbar_init(&xo_full[i], kHXconvWarps / 2); mbar_init(&xo_empty[i], 1); }
+        for (int i = 0; i < P.sxo; ++i) { mbar_init(&xo_full[i], 1); mbar_init(&xo_empty[i], 1); }
         for (int i = 0; i < P.nacc; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 4); }
         mbar_fence_init();
     }
@@ -165,7 +160,6 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
     if (threadIdx.x >= 128 && threadIdx.x < 256) {
         const int col = threadIdx.x - 128;
         const float sc = col < P.N2 ? h_scale_from_bits(P.amax[col >> 1]) : 1.0f;
-        scl[col] = sc;
         inv[col] = P.inv_sA / sc;
     }
     for (int e = threadIdx.x; e < (int)(kHZero / 16); e += kHThreads) {
@@ -179,56 +173,7 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
     tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
 
-    if (warp < kHXconvWarps) {
-        // ================= X converters: fp32 tile -> scaled fp16 hi | lo operand (MN-major, SWIZZLE_128B) =================
-        // two teams of kHXconvWarps / 2 warps take the steps in turn: each team has two step times per tile
-        constexpr int TW_ = kHXconvWarps / 2, TS = 32 * TW_;
-        const int team = warp / TW_, tid = threadIdx.x - team * TS;
-        const int gpr = P.N2 >> 3;              // 8-column chunks per K row
-        TcRing rs, ro;
-        uint32_t turn = 0;
-        auto convert = [&](const float *src, unsigned char *dst, int c) {
-            const int k = c / gpr, col0 = (c - k * gpr) << 3;
-            const float4 v0 = *reinterpret_cast<const float4 *>(src + k * P.N2 + col0);
-            const float4 v1 = *reinterpret_cast<const float4 *>(src + k * P.N2 + col0 + 4);
-            const float4 s0 = *reinterpret_cast<const float4 *>(scl + col0);
-            const float4 s1 = *reinterpret_cast<const float4 *>(scl + col0 + 4);
-            const float x[8] = {v0.x * s0.x, v0.y * s0.y, v0.z * s0.z, v0.w * s0.w, v1.x * s1.x, v1.y * s1.y, v1.z * s1.z, v1.w * s1.w};
-            uint32_t hw[4], lw[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const __half2 h = __floats2half2_rn(x[2 * u], x[2 * u + 1]);
-                const float2 hf = __half22float2(h);
-                const __half2 l = __floats2half2_rn((x[2 * u] - hf.x) * 2048.0f, (x[2 * u + 1] - hf.y) * 2048.0f);
-                hw[u] = *reinterpret_cast<const uint32_t *>(&h);
-                lw[u] = *reinterpret_cast<const uint32_t *>(&l);
-            }
-            *reinterpret_cast<uint4 *>(dst + h_swz((uint32_t)k, (uint32_t)col0)) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
-            *reinterpret_cast<uint4 *>(dst + h_swz((uint32_t)k, (uint32_t)(P.LO + col0))) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
-        };
-        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-            const int nsteps = (min(2, P.L[0] - (g % P.ng0) * 2) == 2) ? 110 : 81;
-            for (int step = 0; step < nsteps; ++step, turn ^= 1u) {
-                if ((int)turn == team) {
-                    TW(0, mbar_wait(&xs_full[rs.stage], rs.phase));
-                    TW(1, mbar_wait(&xo_empty[ro.stage], ro.phase ^ 1u));
-                    tc_fence_after_sync();
-                    TW_BEGIN();
-                    const float *src = reinterpret_cast<const float *>(ringXs + (size_t)rs.stage * P.xs_bytes);
-                    unsigned char *dst = ringXo + (size_t)ro.stage * P.xo_bytes;
-                    int c = tid;
-                    for (; c + TS < P.nchunks; c += 2 * TS) { convert(src, dst, c); convert(src, dst, c + TS); }
-                    if (c < P.nchunks) convert(src, dst, c);
-                    fence_proxy_async_smem();       // generic-proxy writes -> visible to the tensor core's async-proxy reads
-                    __syncwarp();
-                    if (lane == 0) { mbar_arrive(&xo_full[ro.stage]); mbar_arrive(&xs_empty[rs.stage]); }
-                    TW_END(2);
-                }
-                rs.advance(P.sxs);
-                ro.advance(P.sxo);
-            }
-        }
-    } else if (warp < kHXconvWarps + 4) {
+    if (warp < 4) {
         // ================= epilogue: Y = combine((D + 2^-11 (C' + C'')) / (sA sX)) -> global =================
         const int q = warp - kHXconvWarps;                 // = warp % 4: the TMEM lane quarter this warp may access
         const int slot = q >> 1, part = q & 1;
@@ -243,19 +188,17 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
             TW_BEGIN();
             if (slot < grp.G) {
                 const uint32_t d = lane_base + (uint32_t)(rc.stage * P.acc_stride);
-                const uint32_t c1 = d + (uint32_t)P.LO, c2 = d + (uint32_t)P.wideN;
+                const uint32_t c2 = d + (uint32_t)P.LO;
                 const int64_t site = h_site(P, grp.x0 + slot, grp.y, grp.z, grp.t);
                 float2 *yrow = Y + (site * NB + lane) * (int64_t)P.s;
                 for (int c = 0; c < P.N2 / 16; ++c, ++chunk_no) {
-                    uint32_t a[16], b[16], b2[16];
-                    tmem_ld_x16(d + 16u * c, a);
-                    tmem_ld_x16(c1 + 16u * c, b);
-                    tmem_ld_x16(c2 + 16u * c, b2);
-                    tmem_wait_ld();
+                    uint32_t a[16], b[16];
                     float v[16];
+                    tmem_ld_x16(d + 16u * c, a);
+                    tmem_ld_x16(c2 + 16u * c, b);
+                    tmem_wait_ld();
 #pragma unroll
-                    for (int k = 0; k < 16; ++k)
-                        v[k] = (__uint_as_float(a[k]) + (__uint_as_float(b[k]) + __uint_as_float(b2[k])) * (1.0f / 2048.0f)) * inv[16 * c + k];
+                    for (int k = 0; k < 16; ++k) v[k] = (__uint_as_float(a[k]) + __uint_as_float(b[k]) * (1.0f / 2048.0f)) * inv[16 * c + k];
                     float4 *buf = xb + (chunk_no & 1u) * (2 * 2 * 32);
                     if (part == 0) {
                         buf[0 * 32 + lane] = make_float4(v[8], v[9], v[10], v[11]);
@@ -321,20 +264,20 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
             }
         }
     } else if (warp == kHXconvWarps + 5) {
-        // ================= X producer: the neighbour's fp32 X tile (contiguous), once per step =================
+        // ================= X producer: the neighbour's ready-made fp16 operand tile (contiguous), once per step =================
         const uint64_t pol = l2_policy_evict_last();
-        TcRing rs;
+        TcRing ro;
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const TcGroup grp = h_group(P, g, tab2, tab1);
             for (int step = 0; step < grp.nsteps; ++step) {
-                const float *src = X + h_x_site(P, grp, grp.tab[step]) * (int64_t)(NB * P.N2);
-                TW(0, mbar_wait(&xs_empty[rs.stage], rs.phase ^ 1u));
+                const unsigned char *src = Xh + h_x_site(P, grp, grp.tab[step]) * (int64_t)P.xo_bytes;
+                TW(0, mbar_wait(&xo_empty[ro.stage], ro.phase ^ 1u));
                 if (elect_one_sync()) {
-                    mbar_arrive_expect_tx(&xs_full[rs.stage], (uint32_t)P.xs_bytes);
-                    bulk_g2s(ringXs + (size_t)rs.stage * P.xs_bytes, src, (uint32_t)P.xs_bytes, &xs_full[rs.stage], pol);
+                    mbar_arrive_expect_tx(&xo_full[ro.stage], (uint32_t)P.xo_bytes);
+                    bulk_g2s(ringXo + (size_t)ro.stage * P.xo_bytes, src, (uint32_t)P.xo_bytes, &xo_full[ro.stage], pol);
                 }
                 __syncwarp();
-                rs.advance(P.sxs);
+                ro.advance(P.sxo);
             }
         }
     } else if (warp == kHXconvWarps + 6) {
@@ -345,7 +288,7 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
             const TcGroup grp = h_group(P, g, tab2, tab1);
             TW(0, mbar_wait(&acc_empty[rc.stage], rc.phase ^ 1u));
             tc_fence_after_sync();
-            const uint32_t d = tmem + (uint32_t)(rc.stage * P.acc_stride), c2 = d + (uint32_t)P.wideN;
+            const uint32_t d = tmem + (uint32_t)(rc.stage * P.acc_stride), c2 = d + (uint32_t)P.LO;
             for (int step = 0; step < grp.nsteps; ++step) {
                 const uint32_t um = (grp.tab[step] >> 8) & 3u;
                 if (um == 3u && ra.stage == P.sa - 1) {            // the pair would wrap: pass over the last stage
@@ -372,8 +315,8 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const float *__restrict
                         if (um == 3u) { ad_hi = h_desc(hi, kHTile); ad_lo = h_desc(lo, kHTile); }
                         else if (um == 1u) { ad_hi = h_desc(hi, z1 - hi); ad_lo = h_desc(lo, z1 - lo); }      // site 1's atom: zeros
                         else { ad_hi = h_desc(z0, hi - z0); ad_lo = h_desc(z0, lo - z0); }                    // site 0's atom: zeros
-                        umma_f16_ss(d, ad_hi, bd, P.idesc_wide, acc);       // A hi . [X hi | X lo] -> D | C'
-                        umma_f16_ss(c2, ad_lo, bd, P.idesc_lo, acc);        // A lo . X hi -> C''
+                        umma_f16_ss(d, ad_hi, bd, P.idesc_wide, acc);       // A hi . [X hi | X lo] -> D | C
+                        umma_f16_ss(c2, ad_lo, bd, P.idesc_lo, 1u);         // A lo . X hi -> C (same columns, issued after)
                     }
                     umma_commit(&xo_empty[ro.stage]);
                     umma_commit(&a_empty[st0]);
@@ -467,8 +410,46 @@ __global__ void __launch_bounds__(256) relayout_h16_kernel(const cplx<float> *__
     }
 }
 
-inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *amax_dev, const LatticeDims &d, const void *X, void *Y,
-                              int s, int num_sms, cudaStream_t stream)
+// per-apply pre-pass 2: X (fp32, [site][k = basis row][2 s real columns]) -> Xh, one ready-made operand tile per site:
+// the MN-major SWIZZLE_128B shared-memory image of [X_hi | X_lo] (scaled by the column's power of two, split into
+// hi = fp16(x), lo = fp16(2^11 (x - hi))).  Every X tile is read by ~40 groups of sites; it is converted once, here.
+__global__ void __launch_bounds__(256) xsplit_kernel(const float *__restrict__ X, unsigned char *__restrict__ Xh, const uint32_t *__restrict__ amax,
+                                                     int64_t nsites, int s, int LO, int xo_bytes)
+{
+    __shared__ float scl[128];
+    const int N2 = 2 * s, gpr = N2 >> 3, nchunks = 32 * gpr;
+    if (threadIdx.x < 128) scl[threadIdx.x] = threadIdx.x < N2 ? h_scale_from_bits(amax[threadIdx.x >> 1]) : 1.0f;
+    __syncthreads();
+    for (int64_t site = blockIdx.x; site < nsites; site += gridDim.x) {
+        const float *src = X + site * (int64_t)(32 * N2);
+        unsigned char *dst = Xh + site * (int64_t)xo_bytes;
+        for (int c = threadIdx.x; c < nchunks; c += 256) {
+            const int k = c / gpr, col0 = (c - k * gpr) << 3;
+            const float4 v0 = *reinterpret_cast<const float4 *>(src + k * N2 + col0);
+            const float4 v1 = *reinterpret_cast<const float4 *>(src + k * N2 + col0 + 4);
+            const float4 s0 = *reinterpret_cast<const float4 *>(scl + col0);
+            const float4 s1 = *reinterpret_cast<const float4 *>(scl + col0 + 4);
+            const float x[8] = {v0.x * s0.x, v0.y * s0.y, v0.z * s0.z, v0.w * s0.w, v1.x * s1.x, v1.y * s1.y, v1.z * s1.z, v1.w * s1.w};
+            uint32_t hw[4], lw[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const __half2 h = __floats2half2_rn(x[2 * u], x[2 * u + 1]);
+                const float2 hf = __half22float2(h);
+                const __half2 l = __floats2half2_rn((x[2 * u] - hf.x) * 2048.0f, (x[2 * u + 1] - hf.y) * 2048.0f);
+                hw[u] = *reinterpret_cast<const uint32_t *>(&h);
+                lw[u] = *reinterpret_cast<const uint32_t *>(&l);
+            }
+            *reinterpret_cast<uint4 *>(dst + h_swz((uint32_t)k, (uint32_t)col0)) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+            *reinterpret_cast<uint4 *>(dst + h_swz((uint32_t)k, (uint32_t)(LO + col0))) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+        }
+    }
+}
+
+// bytes of one X operand tile for nrhs = s
+inline int h16_xo_bytes(int s) { return (4 * s <= 64) ? 4096 : 2 * ((2 * s + 63) / 64) * 4096; }
+
+inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *amax_dev, unsigned char *Xh, const LatticeDims &d, const void *X,
+                              void *Y, int s, int num_sms, cudaStream_t stream)
 {
     if ((reinterpret_cast<uintptr_t>(X) & 15u) || (reinterpret_cast<uintptr_t>(Y) & 15u)) {
         set_error("tensor path: X and Y must be 16-byte aligned");
@@ -480,24 +461,23 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     P.ngroups = (int32_t)((int64_t)P.ng0 * d.L[1] * d.L[2] * d.L[3]);
     P.s = s;
     P.N2 = 2 * s;
-    int natoms;
-    if (4 * s <= 64) { P.LO = 2 * s; natoms = 1; }
-    else { const int wa = (2 * s + 63) / 64; P.LO = 64 * wa; natoms = 2 * wa; }
+    if (4 * s <= 64) P.LO = 2 * s;
+    else P.LO = 64 * ((2 * s + 63) / 64);
     P.wideN = P.LO + 2 * s;
-    P.acc_stride = P.wideN + 2 * s;
-    const bool two = P.acc_stride <= 256 && s <= 32;       // two CTAs (pipelines) per SM: 256 TMEM columns and half the shared memory each
-    P.tmem_cols = two ? 256 : 512;
+    P.acc_stride = P.wideN;
+    // independent pipelines (CTAs) per SM: as many as tensor memory (power-of-two allocations) and shared memory allow
+    int cps = P.acc_stride <= 128 ? 3 : (P.acc_stride <= 256 ? 2 : 1);
+    if (const char *e = getenv("CMRHS_H16_CPS")) { const int v = atoi(e); if (v >= 1 && v < cps) cps = v; }
+    P.tmem_cols = cps == 3 ? 128 : (cps == 2 ? 256 : 512);
     P.nacc = P.tmem_cols / P.acc_stride;
     if (P.nacc > kHMaxAcc) P.nacc = kHMaxAcc;
-    P.xo_bytes = natoms * 4096;
-    P.xs_bytes = 32 * s * 8;
-    P.nchunks = 8 * s;
+    P.xo_bytes = h16_xo_bytes(s);
     auto clampi = [](int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); };
-    P.sxo = clampi((two ? 16384 : 49152) / P.xo_bytes, 3, kHMaxStagesX);
-    P.sxs = clampi((two ? 16384 : 49152) / P.xs_bytes, 3, kHMaxStagesX);
-    const int64_t fixed = 1024 /* alignment */ + 2 * kHZero + 2 * 2 * 2 * 2 * 32 * 16 /* exchange */ + 2 * kTcMaxSteps * 4 + 1024 /* scales */ +
+    const int smem_cta = cps == 3 ? 74 * 1024 : (cps == 2 ? 113 * 1024 : 227 * 1024);
+    P.sxo = clampi(smem_cta / 5 / P.xo_bytes, 3, kHMaxStagesX);
+    const int64_t fixed = 1024 /* alignment */ + 2 * kHZero + 2 * 2 * 2 * 2 * 32 * 16 /* exchange */ + 2 * kTcMaxSteps * 4 + 512 /* scales */ +
                           1024 /* barriers */ + 64;
-    const int64_t budget = (two ? 113 : 227) * 1024 - fixed - (int64_t)P.sxo * P.xo_bytes - (int64_t)P.sxs * P.xs_bytes;
+    const int64_t budget = smem_cta - fixed - (int64_t)P.sxo * P.xo_bytes;
     P.sa = (int32_t)(budget / kHTile);
     if (P.sa > kHMaxStagesA) P.sa = kHMaxStagesA;
     if (P.sa < 4 || P.nacc < 1) { set_error("tensor path: shared/tensor memory plan does not fit (nrhs %d)", s); return COARSE_UNSUPPORTED; }
@@ -505,28 +485,32 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     P.idesc_lo = umma_idesc_f16_mn(128, P.N2);
     P.inv_sA = inv_sA;
     P.amax = amax_dev;
-    const size_t smem = (size_t)fixed + (size_t)P.sa * kHTile + (size_t)P.sxo * P.xo_bytes + (size_t)P.sxs * P.xs_bytes;
+    const size_t smem = (size_t)fixed + (size_t)P.sa * kHTile + (size_t)P.sxo * P.xo_bytes;
 
-    // pre-pass: per-column max |x| -> the power-of-two column scales (computed in the kernel's prologue)
+    // pre-passes over X: per-column max |x| (-> power-of-two column scales), then the split operand tiles
     CMRHS_CUDA(cudaMemsetAsync(amax_dev, 0, 64 * sizeof(uint32_t), stream));
     const int64_t n = d.V * 32;
     const int rpp = 256 / s;
-    int cgrid = (int)(ceil_div(n, rpp) < (int64_t)num_sms * 8 ? ceil_div(n, rpp) : (int64_t)num_sms * 8);
+    const int cgrid = (int)(ceil_div(n, rpp) < (int64_t)num_sms * 8 ? ceil_div(n, rpp) : (int64_t)num_sms * 8);
     colmax_kernel<<<cgrid, 256, 0, stream>>>(static_cast<const float2 *>(X), n, s, amax_dev);
+    CMRHS_LAUNCH_CHECK();
+    const int xgrid = (int)(d.V < (int64_t)num_sms * 8 ? d.V : (int64_t)num_sms * 8);
+    xsplit_kernel<<<xgrid, 256, 0, stream>>>(static_cast<const float *>(X), Xh, amax_dev, d.V, s, P.LO, P.xo_bytes);
     CMRHS_LAUNCH_CHECK();
 
     static bool attr_set = false;
     if (!attr_set) {
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(113 * 1024)));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
         attr_set = true;
     }
-    const int slots = two ? 2 * num_sms : num_sms;
+    const int slots = cps * num_sms;
     const int grid = P.ngroups < slots ? P.ngroups : slots;
-    if (two)
-        stencil_h16_kernel<4, 2><<<grid, 32 * 12, smem, stream>>>(Ah, static_cast<const float *>(X), static_cast<float2 *>(Y), P);
-    else
-        stencil_h16_kernel<8, 1><<<grid, 32 * 16, smem, stream>>>(Ah, static_cast<const float *>(X), static_cast<float2 *>(Y), P);
+    float2 *Yp = static_cast<float2 *>(Y);
+    if (cps == 3) stencil_h16_kernel<3><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
+    else if (cps == 2) stencil_h16_kernel<2><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
+    else stencil_h16_kernel<1><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
