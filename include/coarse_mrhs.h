@@ -59,10 +59,12 @@ enum {
     COARSE_FLAG_TENSOR_ONLY = 1u << 2,   /* complex64 shapes the tensor-core kernel covers: keep only its layout of A (one
                                             internal copy instead of two); apply / solve with an nrhs that kernel does not
                                             cover (not a multiple of 8) then return COARSE_UNSUPPORTED */
-    COARSE_FLAG_TF32 = 1u << 3           /* complex64, nbasis 32: use the split-TF32 tensor kernel (operator kept as float32)
+    COARSE_FLAG_TF32 = 1u << 3,          /* complex64, nbasis 32: use the split-TF32 tensor kernel (operator kept as float32)
                                             instead of the default split-FP16 kernel (operator stored pre-split as two
                                             binary16 numbers per real: 22-23 significant bits, elements below 2^-29 of the
                                             operator's largest element lose relative precision) */
+    COARSE_FLAG_UNFUSED_LINALG = 1u << 4 /* block_cg_*: run the block rotations and Gram products of an iteration as six
+                                            separate kernels instead of the two fused passes (cross-check / debugging aid) */
 };
 
 #define COARSE_MAX_NRHS 64

@@ -109,14 +109,15 @@ gram_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W
 }
 
 // stage 2: G[e] = sum_b partial[b][e], b in increasing order
+// One warp per entry: lane l sums blocks l, l + 32, ... in increasing order, then a fixed shuffle tree.
 __global__ void gram_reduce_kernel(const zdouble *__restrict__ partial, int nblocks, int ss, zdouble *__restrict__ G)
 {
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (e >= ss) return;
     double re = 0.0, im = 0.0;
-    for (int b = 0; b < nblocks; ++b) { re += partial[(size_t)b * ss + e].re; im += partial[(size_t)b * ss + e].im; }
-    G[e].re = re;
-    G[e].im = im;
+    for (int b = lane; b < nblocks; b += 32) { re += partial[(size_t)b * ss + e].re; im += partial[(size_t)b * ss + e].im; }
+    for (int o = 16; o > 0; o >>= 1) { re += __shfl_down_sync(0xffffffffu, re, o); im += __shfl_down_sync(0xffffffffu, im, o); }
+    if (lane == 0) { G[e].re = re; G[e].im = im; }
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -165,6 +166,216 @@ rotate_kernel(const cplx<T> *U, const zdouble *__restrict__ K, const cplx<T> *Vi
                         if (beta != (T)0) { const cplx<T> w = Vin[e]; v.re = fma(beta, w.re, v.re); v.im = fma(beta, w.im, v.im); }
                         out[e] = v;
                     }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// The two fused passes of one BlockCGrQ iteration (Fig. 2 left, statements 10-13):
+//   pass 1:  X += D K1 ;  T = Q + Z K2 ;  partial(T^H T)          reads D, Z, Q, X   writes X, T
+//   pass 2:  Q = T K3 ;  D = Q + D K4                             reads T, D         writes Q, D
+// (K1 = M C, K2 = -M, K3 = S^-1, K4 = S^H, complex128 on the device, rounded to T at use: DESIGN.md R11.)
+// 10 block passes over HBM instead of the 15 of the unfused sequence (gram, rotate x 4, gram).
+// Thread layout: the s columns are cut into groups of W; a thread owns TR rows x W columns of each product
+// (row lanes interleaved so a warp touches consecutive rows); the Gram part of pass 1 uses W x W sub-blocks of
+// T^H T per thread and the row groups that are left, products in T, sums flushed to double once per row tile.
+// ------------------------------------------------------------------------------------------------------
+template <typename T> struct LaPad { static constexpr int v = sizeof(T) == 4 ? 2 : 1; };   // keeps rows 16-byte aligned, banks spread
+
+// rows r0 .. r0 + nrow of a row-major n x s block -> shared memory with leading dimension su (coalesced)
+template <typename T>
+__device__ __forceinline__ void la_stage_rows(cplx<T> *dst, const cplx<T> *__restrict__ src, int64_t r0, int nrow, int s, int su)
+{
+    const int rpp = kLaThreads / s, row0 = threadIdx.x / s, col = threadIdx.x - row0 * s;
+    if (row0 < rpp)
+        for (int r = row0; r < nrow; r += rpp) dst[r * su + col] = src[(r0 + r) * s + col];
+}
+
+// acc[t][c] = sum_a sU[(rl + t RL)][a] * sK[a][c0 + c]
+template <typename T, int TR, int W>
+__device__ __forceinline__ void la_tile_product(cplx<T> (&acc)[TR][W], const cplx<T> *sU, const cplx<T> *sK, int rl, int RL, int c0, int s, int su)
+{
+#pragma unroll
+    for (int t = 0; t < TR; ++t)
+#pragma unroll
+        for (int c = 0; c < W; ++c) { acc[t][c].re = 0; acc[t][c].im = 0; }
+    for (int a = 0; a < s; ++a) {
+        cplx<T> u[TR], k[W];
+#pragma unroll
+        for (int t = 0; t < TR; ++t) u[t] = sU[(rl + t * RL) * su + a];
+#pragma unroll
+        for (int c = 0; c < W; ++c) k[c] = (c0 + c < s) ? sK[a * s + c0 + c] : cplx<T>{0, 0};
+#pragma unroll
+        for (int t = 0; t < TR; ++t)
+#pragma unroll
+            for (int c = 0; c < W; ++c) cmac(acc[t][c], u[t], k[c]);
+    }
+}
+
+template <typename T, int TR, int W>
+__global__ void __launch_bounds__(kLaThreads)
+bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Q, cplx<T> *X, cplx<T> *Tout,
+                  const zdouble *__restrict__ K1, const zdouble *__restrict__ K2, int64_t n, int s, zdouble *__restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int su = s + LaPad<T>::v;
+    const int ncg = (s + W - 1) / W, RL = kLaThreads / ncg, rows = RL * TR;
+    cplx<T> *sK1 = reinterpret_cast<cplx<T> *>(smem_raw), *sK2 = sK1 + s * s;
+    cplx<T> *sD = sK2 + s * s, *sZ = sD + (size_t)rows * su;            // sD is reused for the T tile
+    for (int e = threadIdx.x; e < s * s; e += kLaThreads) {
+        sK1[e].re = (T)K1[e].re; sK1[e].im = (T)K1[e].im;
+        sK2[e].re = (T)K2[e].re; sK2[e].im = (T)K2[e].im;
+    }
+    const int cg = threadIdx.x % ncg, rl = threadIdx.x / ncg, c0 = cg * W;
+    const bool rot_active = rl < RL;
+    // Gram layout: W x W sub-blocks, RG row groups
+    const int ntile = ncg * ncg, RG = kLaThreads / ntile;
+    const int gt = threadIdx.x % ntile, rg = threadIdx.x / ntile;
+    const bool gram_active = rg < RG;
+    const int ga0 = (gt / ncg) * W, gb0 = (gt % ncg) * W;
+    double accr[W][W], acci[W][W];
+#pragma unroll
+    for (int a = 0; a < W; ++a)
+#pragma unroll
+        for (int b = 0; b < W; ++b) { accr[a][b] = 0.0; acci[a][b] = 0.0; }
+
+    const int64_t ntiles = (n + rows - 1) / rows;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t r0 = t * rows;
+        const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
+        __syncthreads();                                   // previous tile's Gram reads of sD are done (and sK is written)
+        la_stage_rows(sD, D, r0, nrow, s, su);
+        la_stage_rows(sZ, Z, r0, nrow, s, su);
+        for (int e = threadIdx.x + nrow * su; e < rows * su; e += kLaThreads) { sD[e] = {0, 0}; sZ[e] = {0, 0}; }   // ragged tail: zero rows
+        __syncthreads();
+        cplx<T> tv[TR][W];
+        if (rot_active) {
+            cplx<T> acc[TR][W];
+            la_tile_product<T, TR, W>(acc, sD, sK1, rl, RL, c0, s, su);          // D K1
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt) {
+                const int row = rl + tt * RL;
+                if (row < nrow)
+#pragma unroll
+                    for (int c = 0; c < W; ++c)
+                        if (c0 + c < s) {
+                            const int64_t e = (r0 + row) * s + c0 + c;
+                            cplx<T> x = X[e];
+                            x.re += acc[tt][c].re; x.im += acc[tt][c].im;
+                            X[e] = x;
+                        }
+            }
+            la_tile_product<T, TR, W>(tv, sZ, sK2, rl, RL, c0, s, su);           // Z K2
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt) {
+                const int row = rl + tt * RL;
+#pragma unroll
+                for (int c = 0; c < W; ++c) {
+                    if (row < nrow && c0 + c < s) {
+                        const int64_t e = (r0 + row) * s + c0 + c;
+                        const cplx<T> q = Q[e];
+                        tv[tt][c].re += q.re; tv[tt][c].im += q.im;
+                        Tout[e] = tv[tt][c];
+                    } else { tv[tt][c].re = 0; tv[tt][c].im = 0; }
+                }
+            }
+        }
+        __syncthreads();                                   // all reads of sD (as D) are done
+        if (rot_active) {
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt)
+#pragma unroll
+                for (int c = 0; c < W; ++c)
+                    if (c0 + c < s) sD[(rl + tt * RL) * su + c0 + c] = tv[tt][c];
+        }
+        __syncthreads();
+        if (gram_active) {
+            cplx<T> run[W][W];
+#pragma unroll
+            for (int a = 0; a < W; ++a)
+#pragma unroll
+                for (int b = 0; b < W; ++b) { run[a][b].re = 0; run[a][b].im = 0; }
+            for (int k = rg; k < nrow; k += RG) {
+                cplx<T> u[W], w[W];
+#pragma unroll
+                for (int a = 0; a < W; ++a) u[a] = (ga0 + a < s) ? sD[k * su + ga0 + a] : cplx<T>{0, 0};
+#pragma unroll
+                for (int b = 0; b < W; ++b) w[b] = (gb0 + b < s) ? sD[k * su + gb0 + b] : cplx<T>{0, 0};
+#pragma unroll
+                for (int a = 0; a < W; ++a)
+#pragma unroll
+                    for (int b = 0; b < W; ++b) cmac_conj(run[a][b], u[a], w[b]);
+            }
+#pragma unroll
+            for (int a = 0; a < W; ++a)
+#pragma unroll
+                for (int b = 0; b < W; ++b) { accr[a][b] += (double)run[a][b].re; acci[a][b] += (double)run[a][b].im; }
+        }
+    }
+    // reduce the row groups in a fixed order through shared memory (the tile buffers are free now)
+    __syncthreads();
+    double *red = reinterpret_cast<double *>(sD);
+    for (int g = 0; g < RG; ++g) {
+        if (gram_active && rg == g) {
+#pragma unroll
+            for (int a = 0; a < W; ++a)
+#pragma unroll
+                for (int b = 0; b < W; ++b)
+                    if (ga0 + a < s && gb0 + b < s) {
+                        const int e = (ga0 + a) * s + gb0 + b;
+                        if (g == 0) { red[2 * e] = accr[a][b]; red[2 * e + 1] = acci[a][b]; }
+                        else { red[2 * e] += accr[a][b]; red[2 * e + 1] += acci[a][b]; }
+                    }
+        }
+        __syncthreads();
+    }
+    zdouble *out = partial + (size_t)blockIdx.x * s * s;
+    for (int e = threadIdx.x; e < s * s; e += kLaThreads) { out[e].re = red[2 * e]; out[e].im = red[2 * e + 1]; }
+}
+
+template <typename T, int TR, int W>
+__global__ void __launch_bounds__(kLaThreads)
+bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, const zdouble *__restrict__ K3, const zdouble *__restrict__ K4,
+                  int64_t n, int s)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int su = s + LaPad<T>::v;
+    const int ncg = (s + W - 1) / W, RL = kLaThreads / ncg, rows = RL * TR;
+    cplx<T> *sK3 = reinterpret_cast<cplx<T> *>(smem_raw), *sK4 = sK3 + s * s;
+    cplx<T> *sT = sK4 + s * s, *sD = sT + (size_t)rows * su;
+    for (int e = threadIdx.x; e < s * s; e += kLaThreads) {
+        sK3[e].re = (T)K3[e].re; sK3[e].im = (T)K3[e].im;
+        sK4[e].re = (T)K4[e].re; sK4[e].im = (T)K4[e].im;
+    }
+    const int cg = threadIdx.x % ncg, rl = threadIdx.x / ncg, c0 = cg * W;
+    const int64_t ntiles = (n + rows - 1) / rows;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t r0 = t * rows;
+        const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
+        __syncthreads();
+        la_stage_rows(sT, Tin, r0, nrow, s, su);
+        la_stage_rows(sD, D, r0, nrow, s, su);
+        for (int e = threadIdx.x + nrow * su; e < rows * su; e += kLaThreads) { sT[e] = {0, 0}; sD[e] = {0, 0}; }
+        __syncthreads();
+        if (rl < RL) {
+            cplx<T> q[TR][W], d[TR][W];
+            la_tile_product<T, TR, W>(q, sT, sK3, rl, RL, c0, s, su);            // Q = T S^-1
+            la_tile_product<T, TR, W>(d, sD, sK4, rl, RL, c0, s, su);            // D S^H
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt) {
+                const int row = rl + tt * RL;
+                if (row < nrow)
+#pragma unroll
+                    for (int c = 0; c < W; ++c)
+                        if (c0 + c < s) {
+                            const int64_t e = (r0 + row) * s + c0 + c;
+                            Qout[e] = q[tt][c];
+                            cplx<T> v;
+                            v.re = q[tt][c].re + d[tt][c].re;
+                            v.im = q[tt][c].im + d[tt][c].im;
+                            D[e] = v;                                            // D = Q + D S^H (this CTA staged its rows of D first)
+                        }
             }
         }
     }

@@ -194,7 +194,7 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
     const int64_t ntiles = V * kNPoint;
     const size_t a_bytes = (size_t)ntiles * nbasis * nbasis * op->esize;
     const size_t blk_bytes = (size_t)V * nbasis * nrhs_max * op->esize;
-    op->gram_blocks = op->num_sms * 2;
+    op->gram_blocks = op->num_sms * 8;
 #define CMRHS_TRY(expr)                      \
     do {                                     \
         int _s = (expr);                     \
@@ -369,10 +369,13 @@ extern "C" int coarse_op_apply_host(coarse_op_t *op, const void *X_host, void *Y
 template <typename T>
 static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble *G, int64_t n, int s, cudaStream_t stream)
 {
-    const int TT = (s + 15) / 16;
+    int TT = s > 32 ? 4 : (s >= 8 ? 2 : 1);
+    if (const char *e = getenv("CMRHS_GRAM_TT")) { const int v = atoi(e); if (v >= 1 && v <= 4 && (s + v - 1) / v <= 16) TT = v; }
     const int nt = (s + TT - 1) / TT;
     const int RG = kLaThreads / (nt * nt);
-    int rows = (int)(40960 / (2 * (size_t)s * sizeof(cplx<T>)));
+    size_t tile_bytes = 40960;
+    if (const char *e = getenv("CMRHS_GRAM_SMEM")) { const int v = atoi(e); if (v >= 2048 && v <= 65536) tile_bytes = (size_t)v; }
+    int rows = (int)(tile_bytes / (2 * (size_t)s * sizeof(cplx<T>)));
     rows = rows / RG * RG;
     if (rows < RG) rows = RG;
     size_t smem = (size_t)rows * s * 2 * sizeof(cplx<T>);
@@ -395,7 +398,7 @@ static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble 
     }
 #undef CMRHS_GRAM_CASE
     CMRHS_LAUNCH_CHECK();
-    gram_reduce_kernel<<<(s * s + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, s * s, G);
+    gram_reduce_kernel<<<(s * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, s * s, G);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
@@ -438,6 +441,95 @@ static int rotate_dispatch(const coarse_op *op, const void *U, const zdouble *K,
 {
     return op->dtype == COARSE_C64 ? rotate_impl<float>(op, U, K, Vin, out, beta, n, s, stream)
                                    : rotate_impl<double>(op, U, K, Vin, out, beta, n, s, stream);
+}
+
+// ---- the two fused passes of a BlockCGrQ iteration (blockcg_kernels.cuh) ---------------------------------
+struct FusedPlan { int W, TR, rows, grid; size_t smem; };
+
+template <typename T>
+static FusedPlan fused_plan(const coarse_op *op, int64_t n, int s)
+{
+    FusedPlan p;
+    p.W = s >= 8 ? 2 : 1;
+    if (const char *e = getenv("CMRHS_LA_W")) { const int v = atoi(e); if (v == 1 || v == 2 || v == 4) p.W = v; }
+    if ((s + p.W - 1) / p.W > 16) p.W = 4;
+    const int ncg = (s + p.W - 1) / p.W, RL = kLaThreads / ncg, su = s + LaPad<T>::v;
+    int tr0 = 2;
+    if (const char *e = getenv("CMRHS_LA_TR")) { const int v = atoi(e); if (v == 1 || v == 2 || v == 4) tr0 = v; }
+    for (p.TR = tr0; ; p.TR /= 2) {
+        p.rows = RL * p.TR;
+        size_t tiles = (size_t)2 * p.rows * su * sizeof(cplx<T>);
+        const size_t red = (size_t)s * s * sizeof(zdouble);
+        if (tiles < red) tiles = red;
+        p.smem = (size_t)2 * s * s * sizeof(cplx<T>) + tiles;
+        if (p.smem <= 100 * 1024 || p.TR == 1) break;      // two CTAs per SM when possible
+    }
+    int per_sm = p.smem <= 27 * 1024 ? 8 : (p.smem <= 56 * 1024 ? 4 : (p.smem <= 113 * 1024 ? 2 : 1));
+    if (const char *e = getenv("CMRHS_LA_PERSM")) { const int v = atoi(e); if (v >= 1 && v <= 8) per_sm = v; }
+    const int64_t ntiles = ceil_div(n, p.rows);
+    int64_t g = (int64_t)op->num_sms * per_sm;
+    if (g > op->gram_blocks) g = op->gram_blocks;
+    p.grid = (int)(ntiles < g ? ntiles : g);
+    return p;
+}
+
+template <typename T, int TR, int W>
+static int fused1_launch(const coarse_op *op, const FusedPlan &p, const void *D, const void *Z, const void *Q, void *X, void *Tout,
+                         const zdouble *K1, const zdouble *K2, int64_t n, int s, cudaStream_t stream)
+{
+    auto kern = bcg_fused1_kernel<T, TR, W>;
+    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
+    kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)D, (const cplx<T> *)Z, (const cplx<T> *)Q, (cplx<T> *)X, (cplx<T> *)Tout, K1, K2,
+                                                  n, s, op->gram_partial);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+template <typename T, int TR, int W>
+static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Tin, void *D, void *Qout, const zdouble *K3, const zdouble *K4,
+                         int64_t n, int s, cudaStream_t stream)
+{
+    auto kern = bcg_fused2_kernel<T, TR, W>;
+    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
+    kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)Tin, (cplx<T> *)D, (cplx<T> *)Qout, K3, K4, n, s);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+#define CMRHS_FUSED_SWITCH(CALL)                                         \
+    if (p.TR == 4) {                                                     \
+        if (p.W == 4) return CALL(4, 4); if (p.W == 2) return CALL(4, 2); return CALL(4, 1); \
+    }                                                                    \
+    if (p.TR == 2) {                                                     \
+        if (p.W == 4) return CALL(2, 4); if (p.W == 2) return CALL(2, 2); return CALL(2, 1); \
+    }                                                                    \
+    if (p.W == 4) return CALL(1, 4); if (p.W == 2) return CALL(1, 2); return CALL(1, 1);
+
+// X += D K1 ; T = Q + Z K2 ; G = T^H T   (G through the deterministic two-stage reduction)
+template <typename T>
+static int fused1_impl(const coarse_op *op, const void *D, const void *Z, const void *Q, void *X, void *Tout, const zdouble *K1,
+                       const zdouble *K2, zdouble *G, int64_t n, int s, cudaStream_t stream)
+{
+    const FusedPlan p = fused_plan<T>(op, n, s);
+    auto run = [&]() -> int {
+#define CMRHS_F1(TRV, WV) fused1_launch<T, TRV, WV>(op, p, D, Z, Q, X, Tout, K1, K2, n, s, stream)
+        CMRHS_FUSED_SWITCH(CMRHS_F1)
+#undef CMRHS_F1
+    };
+    int st = run();
+    if (st != COARSE_OK) return st;
+    gram_reduce_kernel<<<(s * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, p.grid, s * s, G);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+// Q = T K3 ; D = Q + D K4
+template <typename T>
+static int fused2_impl(const coarse_op *op, const void *Tin, void *D, void *Qout, const zdouble *K3, const zdouble *K4, int64_t n, int s,
+                       cudaStream_t stream)
+{
+    const FusedPlan p = fused_plan<T>(op, n, s);
+#define CMRHS_F2(TRV, WV) fused2_launch<T, TRV, WV>(op, p, Tin, D, Qout, K3, K4, n, s, stream)
+    CMRHS_FUSED_SWITCH(CMRHS_F2)
+#undef CMRHS_F2
 }
 
 static int axpby_dispatch(const coarse_op *op, const void *U, const void *W, void *out, double a, double b, int64_t total,
@@ -568,12 +660,22 @@ static int bcg_step(coarse_op *op, cudaStream_t stream)
     CMRHS_STEP(apply_impl(op, D, Z, s, stream));                                   // Z_k = H D_k
     CMRHS_STEP(gram_dispatch(op, D, Z, w.G, n, s, stream));                        // D^H Z
     CMRHS_STEP(small_launch(bcg_step1_kernel, op, s, 3, stream));                  // M, K1 = M C, K2 = -M
-    CMRHS_STEP(rotate_dispatch(op, D, w.K1, X, X, 1.0, n, s, stream));             // X += D M C
-    CMRHS_STEP(rotate_dispatch(op, Z, w.K2, Q, T, 1.0, n, s, stream));             // T = Q - Z M
-    CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));                        // T^H T
-    CMRHS_STEP(small_launch(bcg_step2_kernel, op, s, 3, stream));                  // S, K3 = S^-1, K4 = S^H, C = S C
-    CMRHS_STEP(rotate_dispatch(op, T, w.K3, nullptr, Q, 0.0, n, s, stream));       // Q = T S^-1
-    CMRHS_STEP(rotate_dispatch(op, D, w.K4, Q, D, 1.0, n, s, stream));             // D = Q + D S^H
+    if (op->flags & COARSE_FLAG_UNFUSED_LINALG) {
+        CMRHS_STEP(rotate_dispatch(op, D, w.K1, X, X, 1.0, n, s, stream));             // X += D M C
+        CMRHS_STEP(rotate_dispatch(op, Z, w.K2, Q, T, 1.0, n, s, stream));             // T = Q - Z M
+        CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));                        // T^H T
+        CMRHS_STEP(small_launch(bcg_step2_kernel, op, s, 3, stream));                  // S, K3 = S^-1, K4 = S^H, C = S C
+        CMRHS_STEP(rotate_dispatch(op, T, w.K3, nullptr, Q, 0.0, n, s, stream));       // Q = T S^-1
+        CMRHS_STEP(rotate_dispatch(op, D, w.K4, Q, D, 1.0, n, s, stream));             // D = Q + D S^H
+    } else if (op->dtype == COARSE_C64) {
+        CMRHS_STEP(fused1_impl<float>(op, D, Z, Q, X, T, w.K1, w.K2, w.G, n, s, stream));   // X += D M C ; T = Q - Z M ; T^H T
+        CMRHS_STEP(small_launch(bcg_step2_kernel, op, s, 3, stream));                        // S, K3 = S^-1, K4 = S^H, C = S C
+        CMRHS_STEP(fused2_impl<float>(op, T, D, Q, w.K3, w.K4, n, s, stream));               // Q = T S^-1 ; D = Q + D S^H
+    } else {
+        CMRHS_STEP(fused1_impl<double>(op, D, Z, Q, X, T, w.K1, w.K2, w.G, n, s, stream));
+        CMRHS_STEP(small_launch(bcg_step2_kernel, op, s, 3, stream));
+        CMRHS_STEP(fused2_impl<double>(op, T, D, Q, w.K3, w.K4, n, s, stream));
+    }
     op->bcg_its += 1;
     return COARSE_OK;
 }
