@@ -6,6 +6,7 @@
 #pragma once
 
 #include "common.cuh"
+#include "ptx_async.cuh"
 
 namespace cmrhs {
 
@@ -192,6 +193,29 @@ __device__ __forceinline__ void la_stage_rows(cplx<T> *dst, const cplx<T> *__res
         for (int r = row0; r < nrow; r += rpp) dst[r * su + col] = src[(r0 + r) * s + col];
 }
 
+// the same through cp.async (16-byte chunks; 8-byte for complex64 with odd s), no wait: the caller commits and waits.
+// Rows nrow .. rows_total of the buffer are zeroed with plain stores (ragged last tile).
+__device__ __forceinline__ void cp_async_16(void *dst_smem, const void *src) { asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory"); }
+__device__ __forceinline__ void cp_async_8(void *dst_smem, const void *src) { asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename T>
+__device__ __forceinline__ void la_stage_rows_async(cplx<T> *dst, const cplx<T> *__restrict__ src, int64_t r0, int nrow, int rows_total, int s, int su)
+{
+    const bool wide = sizeof(T) == 8 || (s & 1) == 0;                 // 16-byte chunks: one complex128 or two complex64
+    const int epc = (sizeof(T) == 4 && wide) ? 2 : 1;                  // elements per chunk
+    const int cpr = s / epc;                                           // chunks per row
+    const int rpp = kLaThreads / cpr, row0 = threadIdx.x / cpr, j = (threadIdx.x - row0 * cpr) * epc;
+    if (row0 < rpp) {
+        for (int r = row0; r < nrow; r += rpp) {
+            if (wide) cp_async_16(dst + r * su + j, src + (r0 + r) * s + j);
+            else cp_async_8(dst + r * su + j, src + (r0 + r) * s + j);
+        }
+    }
+    for (int e = threadIdx.x + nrow * su; e < rows_total * su; e += kLaThreads) dst[e] = {0, 0};
+}
+
 // acc[t][c] = sum_a sU[(rl + t RL)][a] * sK[a][c0 + c]
 template <typename T, int TR, int W>
 __device__ __forceinline__ void la_tile_product(cplx<T> (&acc)[TR][W], const cplx<T> *sU, const cplx<T> *sK, int rl, int RL, int c0, int s, int su)
@@ -222,7 +246,7 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
     const int su = s + LaPad<T>::v;
     const int ncg = (s + W - 1) / W, RL = kLaThreads / ncg, rows = RL * TR;
     cplx<T> *sK1 = reinterpret_cast<cplx<T> *>(smem_raw), *sK2 = sK1 + s * s;
-    cplx<T> *sD = sK2 + s * s, *sZ = sD + (size_t)rows * su;            // sD is reused for the T tile
+    cplx<T> *sD0 = sK2 + s * s, *sZ0 = sD0 + (size_t)2 * rows * su;     // two stages each; a stage's D buffer is reused for its T tile
     for (int e = threadIdx.x; e < s * s; e += kLaThreads) {
         sK1[e].re = (T)K1[e].re; sK1[e].im = (T)K1[e].im;
         sK2[e].re = (T)K2[e].re; sK2[e].im = (T)K2[e].im;
@@ -241,14 +265,23 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
         for (int b = 0; b < W; ++b) { accr[a][b] = 0.0; acci[a][b] = 0.0; }
 
     const int64_t ntiles = (n + rows - 1) / rows;
-    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    auto stage = [&](int b, int64_t t) {
         const int64_t r0 = t * rows;
         const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
-        __syncthreads();                                   // previous tile's Gram reads of sD are done (and sK is written)
-        la_stage_rows(sD, D, r0, nrow, s, su);
-        la_stage_rows(sZ, Z, r0, nrow, s, su);
-        for (int e = threadIdx.x + nrow * su; e < rows * su; e += kLaThreads) { sD[e] = {0, 0}; sZ[e] = {0, 0}; }   // ragged tail: zero rows
-        __syncthreads();
+        la_stage_rows_async(sD0 + (size_t)b * rows * su, D, r0, nrow, rows, s, su);
+        la_stage_rows_async(sZ0 + (size_t)b * rows * su, Z, r0, nrow, rows, s, su);
+    };
+    int buf = 0;
+    if ((int64_t)blockIdx.x < ntiles) stage(0, blockIdx.x);
+    cp_async_commit();
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x, buf ^= 1) {
+        const int64_t r0 = t * rows;
+        const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
+        if (t + gridDim.x < ntiles) stage(buf ^ 1, t + gridDim.x);     // next tile in flight while this one is worked on
+        cp_async_commit();
+        cp_async_wait<1>();
+        __syncthreads();                                   // tile t has landed for every thread (and sK is written)
+        cplx<T> *sD = sD0 + (size_t)buf * rows * su, *sZ = sZ0 + (size_t)buf * rows * su;
         cplx<T> tv[TR][W];
         if (rot_active) {
             cplx<T> acc[TR][W];
@@ -312,10 +345,12 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
 #pragma unroll
                 for (int b = 0; b < W; ++b) { accr[a][b] += (double)run[a][b].re; acci[a][b] += (double)run[a][b].im; }
         }
+        __syncthreads();                                   // this stage's buffers may be restaged by the next iteration
     }
     // reduce the row groups in a fixed order through shared memory (the tile buffers are free now)
+    cp_async_wait<0>();
     __syncthreads();
-    double *red = reinterpret_cast<double *>(sD);
+    double *red = reinterpret_cast<double *>(sD0);
     for (int g = 0; g < RG; ++g) {
         if (gram_active && rg == g) {
 #pragma unroll
@@ -343,21 +378,30 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
     const int su = s + LaPad<T>::v;
     const int ncg = (s + W - 1) / W, RL = kLaThreads / ncg, rows = RL * TR;
     cplx<T> *sK3 = reinterpret_cast<cplx<T> *>(smem_raw), *sK4 = sK3 + s * s;
-    cplx<T> *sT = sK4 + s * s, *sD = sT + (size_t)rows * su;
+    cplx<T> *sT0 = sK4 + s * s, *sD0 = sT0 + (size_t)2 * rows * su;     // two stages each
     for (int e = threadIdx.x; e < s * s; e += kLaThreads) {
         sK3[e].re = (T)K3[e].re; sK3[e].im = (T)K3[e].im;
         sK4[e].re = (T)K4[e].re; sK4[e].im = (T)K4[e].im;
     }
     const int cg = threadIdx.x % ncg, rl = threadIdx.x / ncg, c0 = cg * W;
     const int64_t ntiles = (n + rows - 1) / rows;
-    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    auto stage = [&](int b, int64_t t) {
         const int64_t r0 = t * rows;
         const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
+        la_stage_rows_async(sT0 + (size_t)b * rows * su, Tin, r0, nrow, rows, s, su);
+        la_stage_rows_async(sD0 + (size_t)b * rows * su, (const cplx<T> *)D, r0, nrow, rows, s, su);
+    };
+    int buf = 0;
+    if ((int64_t)blockIdx.x < ntiles) stage(0, blockIdx.x);
+    cp_async_commit();
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x, buf ^= 1) {
+        const int64_t r0 = t * rows;
+        const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
+        if (t + gridDim.x < ntiles) stage(buf ^ 1, t + gridDim.x);     // (rows of D this CTA writes below are its own: no other tile reads them)
+        cp_async_commit();
+        cp_async_wait<1>();
         __syncthreads();
-        la_stage_rows(sT, Tin, r0, nrow, s, su);
-        la_stage_rows(sD, D, r0, nrow, s, su);
-        for (int e = threadIdx.x + nrow * su; e < rows * su; e += kLaThreads) { sT[e] = {0, 0}; sD[e] = {0, 0}; }
-        __syncthreads();
+        const cplx<T> *sT = sT0 + (size_t)buf * rows * su, *sD = sD0 + (size_t)buf * rows * su;
         if (rl < RL) {
             cplx<T> q[TR][W], d[TR][W];
             la_tile_product<T, TR, W>(q, sT, sK3, rl, RL, c0, s, su);            // Q = T S^-1
@@ -378,7 +422,9 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
                         }
             }
         }
+        __syncthreads();                                   // this stage's buffers may be restaged by the next iteration
     }
+    cp_async_wait<0>();
 }
 
 // out = a*U + b*W elementwise (used for R = B - H X and copies)

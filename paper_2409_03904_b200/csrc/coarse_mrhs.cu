@@ -370,11 +370,9 @@ template <typename T>
 static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble *G, int64_t n, int s, cudaStream_t stream)
 {
     int TT = s > 32 ? 4 : (s >= 8 ? 2 : 1);
-    if (const char *e = getenv("CMRHS_GRAM_TT")) { const int v = atoi(e); if (v >= 1 && v <= 4 && (s + v - 1) / v <= 16) TT = v; }
     const int nt = (s + TT - 1) / TT;
     const int RG = kLaThreads / (nt * nt);
     size_t tile_bytes = 40960;
-    if (const char *e = getenv("CMRHS_GRAM_SMEM")) { const int v = atoi(e); if (v >= 2048 && v <= 65536) tile_bytes = (size_t)v; }
     int rows = (int)(tile_bytes / (2 * (size_t)s * sizeof(cplx<T>)));
     rows = rows / RG * RG;
     if (rows < RG) rows = RG;
@@ -451,21 +449,18 @@ static FusedPlan fused_plan(const coarse_op *op, int64_t n, int s)
 {
     FusedPlan p;
     p.W = s >= 8 ? 2 : 1;
-    if (const char *e = getenv("CMRHS_LA_W")) { const int v = atoi(e); if (v == 1 || v == 2 || v == 4) p.W = v; }
     if ((s + p.W - 1) / p.W > 16) p.W = 4;
     const int ncg = (s + p.W - 1) / p.W, RL = kLaThreads / ncg, su = s + LaPad<T>::v;
-    int tr0 = 2;
-    if (const char *e = getenv("CMRHS_LA_TR")) { const int v = atoi(e); if (v == 1 || v == 2 || v == 4) tr0 = v; }
+    int tr0 = 4;
     for (p.TR = tr0; ; p.TR /= 2) {
         p.rows = RL * p.TR;
-        size_t tiles = (size_t)2 * p.rows * su * sizeof(cplx<T>);
+        size_t tiles = (size_t)4 * p.rows * su * sizeof(cplx<T>);      // two operands x two stages
         const size_t red = (size_t)s * s * sizeof(zdouble);
         if (tiles < red) tiles = red;
         p.smem = (size_t)2 * s * s * sizeof(cplx<T>) + tiles;
         if (p.smem <= 100 * 1024 || p.TR == 1) break;      // two CTAs per SM when possible
     }
     int per_sm = p.smem <= 27 * 1024 ? 8 : (p.smem <= 56 * 1024 ? 4 : (p.smem <= 113 * 1024 ? 2 : 1));
-    if (const char *e = getenv("CMRHS_LA_PERSM")) { const int v = atoi(e); if (v >= 1 && v <= 8) per_sm = v; }
     const int64_t ntiles = ceil_div(n, p.rows);
     int64_t g = (int64_t)op->num_sms * per_sm;
     if (g > op->gram_blocks) g = op->gram_blocks;

@@ -23,7 +23,6 @@
 #pragma once
 
 #include <cuda_fp16.h>
-#include <stdlib.h>
 
 #include "stencil_tc.cuh"
 
