@@ -7,17 +7,20 @@
 //   a  = sA a_true            (sA: one power of two per operator, max |a| -> [2^14, 2^15))
 //   a  = hi + 2^-11 lo        hi = fp16(a), lo = fp16(2^11 (a - hi))      22-23 significant bits in the same 4 bytes
 //   x  = sX_r x_true          (sX_r: one power of two per right-hand side column, from a max-abs pre-pass over X)
-//   Y  = (D + 2^-11 (C' + C'')) / (sA sX_r),   D = A_hi X_hi,  C' = A_hi X_lo,  C'' = A_lo X_hi   (FP32 in TMEM)
+//   Y  = (D + 2^-11 C) / (sA sX_r),   D = A_hi X_hi,  C = A_hi X_lo + A_lo X_hi   (FP32 accumulators in TMEM)
 // * The operator is stored ALREADY SPLIT in HBM (coarse_op_create, same 8 bytes per complex as complex64): a stencil
 //   matrix is one 8 KB tile [hi 4 KB | lo 4 KB], each half the MN-major SWIZZLE_128B shared-memory image of the
 //   64 x 32 (M x K) operand [Re A ; Im A] -- one 1-D bulk copy puts it in place, the tensor core reads it from there.
 //   Nothing converts A on chip: no converter warps, no TMEM operand panels (stencil_tc.cuh needs twelve warps for it).
 // * M = 128 = two sites = two swizzle atoms; the descriptor's leading-dimension byte offset is the distance between
 //   the two tiles.  A step whose X tile only one site uses points the other atom at a block of zeros.
-// * K = 16 per instruction: 2 k-steps x (A_hi . [X_hi | X_lo] -> D | C',  A_lo . X_hi -> C'') = 4 MMAs per step
+// * K = 16 per instruction: 2 k-steps x (A_hi . [X_hi | X_lo] -> D | C,  then A_lo . X_hi -> C) = 4 MMAs per step
 //   (stencil_tc.cuh: 8-12).
-// * X: fp32 tile by 1-D bulk copy -> eight warps scale, split and write the fp16 operand [hi | lo] (MN-major,
-//   SWIZZLE_128B) -> MMA.  The epilogue undoes the scales and combines Re/Im as in stencil_tc.cuh.
+// * X: every site's tile is scaled, split and written ONCE per apply as a ready-made operand tile [hi | lo] (MN-major,
+//   SWIZZLE_128B) by two pre-pass kernels (colmax_kernel, xsplit_kernel); the stencil kernel bulk-copies it like A.
+//   The epilogue undoes the scales and combines Re/Im as in stencil_tc.cuh.
+// * The time of one pipeline is the serial latency of its hand-shakes, not any unit's throughput: up to three CTAs
+//   (independent pipelines, 128 TMEM columns each) run per SM.
 // Range: elements smaller than 2^-29 of the operator's (a column's) largest element lose relative precision
 // (absolute error <= 2^-25 of the largest): norm-wise errors stay at the 1e-7 level.
 #pragma once
@@ -44,7 +47,7 @@ struct HParams {
     int32_t LO;           // operand column of the lo half: 2 s if 4 s <= 64 (hi | lo share one 64-column atom), else a multiple of 64
     int32_t wideN;        // LO + 2 s: N of the A_hi MMA ([X_hi | X_lo] -> D | C); the A_lo . X_hi MMA adds into C (TMEM column LO)
     int32_t acc_stride, nacc;
-    int32_t tmem_cols;    // 512 (one CTA per SM) or 256 (two)
+    int32_t tmem_cols;    // 512 (one CTA per SM), 256 (two) or 128 (three)
     int32_t sa, sxo;      // ring depths: A tiles, X operand tiles
     int32_t xo_bytes;     // fp16 X operand tile: atoms * 4096
     uint32_t idesc_wide, idesc_lo;
@@ -173,7 +176,7 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
     const uint32_t tmem = *tmem_slot;
 
     if (warp < 4) {
-        // ================= epilogue: Y = combine((D + 2^-11 (C' + C'')) / (sA sX)) -> global =================
+        // ================= epilogue: Y = combine((D + 2^-11 C) / (sA sX)) -> global =================
         const int q = warp - kHXconvWarps;                 // = warp % 4: the TMEM lane quarter this warp may access
         const int slot = q >> 1, part = q & 1;
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
@@ -466,7 +469,6 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     P.acc_stride = P.wideN;
     // independent pipelines (CTAs) per SM: as many as tensor memory (power-of-two allocations) and shared memory allow
     int cps = P.acc_stride <= 128 ? 3 : (P.acc_stride <= 256 ? 2 : 1);
-    if (const char *e = getenv("CMRHS_H16_CPS")) { const int v = atoi(e); if (v >= 1 && v < cps) cps = v; }
     P.tmem_cols = cps == 3 ? 128 : (cps == 2 ? 256 : 512);
     P.nacc = P.tmem_cols / P.acc_stride;
     if (P.nacc > kHMaxAcc) P.nacc = kHMaxAcc;
