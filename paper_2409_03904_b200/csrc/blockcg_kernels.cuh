@@ -217,19 +217,22 @@ __device__ __forceinline__ void la_stage_rows_async(cplx<T> *dst, const cplx<T> 
 }
 
 // acc[t][c] = sum_a sU[(rl + t RL)][a] * sK[a][c0 + c]
-template <typename T, int TR, int W>
-__device__ __forceinline__ void la_tile_product(cplx<T> (&acc)[TR][W], const cplx<T> *sU, const cplx<T> *sK, int rl, int RL, int c0, int s, int su)
+// S > 0: s is the compile-time constant S (a multiple of W): the a-loop unrolls and the column guard disappears
+template <typename T, int TR, int W, int S = 0>
+__device__ __forceinline__ void la_tile_product(cplx<T> (&acc)[TR][W], const cplx<T> *sU, const cplx<T> *sK, int rl, int RL, int c0, int s_rt, int su_rt)
 {
+    const int s = S ? S : s_rt, su = S ? S + LaPad<T>::v : su_rt;
 #pragma unroll
     for (int t = 0; t < TR; ++t)
 #pragma unroll
         for (int c = 0; c < W; ++c) { acc[t][c].re = 0; acc[t][c].im = 0; }
+#pragma unroll(S ? 16 : 1)
     for (int a = 0; a < s; ++a) {
         cplx<T> u[TR], k[W];
 #pragma unroll
         for (int t = 0; t < TR; ++t) u[t] = sU[(rl + t * RL) * su + a];
 #pragma unroll
-        for (int c = 0; c < W; ++c) k[c] = (c0 + c < s) ? sK[a * s + c0 + c] : cplx<T>{0, 0};
+        for (int c = 0; c < W; ++c) k[c] = (S || c0 + c < s) ? sK[a * s + c0 + c] : cplx<T>{0, 0};
 #pragma unroll
         for (int t = 0; t < TR; ++t)
 #pragma unroll
@@ -237,12 +240,13 @@ __device__ __forceinline__ void la_tile_product(cplx<T> (&acc)[TR][W], const cpl
     }
 }
 
-template <typename T, int TR, int W>
+template <typename T, int TR, int W, int S = 0>
 __global__ void __launch_bounds__(kLaThreads)
 bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Q, cplx<T> *X, cplx<T> *Tout,
-                  const zdouble *__restrict__ K1, const zdouble *__restrict__ K2, int64_t n, int s, zdouble *__restrict__ partial)
+                  const zdouble *__restrict__ K1, const zdouble *__restrict__ K2, int64_t n, int s_rt, zdouble *__restrict__ partial)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int s = S ? S : s_rt;
     const int su = s + LaPad<T>::v;
     const int ncg = (s + W - 1) / W, RL = kLaThreads / ncg, rows = RL * TR;
     cplx<T> *sK1 = reinterpret_cast<cplx<T> *>(smem_raw), *sK2 = sK1 + s * s;
@@ -285,27 +289,27 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
         cplx<T> tv[TR][W];
         if (rot_active) {
             cplx<T> acc[TR][W];
-            la_tile_product<T, TR, W>(acc, sD, sK1, rl, RL, c0, s, su);          // D K1
+            la_tile_product<T, TR, W, S>(acc, sD, sK1, rl, RL, c0, s, su);          // D K1
 #pragma unroll
             for (int tt = 0; tt < TR; ++tt) {
                 const int row = rl + tt * RL;
                 if (row < nrow)
 #pragma unroll
                     for (int c = 0; c < W; ++c)
-                        if (c0 + c < s) {
+                        if (S || c0 + c < s) {
                             const int64_t e = (r0 + row) * s + c0 + c;
                             cplx<T> x = X[e];
                             x.re += acc[tt][c].re; x.im += acc[tt][c].im;
                             X[e] = x;
                         }
             }
-            la_tile_product<T, TR, W>(tv, sZ, sK2, rl, RL, c0, s, su);           // Z K2
+            la_tile_product<T, TR, W, S>(tv, sZ, sK2, rl, RL, c0, s, su);           // Z K2
 #pragma unroll
             for (int tt = 0; tt < TR; ++tt) {
                 const int row = rl + tt * RL;
 #pragma unroll
                 for (int c = 0; c < W; ++c) {
-                    if (row < nrow && c0 + c < s) {
+                    if (row < nrow && (S || c0 + c < s)) {
                         const int64_t e = (r0 + row) * s + c0 + c;
                         const cplx<T> q = Q[e];
                         tv[tt][c].re += q.re; tv[tt][c].im += q.im;
@@ -320,7 +324,7 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
             for (int tt = 0; tt < TR; ++tt)
 #pragma unroll
                 for (int c = 0; c < W; ++c)
-                    if (c0 + c < s) sD[(rl + tt * RL) * su + c0 + c] = tv[tt][c];
+                    if (S || c0 + c < s) sD[(rl + tt * RL) * su + c0 + c] = tv[tt][c];
         }
         __syncthreads();
         if (gram_active) {
@@ -332,9 +336,9 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
             for (int k = rg; k < nrow; k += RG) {
                 cplx<T> u[W], w[W];
 #pragma unroll
-                for (int a = 0; a < W; ++a) u[a] = (ga0 + a < s) ? sD[k * su + ga0 + a] : cplx<T>{0, 0};
+                for (int a = 0; a < W; ++a) u[a] = (S || ga0 + a < s) ? sD[k * su + ga0 + a] : cplx<T>{0, 0};
 #pragma unroll
-                for (int b = 0; b < W; ++b) w[b] = (gb0 + b < s) ? sD[k * su + gb0 + b] : cplx<T>{0, 0};
+                for (int b = 0; b < W; ++b) w[b] = (S || gb0 + b < s) ? sD[k * su + gb0 + b] : cplx<T>{0, 0};
 #pragma unroll
                 for (int a = 0; a < W; ++a)
 #pragma unroll
@@ -369,12 +373,13 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
     for (int e = threadIdx.x; e < s * s; e += kLaThreads) { out[e].re = red[2 * e]; out[e].im = red[2 * e + 1]; }
 }
 
-template <typename T, int TR, int W>
+template <typename T, int TR, int W, int S = 0>
 __global__ void __launch_bounds__(kLaThreads)
 bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, const zdouble *__restrict__ K3, const zdouble *__restrict__ K4,
-                  int64_t n, int s)
+                  int64_t n, int s_rt)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int s = S ? S : s_rt;
     const int su = s + LaPad<T>::v;
     const int ncg = (s + W - 1) / W, RL = kLaThreads / ncg, rows = RL * TR;
     cplx<T> *sK3 = reinterpret_cast<cplx<T> *>(smem_raw), *sK4 = sK3 + s * s;
@@ -404,15 +409,15 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
         const cplx<T> *sT = sT0 + (size_t)buf * rows * su, *sD = sD0 + (size_t)buf * rows * su;
         if (rl < RL) {
             cplx<T> q[TR][W], d[TR][W];
-            la_tile_product<T, TR, W>(q, sT, sK3, rl, RL, c0, s, su);            // Q = T S^-1
-            la_tile_product<T, TR, W>(d, sD, sK4, rl, RL, c0, s, su);            // D S^H
+            la_tile_product<T, TR, W, S>(q, sT, sK3, rl, RL, c0, s, su);            // Q = T S^-1
+            la_tile_product<T, TR, W, S>(d, sD, sK4, rl, RL, c0, s, su);            // D S^H
 #pragma unroll
             for (int tt = 0; tt < TR; ++tt) {
                 const int row = rl + tt * RL;
                 if (row < nrow)
 #pragma unroll
                     for (int c = 0; c < W; ++c)
-                        if (c0 + c < s) {
+                        if (S || c0 + c < s) {
                             const int64_t e = (r0 + row) * s + c0 + c;
                             Qout[e] = q[tt][c];
                             cplx<T> v;

@@ -468,29 +468,34 @@ static FusedPlan fused_plan(const coarse_op *op, int64_t n, int s)
     return p;
 }
 
-template <typename T, int TR, int W>
+template <typename T, int TR, int W, int S = 0>
 static int fused1_launch(const coarse_op *op, const FusedPlan &p, const void *D, const void *Z, const void *Q, void *X, void *Tout,
                          const zdouble *K1, const zdouble *K2, int64_t n, int s, cudaStream_t stream)
 {
-    auto kern = bcg_fused1_kernel<T, TR, W>;
+    auto kern = bcg_fused1_kernel<T, TR, W, S>;
     CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
     kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)D, (const cplx<T> *)Z, (const cplx<T> *)Q, (cplx<T> *)X, (cplx<T> *)Tout, K1, K2,
                                                   n, s, op->gram_partial);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
-template <typename T, int TR, int W>
+template <typename T, int TR, int W, int S = 0>
 static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Tin, void *D, void *Qout, const zdouble *K3, const zdouble *K4,
                          int64_t n, int s, cudaStream_t stream)
 {
-    auto kern = bcg_fused2_kernel<T, TR, W>;
+    auto kern = bcg_fused2_kernel<T, TR, W, S>;
     CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
     kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)Tin, (cplx<T> *)D, (cplx<T> *)Qout, K3, K4, n, s);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
 
+// the common block widths run kernels with s as a compile-time constant (plan TR 4, W 2)
 #define CMRHS_FUSED_SWITCH(CALL)                                         \
+    if (p.TR == 4 && p.W == 2) {                                         \
+        if (s == 8) return CALL(4, 2, 8); if (s == 16) return CALL(4, 2, 16); if (s == 32) return CALL(4, 2, 32); \
+        if (s == 64) return CALL(4, 2, 64);                              \
+    }                                                                    \
     if (p.TR == 4) {                                                     \
         if (p.W == 4) return CALL(4, 4); if (p.W == 2) return CALL(4, 2); return CALL(4, 1); \
     }                                                                    \
@@ -506,7 +511,7 @@ static int fused1_impl(const coarse_op *op, const void *D, const void *Z, const 
 {
     const FusedPlan p = fused_plan<T>(op, n, s);
     auto run = [&]() -> int {
-#define CMRHS_F1(TRV, WV) fused1_launch<T, TRV, WV>(op, p, D, Z, Q, X, Tout, K1, K2, n, s, stream)
+#define CMRHS_F1(TRV, WV, ...) fused1_launch<T, TRV, WV, ##__VA_ARGS__>(op, p, D, Z, Q, X, Tout, K1, K2, n, s, stream)
         CMRHS_FUSED_SWITCH(CMRHS_F1)
 #undef CMRHS_F1
     };
@@ -522,7 +527,7 @@ static int fused2_impl(const coarse_op *op, const void *Tin, void *D, void *Qout
                        cudaStream_t stream)
 {
     const FusedPlan p = fused_plan<T>(op, n, s);
-#define CMRHS_F2(TRV, WV) fused2_launch<T, TRV, WV>(op, p, Tin, D, Qout, K3, K4, n, s, stream)
+#define CMRHS_F2(TRV, WV, ...) fused2_launch<T, TRV, WV, ##__VA_ARGS__>(op, p, Tin, D, Qout, K3, K4, n, s, stream)
     CMRHS_FUSED_SWITCH(CMRHS_F2)
 #undef CMRHS_F2
 }

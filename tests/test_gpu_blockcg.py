@@ -202,3 +202,31 @@ def test_begin_step_end_equals_solve(cfg1):
     assert rel_err_cols(to_np(Xd), ref["X"]) <= 1e-12
     assert np.allclose(out["rel_res_recursive"], ref["history"][-1], rtol=1e-6)
     assert max(out["rel_res_true"]) <= 1e-10
+
+
+@pytest.mark.parametrize("dims,nb,s,dtype,tol", [
+    ((4, 4, 4, 4), 32, 16, "c64", 1e-6),
+    ((3, 3, 3, 5), 24, 8, "c128", 1e-10),
+    ((3, 3, 2, 4), 13, 5, "c128", 1e-10),       # odd s: 8-byte cp.async chunks do not apply to complex128; ragged column groups
+    ((3, 3, 2, 4), 16, 7, "c64", 1e-6),         # odd s in complex64: 8-byte chunks, ragged column groups
+    ((3, 3, 3, 3), 32, 64, "c64", 1e-6),        # widest block
+    ((3, 3, 3, 3), 8, 33, "c128", 1e-10),       # s > 32 in complex128
+])
+def test_fused_passes_equal_the_unfused_kernel_sequence(dims, nb, s, dtype, tol):
+    # the two fused passes of an iteration (bcg_fused1/2_kernel) against the six-kernel sequence (COARSE_FLAG_UNFUSED_LINALG)
+    # and against the oracle: same iteration count, same residual history, same solution
+    A, c, _, B = host_case(dims, nb, s, 91, 1.03)
+    ref = oracle.block_cg(dims, A, B, tol=tol, maxiter=100)
+    outs = []
+    for flags in (0, cm.binding.FLAG_UNFUSED_LINALG):
+        op = cm.CoarseOperator(dims, to_dev(A, dtype), s, flags=flags)
+        out = op.block_cg(to_dev(B, dtype), to_dev(np.zeros_like(B), dtype), tol=tol, maxiter=100)
+        op.close()
+        out["X"] = to_np(out["X"])
+        _check_solve(out, ref, tol, dtype)
+        outs.append(out)
+    assert outs[0]["iterations"] == outs[1]["iterations"]
+    assert rel_err_cols(outs[0]["X"], outs[1]["X"]) <= (1e-12 if dtype == "c128" else 2e-6)
+    k = outs[0]["iterations"]
+    h0, h1 = np.array(outs[0]["history"][:k + 1]), np.array(outs[1]["history"][:k + 1])
+    assert np.allclose(h0, h1, rtol=1e-9 if dtype == "c128" else 2e-2)
