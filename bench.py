@@ -225,11 +225,12 @@ def whole_job_value(world: int, steps: int, flops_per_step_per_rank: float, ms_m
 
 
 # ---- our arm ---------------------------------------------------------------------------------------------------
-def load_traffic(kernel_name):
-    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture, or None."""
+def load_traffic(key):
+    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture of this workload
+    (key = workload|kernel@nrhs), or None when no capture of that combination is committed."""
     path = os.path.join(ROOT, "profiles", "apply_traffic.json")
     if os.path.exists(path):
-        return json.load(open(path)).get(kernel_name)
+        return json.load(open(path)).get(key)
     return None
 
 
@@ -319,7 +320,7 @@ def run_ours(args, cfg):
         roofline = dict(bound=rf["bound"], achieved=a_tflops, peak=rf["pipe_tflops"], unit="TFLOP/s", frac=a_tflops / rf["pipe_tflops"],
                         peak_note=("measured sustained bf16 GEMM [x nominal TF32/bf16 (1.1/2.25) for the TF32 kernel] / 3 products per algorithmic product"
                                    if rf["bound"] == "tensor" else "148 SMs x FMA lanes x 2 x max SM clock"))
-    roofline.update(traffic=load_traffic(f"{kernel_name}@nrhs{s}"), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
+    roofline.update(traffic=load_traffic(f"{cfg['name']}|{kernel_name}@nrhs{s}"), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
                     share_of_step=a_ms * len(apply_ms) / ms if apply_ms else None, peak_source=peaks["source"],
                     intensity_flop_per_byte=rf["intensity"], hbm_gbs_achieved=a_gbs,
                     frac_of_min_peak_IxBW=a_tflops / rf["roof_tflops"])

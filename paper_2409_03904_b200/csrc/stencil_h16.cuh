@@ -51,6 +51,10 @@ struct HParams {
     int32_t sa, sxo;      // ring depths: A tiles, X operand tiles
     int32_t xo_bytes;     // fp16 X operand tile: atoms * 4096
     uint32_t idesc_wide, idesc_lo;
+    int32_t tr;           // 1: transposed form (nrhs > 32): the X tile is the M-side operand (M = 2 nrhs real columns, padded to
+                          //    128), the stencil matrix the N side ([A_hi | A_lo], N = 128); one accumulator (D 64 | C 64 columns)
+                          //    PER SITE, so a step only one site uses costs half a step -- no M rows are spent on zeros
+    uint32_t idesc_t_wide, idesc_t_lo;
     float inv_sA;         // 1 / sA
     const uint32_t *amax; // [s] bit patterns of max |Re|, |Im| per column of X (pre-pass)
 };
@@ -122,7 +126,7 @@ __device__ __forceinline__ int64_t h_x_site(const HParams &P, const TcGroup &g, 
     return h_site(P, tc_wrap(g.x0 + j - 1, P.L[0]), tc_wrap(g.y + dy, P.L[1]), tc_wrap(g.z + dz, P.L[2]), tc_wrap(g.t + dt, P.L[3]));
 }
 
-template <int kCtasPerSm>
+template <int kCtasPerSm, bool kTr>
 __global__ void __launch_bounds__(kHThreads, kCtasPerSm)
 stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__restrict__ Xh, float2 *__restrict__ Y, const HParams P)
 {
@@ -188,6 +192,34 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
             TW(0, mbar_wait(&acc_full[rc.stage], rc.phase));
             tc_fence_after_sync();
             TW_BEGIN();
+            if constexpr (kTr) {
+                // lanes = real columns n = (r, re/im) of Y^T, columns = (part, i): Y_re = P[(r,0)] - Q[(r,1)], Y_im = P[(r,1)] + Q[(r,0)]
+                const int n = 32 * q + lane, r = n >> 1, c = n & 1;
+                const bool live = n < P.N2;
+                const float sc = live ? inv[n] * 1.0f : 0.0f;
+                float *Yf = reinterpret_cast<float *>(Y);
+                for (int i = 0; i < grp.G; ++i) {
+                    const uint32_t ds = lane_base + (uint32_t)(rc.stage * P.acc_stride) + 128u * (uint32_t)i;
+                    const int64_t site = h_site(P, grp.x0 + i, grp.y, grp.z, grp.t);
+#pragma unroll
+                    for (int half = 0; half < 2; ++half) {
+                        uint32_t dp[16], cp[16], dq[16], cq[16];
+                        tmem_ld_x16(ds + 16u * half, dp);
+                        tmem_ld_x16(ds + 64u + 16u * half, cp);
+                        tmem_ld_x16(ds + 32u + 16u * half, dq);
+                        tmem_ld_x16(ds + 96u + 16u * half, cq);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int k = 0; k < 16; ++k) {
+                            const float pv = (__uint_as_float(dp[k]) + __uint_as_float(cp[k]) * (1.0f / 2048.0f)) * sc;
+                            const float qv = (__uint_as_float(dq[k]) + __uint_as_float(cq[k]) * (1.0f / 2048.0f)) * sc;
+                            const float qo = __shfl_xor_sync(0xffffffffu, qv, 1);
+                            const float val = c == 0 ? pv - qo : pv + qo;
+                            if (live) Yf[((site * NB + 16 * half + k) * (int64_t)P.s + r) * 2 + c] = val;
+                        }
+                    }
+                }
+            } else
             if (slot < grp.G) {
                 const uint32_t d = lane_base + (uint32_t)(rc.stage * P.acc_stride);
                 const uint32_t c2 = d + (uint32_t)P.LO;
@@ -244,7 +276,7 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
             for (int step = 0; step < grp.nsteps; ++step) {
                 const uint32_t e = grp.tab[step];
                 const int off3 = (int)(e & 31u);
-                if (((e >> 8) & 3u) == 3u && ra.stage == P.sa - 1) {
+                if (!kTr && ((e >> 8) & 3u) == 3u && ra.stage == P.sa - 1) {
                     TW(0, mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u));
                     if (elect_one_sync()) mbar_arrive(&a_full[ra.stage]);
                     __syncwarp();
@@ -291,6 +323,53 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
             TW(0, mbar_wait(&acc_empty[rc.stage], rc.phase ^ 1u));
             tc_fence_after_sync();
             const uint32_t d = tmem + (uint32_t)(rc.stage * P.acc_stride), c2 = d + (uint32_t)P.LO;
+            if constexpr (kTr) {
+                // transposed form: D_site[(r,c)][(part,i)] += X^T . [A_hi | A_lo]  -- one accumulator (128 columns) per site
+                uint32_t seen = 0u;
+                const uint32_t lo_atoms = (uint32_t)(P.LO >> 6) * 4096u;
+                for (int step = 0; step < grp.nsteps; ++step) {
+                    const uint32_t um = (grp.tab[step] >> 8) & 3u;
+                    TcRing r1 = ra;
+                    r1.advance(P.sa);
+                    TW(1, mbar_wait(&a_full[ra.stage], ra.phase));
+                    if (um == 3u) TW(1, mbar_wait(&a_full[r1.stage], r1.phase));
+                    TW(2, mbar_wait(&xo_full[ro.stage], ro.phase));
+                    tc_fence_after_sync();
+                    TW_BEGIN();
+                    if (elect_one_sync()) {
+                        const uint32_t xo = smem_u32(ringXo + (size_t)ro.stage * P.xo_bytes);
+                        int nth = 0;
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            if (!((um >> i) & 1u)) continue;
+                            const uint32_t tile = ring0 + (uint32_t)(nth == 0 ? ra.stage : r1.stage) * kHTile;
+                            const uint32_t ds = d + 128u * (uint32_t)i;
+#pragma unroll
+                            for (int ks = 0; ks < 2; ++ks) {
+                                const uint64_t x_hi = h_desc(xo + (uint32_t)ks * 2048u, 4096u);
+                                const uint64_t x_lo = h_desc(xo + lo_atoms + (uint32_t)ks * 2048u, 4096u);
+                                const uint64_t a_w = h_desc(tile + (uint32_t)ks * 2048u, 4096u);       // [A_hi | A_lo]: adjacent 4 KB atoms
+                                const uint32_t acc = (((seen >> i) & 1u) | (uint32_t)ks) != 0u ? 1u : 0u;
+                                umma_f16_ss(ds, x_hi, a_w, P.idesc_t_wide, acc);            // X_hi^T . [A_hi | A_lo] -> D | C
+                                umma_f16_ss(ds + 64u, x_lo, a_w, P.idesc_t_lo, 1u);         // X_lo^T . A_hi -> C
+                            }
+                            ++nth;
+                        }
+                        umma_commit(&xo_empty[ro.stage]);
+                        umma_commit(&a_empty[ra.stage]);
+                        if (um == 3u) umma_commit(&a_empty[r1.stage]);
+                        if (step == grp.nsteps - 1) umma_commit(&acc_full[rc.stage]);
+                    }
+                    __syncwarp();
+                    TW_END(3);
+                    seen |= um;
+                    ra.advance(P.sa);
+                    if (um == 3u) ra.advance(P.sa);
+                    ro.advance(P.sxo);
+                }
+                rc.advance(P.nacc);
+                continue;
+            }
             for (int step = 0; step < grp.nsteps; ++step) {
                 const uint32_t um = (grp.tab[step] >> 8) & 3u;
                 if (um == 3u && ra.stage == P.sa - 1) {            // the pair would wrap: pass over the last stage
@@ -467,6 +546,8 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     else P.LO = 64 * ((2 * s + 63) / 64);
     P.wideN = P.LO + 2 * s;
     P.acc_stride = P.wideN;
+    P.tr = s > 48 ? 1 : 0;             // measured on B200: equal to the paired form at nrhs 48 and 64, 14 % faster at 56
+    if (P.tr) P.acc_stride = 256;            // two sites x (D 64 | C 64)
     // independent pipelines (CTAs) per SM: as many as tensor memory (power-of-two allocations) and shared memory allow
     int cps = P.acc_stride <= 128 ? 3 : (P.acc_stride <= 256 ? 2 : 1);
     P.tmem_cols = cps == 3 ? 128 : (cps == 2 ? 256 : 512);
@@ -484,6 +565,8 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     if (P.sa < 4 || P.nacc < 1) { set_error("tensor path: shared/tensor memory plan does not fit (nrhs %d)", s); return COARSE_UNSUPPORTED; }
     P.idesc_wide = umma_idesc_f16_mn(128, P.wideN);
     P.idesc_lo = umma_idesc_f16_mn(128, P.N2);
+    P.idesc_t_wide = umma_idesc_f16_mn(128, 128);
+    P.idesc_t_lo = umma_idesc_f16_mn(128, 64);
     P.inv_sA = inv_sA;
     P.amax = amax_dev;
     const size_t smem = (size_t)fixed + (size_t)P.sa * kHTile + (size_t)P.sxo * P.xo_bytes;
@@ -501,17 +584,19 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
 
     static bool attr_set = false;
     if (!attr_set) {
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
+        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
         attr_set = true;
     }
     const int slots = cps * num_sms;
     const int grid = P.ngroups < slots ? P.ngroups : slots;
     float2 *Yp = static_cast<float2 *>(Y);
-    if (cps == 3) stencil_h16_kernel<3><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
-    else if (cps == 2) stencil_h16_kernel<2><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
-    else stencil_h16_kernel<1><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
+    if (P.tr) stencil_h16_kernel<2, true><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
+    else if (cps == 3) stencil_h16_kernel<3, false><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
+    else if (cps == 2) stencil_h16_kernel<2, false><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
+    else stencil_h16_kernel<1, false><<<grid, kHThreads, smem, stream>>>(Ah, Xh, Yp, P);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
