@@ -225,7 +225,7 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
                 const uint32_t c2 = d + (uint32_t)P.LO;
                 const int64_t site = h_site(P, grp.x0 + slot, grp.y, grp.z, grp.t);
                 float2 *yrow = Y + (site * NB + lane) * (int64_t)P.s;
-                for (int c = 0; c < P.N2 / 16; ++c, ++chunk_no) {
+                for (int c = 0; c < (P.N2 + 15) / 16; ++c, ++chunk_no) {
                     uint32_t a[16], b[16];
                     float v[16];
                     tmem_ld_x16(d + 16u * c, a);
@@ -251,9 +251,11 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
                         r0 = make_float4(o0.x - v[9], o0.y + v[8], o0.z - v[11], o0.w + v[10]);
                         r1 = make_float4(o1.x - v[13], o1.y + v[12], o1.z - v[15], o1.w + v[14]);
                     }
-                    float4 *dstp = reinterpret_cast<float4 *>(yrow + 8 * c + 4 * part);
-                    dstp[0] = r0;
-                    dstp[1] = r1;
+                    if (8 * c + 4 * part < P.s) {            // (false only for the upper half of the single chunk of nrhs 4)
+                        float4 *dstp = reinterpret_cast<float4 *>(yrow + 8 * c + 4 * part);
+                        dstp[0] = r0;
+                        dstp[1] = r1;
+                    }
                 }
             }
             tc_fence_before_sync();
@@ -427,8 +429,9 @@ stencil_h16_kernel(const unsigned char *__restrict__ Ah, const unsigned char *__
 }
 
 // ---- host side ------------------------------------------------------------------------------------------------
-// shapes the FP16-split kernel covers: complex64, nbasis 32, nrhs a multiple of 8
-inline bool h16_supported(int nb, int s) { return nb == 32 && s >= 8 && s <= 64 && s % 8 == 0; }
+// shapes the FP16-split kernel covers: complex64, nbasis 32, nrhs a multiple of 8, or 4 (the A_lo MMA then runs at the
+// minimum N = 16 and also writes 8 unused accumulator columns)
+inline bool h16_supported(int nb, int s) { return nb == 32 && ((s >= 8 && s <= 64 && s % 8 == 0) || s == 4); }
 
 // max |v| over a float array, as the bit pattern of a non-negative float (order-independent: atomicMax on the bits)
 __global__ void absmax_kernel(const float *__restrict__ v, int64_t n, uint32_t *__restrict__ out)
@@ -546,6 +549,7 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     else P.LO = 64 * ((2 * s + 63) / 64);
     P.wideN = P.LO + 2 * s;
     P.acc_stride = P.wideN;
+    if (P.N2 < 16) P.acc_stride = P.LO + 16;  // nrhs 4: the A_lo MMA has N = 16
     P.tr = s > 48 ? 1 : 0;             // measured on B200: equal to the paired form at nrhs 48 and 64, 14 % faster at 56
     if (P.tr) P.acc_stride = 256;            // two sites x (D 64 | C 64)
     // independent pipelines (CTAs) per SM: as many as tensor memory (power-of-two allocations) and shared memory allow
@@ -564,7 +568,7 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     if (P.sa > kHMaxStagesA) P.sa = kHMaxStagesA;
     if (P.sa < 4 || P.nacc < 1) { set_error("tensor path: shared/tensor memory plan does not fit (nrhs %d)", s); return COARSE_UNSUPPORTED; }
     P.idesc_wide = umma_idesc_f16_mn(128, P.wideN);
-    P.idesc_lo = umma_idesc_f16_mn(128, P.N2);
+    P.idesc_lo = umma_idesc_f16_mn(128, P.N2 < 16 ? 16 : P.N2);
     P.idesc_t_wide = umma_idesc_f16_mn(128, 128);
     P.idesc_t_lo = umma_idesc_f16_mn(128, 64);
     P.inv_sA = inv_sA;
