@@ -355,6 +355,22 @@ def run_ours(args, cfg):
     bcg = dict(seconds=sol["seconds"], iterations=sol["iterations"], status=sol["status"], tol=cfg["tol"],
                max_true_rel_res=max(sol["rel_res_true"]))
 
+    # ---- Chebyshev polynomial coarse solve (the paper's coarse solve is order 120) ----
+    cheb = None
+    if args.cheby_order > 0:
+        lo_c, hi_c = c - 12.0, c + 12.0                 # safely around the synthetic operator's spectrum (c +- 7)
+        op.cheby_apply(B, lo_c, hi_c, 3, X=Xs)          # warm-up
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        op.cheby_apply(B, lo_c, hi_c, args.cheby_order, X=Xs)
+        ev[1].record()
+        torch.cuda.synchronize()
+        t_c = ev[0].elapsed_time(ev[1]) * 1e-3
+        napp = args.cheby_order - 1
+        cheb = dict(order=args.cheby_order, lo=lo_c, hi=hi_c, seconds=t_c, applies=napp,
+                    tflops=napp * apply_flops(V, nb, s) / t_c / 1e12)
+
     # ---- e2e: the same solve through the C-ABI call with pinned HOST buffers ----------------------------------
     Bh = B.cpu().pin_memory()
     Xh = torch.zeros_like(Bh).pin_memory()
@@ -394,7 +410,7 @@ def run_ours(args, cfg):
                             operator_bytes=81 * V * nb * nb * esize, parallelism="replicas only" if world > 1 else "1 GPU",
                             l2="inputs (27.5 GB operator) larger than L2; no flush", diagonal_shift_c=c),
                 clocks=clk, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,
-                sweep=sweep, block_cg_solve=bcg,
+                sweep=sweep, block_cg_solve=bcg, cheby_solve=cheb,
                 step_breakdown=dict(apply_ms=a_ms, other_ms=ms / K - a_ms, final_recursive_rel_res=max(out["rel_res_recursive"])))
     print(json.dumps(line))
     op.close()
@@ -414,6 +430,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3: the Nrhs-sweep workload)")
     ap.add_argument("--no-sweep", dest="sweep", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cheby-order", type=int, default=120, help="order of the Chebyshev coarse solve timed beside block CG (0: skip)")
     ap.add_argument("--cpu-sites", type=int, default=4096, help="sampled sites of the cpu_baseline leg")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="CPU time budget of the cpu_baseline leg")
     ap.add_argument("--ref-sites", type=int, default=384, help="sampled sites per step of --impl reference")

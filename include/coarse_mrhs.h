@@ -143,6 +143,22 @@ int block_cg_begin(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs
 int block_cg_step(coarse_op_t *op, int32_t count, void *stream);
 int block_cg_end(coarse_op_t *op, block_cg_result *res, void *stream);
 
+/*
+ * coarse_cheby_apply -- stationary polynomial coarse solve  X = P(H) B,  P = "Chebyshev approximation to 1/x over
+ * eigenspan [lo, hi]" of the given order, "coefficients ... at the Chebyshev interpolation points from the target function
+ * 1/x" (section 2.3; the paper's tuned coarse solve is [lo, hi, order] = [0.02, 40, 120], its smoother
+ * [2.0, 92.0] order 8).  Reading (R16): `order` = number of coefficients (degree order - 1), interpolation at the
+ * first-kind Chebyshev points of [lo, hi]; P(H) B by the three-term recurrence on blocks: order - 1 applications of the
+ * operator, each followed by ONE fused elementwise pass (T_{j+1} = 2 (a H T_j + b T_j) - T_{j-1}; X += c_{j+1} T_{j+1}),
+ * no reductions, no host synchronisation.
+ *   B_dev, X_dev : [V][nb][nrhs] device blocks of the operator's dtype, X_dev != B_dev; B is not modified
+ *   lo, hi       : 0 < lo < hi;  order >= 1;  coefficients are computed on the host in double precision
+ * Asynchronous on `stream`; uses the handle's block-CG workspace (do not interleave with a begin/step/end solve).
+ * Errors: COARSE_INVALID_ARG (NULL, aliasing, lo/hi/order/nrhs out of range), kernel launch errors.
+ */
+int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double lo, double hi, int32_t order,
+                       void *stream);
+
 /* Same with HOST buffers for B (in) and X (in: X0, out: solution). */
 int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
                         int32_t maxiter, block_cg_result *res, void *stream);

@@ -24,6 +24,7 @@ EXPORTS = [
     "block_cg_solve_host", "block_cg_begin", "block_cg_step", "block_cg_end", "coarse_block_gram", "coarse_small_cholesky", "coarse_small_hpd_inverse",
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
+    "coarse_cheby_apply",
 ]
 
 
@@ -75,6 +76,7 @@ def lib():
             "coarse_last_error": (C.c_char_p, []),
             "coarse_op_profile": (C.c_int, [vp, i32]),
             "coarse_op_profile_read": (C.c_int, [vp, C.POINTER(dbl), i32, C.POINTER(i32)]),
+            "coarse_cheby_apply": (C.c_int, [vp, vp, vp, i32, dbl, dbl, i32, vp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -166,6 +168,15 @@ class CoarseOperator:
         self._block_ok(Y)
         _check(lib().coarse_op_apply(self._h, _dev(X), _dev(Y), s, _stream(stream)))
         return Y
+
+    def cheby_apply(self, B: torch.Tensor, lo: float, hi: float, order: int, X: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+        """coarse_cheby_apply: X = P(H) B, P the order-`order` Chebyshev interpolant of 1/x on [lo, hi]."""
+        s = self._block_ok(B)
+        if X is None:
+            X = torch.empty_like(B)
+        self._block_ok(X)
+        _check(lib().coarse_cheby_apply(self._h, _dev(B), _dev(X), s, float(lo), float(hi), int(order), _stream(stream)))
+        return X
 
     def apply_host(self, X: torch.Tensor, Y: torch.Tensor, stream=None) -> torch.Tensor:
         """coarse_op_apply_host: X, Y are (pinned) HOST tensors; H2D + apply + D2H + sync."""

@@ -432,6 +432,28 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
     cp_async_wait<0>();
 }
 
+// Chebyshev recurrence, one fused elementwise pass:
+//   Tn = ca * Z + cb * Tc - cp * Tp   (Z = H Tc from the stencil kernel; Tn overwrites Tp)
+//   X  = cx * X + cn * Tn             (cx = 0 on the first call: X need not be initialised)
+template <typename T>
+__global__ void cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Tc, cplx<T> *Tp, cplx<T> *X,
+                                  T ca, T cb, T cp, T cx, T cn, int64_t total)
+{
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        const cplx<T> z = Z[e], tc = Tc[e];
+        cplx<T> tn;
+        tn.re = ca * z.re + cb * tc.re;
+        tn.im = ca * z.im + cb * tc.im;
+        if (cp != (T)0) { const cplx<T> tp = Tp[e]; tn.re -= cp * tp.re; tn.im -= cp * tp.im; }
+        Tp[e] = tn;
+        cplx<T> x = {0, 0};
+        if (cx != (T)0) { const cplx<T> xo = X[e]; x.re = cx * xo.re; x.im = cx * xo.im; }
+        x.re += cn * tn.re;
+        x.im += cn * tn.im;
+        X[e] = x;
+    }
+}
+
 // out = a*U + b*W elementwise (used for R = B - H X and copies)
 template <typename T>
 __global__ void axpby_kernel(const cplx<T> *U, const cplx<T> *W, cplx<T> *out, T a, T b, int64_t total)

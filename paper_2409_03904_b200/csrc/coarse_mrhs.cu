@@ -6,6 +6,8 @@
 #include <cstring>
 #include <atomic>
 #include <new>
+#include <vector>
+#include <cmath>
 
 #include "blockcg_kernels.cuh"
 #include "common.cuh"
@@ -858,6 +860,57 @@ extern "C" int block_cg_end(coarse_op_t *op, block_cg_result *res, void *stream)
 }
 
 // ---- per-launch timing of the stencil kernel, for bench.py's roofline object --------------------------------
+// ---- Chebyshev polynomial coarse solve ------------------------------------------------
+extern "C" int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double lo, double hi, int32_t order,
+                                  void *stream_v)
+{
+    if (!op || !B_dev || !X_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (B_dev == X_dev) { set_error("X must not alias B"); return COARSE_INVALID_ARG; }
+    if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (!(lo > 0.0) || !(hi > lo) || order < 1 || order > 100000) { set_error("need 0 < lo < hi and 1 <= order <= 100000"); return COARSE_INVALID_ARG; }
+    if (op->bcg_active) { set_error("coarse_cheby_apply inside an active block_cg_begin/end solve"); return COARSE_INVALID_ARG; }
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    // c_j = (2/n) sum_k f(x_k) cos(pi j (k + 1/2) / n), f = 1/x at the first-kind Chebyshev points of [lo, hi]
+    const int n = order;
+    std::vector<double> c((size_t)n), fk((size_t)n);
+    const double PI = 3.14159265358979323846;
+    for (int k = 0; k < n; ++k) fk[(size_t)k] = 1.0 / (0.5 * (hi + lo) + 0.5 * (hi - lo) * cos(PI * (k + 0.5) / n));
+    for (int j = 0; j < n; ++j) {
+        double acc = 0.0;
+        for (int k = 0; k < n; ++k) acc += fk[(size_t)k] * cos(PI * j * (k + 0.5) / n);
+        c[(size_t)j] = 2.0 * acc / n;
+    }
+    const double alpha = 2.0 / (hi - lo), beta = -(hi + lo) / (hi - lo);      // y(H) = alpha H + beta
+    const int64_t total = op->dims.V * op->nb * (int64_t)nrhs;
+    const size_t blk_bytes = (size_t)total * op->esize;
+    void *Z = op->blk[2], *Ta = op->blk[0], *Tb = op->blk[1];
+    const int grid = (int)(ceil_div(total, 256) < (int64_t)op->num_sms * 16 ? ceil_div(total, 256) : (int64_t)op->num_sms * 16);
+    auto step = [&](const void *z, const void *tc, void *tp, double ca, double cb, double cp, double cx, double cn) -> int {
+        if (op->dtype == COARSE_C64)
+            cheby_step_kernel<float><<<grid, 256, 0, stream>>>((const cplx<float> *)z, (const cplx<float> *)tc, (cplx<float> *)tp,
+                                                               (cplx<float> *)X_dev, (float)ca, (float)cb, (float)cp, (float)cx, (float)cn, total);
+        else
+            cheby_step_kernel<double><<<grid, 256, 0, stream>>>((const cplx<double> *)z, (const cplx<double> *)tc, (cplx<double> *)tp,
+                                                                (cplx<double> *)X_dev, ca, cb, cp, cx, cn, total);
+        CMRHS_LAUNCH_CHECK();
+        return COARSE_OK;
+    };
+    if (n == 1) return axpby_dispatch(op, B_dev, B_dev, X_dev, 0.5 * c[0], 0.0, total, stream);          // X = (c_0 / 2) B
+    // T_0 = B ;  T_1 = y(H) B -> Ta ;  X = (c_0/2) T_0 + c_1 T_1
+    CMRHS_STEP(apply_impl(op, B_dev, Z, nrhs, stream));
+    CMRHS_STEP(axpby_dispatch(op, B_dev, B_dev, X_dev, 0.5 * c[0], 0.0, total, stream));
+    CMRHS_STEP(step(Z, B_dev, Ta, alpha, beta, 0.0, 1.0, c[1]));
+    if (n == 2) return COARSE_OK;
+    CMRHS_CUDA(cudaMemcpyAsync(Tb, B_dev, blk_bytes, cudaMemcpyDeviceToDevice, stream));               // T_prev = T_0
+    void *tc = Ta, *tp = Tb;
+    for (int j = 1; j < n - 1; ++j) {
+        CMRHS_STEP(apply_impl(op, tc, Z, nrhs, stream));                                               // Z = H T_j
+        CMRHS_STEP(step(Z, tc, tp, 2.0 * alpha, 2.0 * beta, 1.0, 1.0, c[(size_t)j + 1]));              // T_{j+1} -> tp ; X += c_{j+1} T_{j+1}
+        void *t = tc; tc = tp; tp = t;
+    }
+    return COARSE_OK;
+}
+
 extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)
 {
     if (!op) { set_error("NULL argument"); return COARSE_INVALID_ARG; }

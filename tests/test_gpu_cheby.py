@@ -1,0 +1,76 @@
+"""-m gpu parity of coarse_cheby_apply (Chebyshev polynomial coarse solve) against oracle/cheby_oracle.py.
+
+Tolerances: the polynomial is evaluated by a three-term recurrence with order - 1 applications of the operator; rounding
+errors of the apply (1e-15 complex128, ~1.5e-7 complex64 per application) accumulate at most linearly in
+the order while the terms T_j(y(H)) B stay bounded by ||B|| (spectrum inside [lo, hi]); the result is compared norm-wise per
+column: <= 1e-12 (complex128), <= 1e-5 (complex64) -- north_star's figures -- for orders up to 32.
+"""
+import numpy as np
+import pytest
+import torch
+
+from gpu_common import TOL, host_case, to_dev, to_np
+from helpers import rel_err_cols
+from oracle import cheby_oracle, oracle
+
+pytestmark = pytest.mark.gpu
+
+import paper_2409_03904_b200 as cm  # noqa: E402
+
+
+def _gpu(dims, A, B, dtype, lo, hi, order, flags=0):
+    s = B.shape[-1]
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), s, flags=flags)
+    name = op.kernel_name(s)
+    Bd = to_dev(B, dtype)
+    X = to_np(op.cheby_apply(Bd, lo, hi, order))
+    assert np.array_equal(to_np(Bd), B.astype(np.complex64 if dtype == "c64" else np.complex128).astype(np.complex128))   # B untouched
+    op.close()
+    return X, name
+
+
+@pytest.mark.parametrize("dims,nb,s,dtype,order", [
+    ((4, 4, 4, 4), 8, 4, "c128", 12),       # BASELINE configs[0] shape
+    ((3, 3, 3, 5), 24, 8, "c128", 9),       # configs[1] shape, ragged lattice
+    ((4, 4, 4, 4), 32, 16, "c64", 8),       # configs[2] shape: FP16-split tensor kernel underneath; the paper's smoother order
+    ((3, 3, 2, 4), 32, 64, "c64", 16),      # transposed tensor form underneath
+    ((3, 2, 2, 3), 13, 5, "c128", 32),      # generic stencil kernel, odd sizes
+    ((4, 3, 3, 4), 24, 16, "c64", 1),       # order 1: X = B / midpoint
+    ((4, 3, 3, 4), 24, 16, "c64", 2),       # order 2: one application
+])
+def test_cheby_apply_matches_oracle(dims, nb, s, dtype, order):
+    A, c, _, B = host_case(dims, nb, s, seed=500 + nb + s, factor=1.05)
+    # the synthetic operator's spectrum lies within c +- 7 (off-diagonal part ~ +-2 sqrt(80/nb)); take a safe interval
+    lo, hi = c - 12.0, c + 12.0
+    X, name = _gpu(dims, A, B, dtype, lo, hi, order)
+    ref = cheby_oracle.cheby_apply(dims, A, B, lo, hi, order)
+    assert rel_err_cols(X, ref) <= TOL[dtype], (name, rel_err_cols(X, ref))
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_cheby_apply_is_an_approximate_inverse(dtype):
+    # property that holds at any size: ||B - H P(H) B|| <= ||B|| / |T_n(y(0))| (+ rounding) when spec(H) is inside [lo, hi]
+    dims, nb, s, order = (4, 4, 4, 6), 32, 16, 10
+    A, c, _, B = host_case(dims, nb, s, seed=9, factor=1.02)
+    lo, hi = c - 12.0, c + 12.0
+    X, _ = _gpu(dims, A, B, dtype, lo, hi, order)
+    R = B - oracle.apply(dims, A, X)
+    y0 = (hi + lo) / (hi - lo)
+    bound = 1.0 / np.cosh(order * np.arccosh(y0))
+    floor = 1e-13 if dtype == "c128" else 5e-7
+    rel = np.linalg.norm(R.reshape(-1, s), axis=0) / np.linalg.norm(B.reshape(-1, s), axis=0)
+    assert np.all(rel <= bound + floor), (rel.max(), bound)
+
+
+def test_cheby_apply_rejects_bad_arguments():
+    dims, nb, s = (2, 2, 2, 2), 8, 4
+    A, c, _, B = host_case(dims, nb, s, seed=1, factor=1.05)
+    op = cm.CoarseOperator(dims, to_dev(A, "c128"), s)
+    Bd = to_dev(B, "c128")
+    for lo, hi, order in [(0.0, 1.0, 4), (2.0, 1.0, 4), (1.0, 2.0, 0), (-1.0, 2.0, 3)]:
+        with pytest.raises(cm.binding.CoarseError) as ei:
+            op.cheby_apply(Bd, lo, hi, order)
+        assert ei.value.status == cm.binding.INVALID_ARG
+    with pytest.raises(cm.binding.CoarseError):
+        op.cheby_apply(Bd, 1.0, 2.0, 4, X=Bd)
+    op.close()
