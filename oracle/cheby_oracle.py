@@ -72,3 +72,32 @@ def cheby_apply(dims, A, B, lo: float, hi: float, order: int) -> np.ndarray:
         X = X + c[j + 1] * t_next
         t_prev, t_cur = t_cur, t_next
     return X
+
+
+# ---- multi-RHS deflation and the composite "Defl + Cheby" coarse solve (Eq. 7-12) ----
+# Definitions written out (complex128): with the n_ev lowest eigenpairs (|i>, lambda_i) of H as columns of Vev [n][nev],
+#   b_par  = (sum_i |i><i|) b                      (Eq. 8)
+#   b_perp = (1 - sum_i |i><i|) b                  (Eq. 9)
+#   Q b_par = (sum_i |i><i| / lambda_i) b          (Eq. 10)
+#   Q^{Cheby+defl} b = Defl(b_par) + P^{Cheby}(b_perp)     (Eq. 12)
+# applied to a block of right-hand sides at once (two tall-skinny products).
+# Pins: tests/test_oracle_cheby.py (full basis => H^-1 b by numpy.linalg.solve; b_par + b_perp = b; V^H b_perp = 0;
+# Eq. 11's diagonal form through a dense eigendecomposition).
+
+def deflate(Vev, lam, B):
+    """Vev [n][nev] (orthonormal columns), lam [nev], B [n][s]  ->  (Q b_par, b_perp), both [n][s]."""
+    Vev = np.asarray(Vev, dtype=np.complex128)
+    B = np.asarray(B, dtype=np.complex128)
+    C = Vev.conj().T @ B                                  # <i|b>
+    b_par = Vev @ C
+    b_perp = B - b_par
+    q_b_par = Vev @ (C / np.asarray(lam, dtype=np.float64)[:, None])
+    return q_b_par, b_perp
+
+
+def cheby_defl_solve(dims, A, Vev, lam, B, lo: float, hi: float, order: int) -> np.ndarray:
+    """Eq. 12 on a block B [V][nb][s]; Vev [V*nb][nev]."""
+    shape = B.shape
+    n, s = shape[0] * shape[1], shape[2]
+    q_b_par, b_perp = deflate(Vev, lam, np.asarray(B, dtype=np.complex128).reshape(n, s))
+    return q_b_par.reshape(shape) + cheby_apply(dims, A, b_perp.reshape(shape), lo, hi, order)

@@ -87,3 +87,49 @@ def test_columns_are_independent_and_map_is_linear():
         assert np.allclose(Xr[:, :, 0], X[:, :, r], rtol=1e-13, atol=1e-15)
     X2 = cheby_oracle.cheby_apply(dims, A, (2 - 1j) * B, lo, hi, order)
     assert np.allclose(X2, (2 - 1j) * X, rtol=1e-13, atol=1e-15)
+
+
+# ---- deflation and the composite solve (Eq. 7-12) ------------------------------------------------------------
+def _tiny_eigensystem(dims=(2, 2, 2, 2), nb=4, seed=13):
+    A, c = synth.make_operator(dims, nb, seed, 1.05)
+    H = dense_matrix(dims, A.astype(np.complex128))
+    lam, U = np.linalg.eigh(H)
+    return A, H, lam, U
+
+
+def test_deflation_with_the_full_basis_is_the_inverse():
+    A, H, lam, U = _tiny_eigensystem()
+    rng = np.random.default_rng(0)
+    B = rng.standard_normal((H.shape[0], 3)) + 1j * rng.standard_normal((H.shape[0], 3))
+    q, perp = cheby_oracle.deflate(U, lam, B)
+    assert np.allclose(q, np.linalg.solve(H, B), rtol=1e-11, atol=1e-13)
+    assert np.linalg.norm(perp) <= 1e-12 * np.linalg.norm(B)
+
+
+@pytest.mark.parametrize("nev", [1, 5, 16])
+def test_deflation_splits_the_source(nev):
+    A, H, lam, U = _tiny_eigensystem()
+    rng = np.random.default_rng(nev)
+    B = rng.standard_normal((H.shape[0], 4)) + 1j * rng.standard_normal((H.shape[0], 4))
+    V = U[:, :nev]
+    q, perp = cheby_oracle.deflate(V, lam[:nev], B)
+    assert np.linalg.norm(V.conj().T @ perp) <= 1e-12 * np.linalg.norm(B)            # b_perp is orthogonal to the space
+    assert np.allclose(H @ q + perp, B, rtol=1e-11, atol=1e-12)                       # H Q b_par = b_par, b_par + b_perp = b
+    q2, perp2 = cheby_oracle.deflate(V, lam[:nev], perp)                              # projecting twice changes nothing
+    assert np.linalg.norm(q2) <= 1e-12 * np.linalg.norm(B) and np.allclose(perp2, perp, atol=1e-12)
+
+
+@pytest.mark.parametrize("nev,order", [(4, 6), (10, 12)])
+def test_composite_solve_is_diagonal_in_the_eigenbasis(nev, order):
+    # Eq. 11: Q = diag(1/lambda_1 .. 1/lambda_nev, P(lambda_nev+1) .. P(lambda_max)) in the eigenbasis
+    dims, nb, s = (2, 2, 2, 2), 4, 3
+    A, H, lam, U = _tiny_eigensystem(dims, nb)
+    B = synth.make_block(dims, nb, s, 3, synth.TAG_B)
+    lo, hi = 0.9 * lam[nev], 1.1 * lam[-1]
+    a = npcheb.chebinterpolate(lambda y: 1.0 / (0.5 * (hi + lo) + 0.5 * (hi - lo) * y), order - 1)
+    qdiag = npcheb.chebval((2 * lam - hi - lo) / (hi - lo), a)
+    qdiag[:nev] = 1.0 / lam[:nev]
+    n = H.shape[0]
+    ref = (U * qdiag) @ (U.conj().T @ B.reshape(n, s))
+    X = cheby_oracle.cheby_defl_solve(dims, A, U[:, :nev], lam[:nev], B, lo, hi, order)
+    assert rel_err_cols(X.reshape(n, 1, s), ref.reshape(n, 1, s)) <= 1e-11
