@@ -159,6 +159,23 @@ int block_cg_end(coarse_op_t *op, block_cg_result *res, void *stream);
 int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double lo, double hi, int32_t order,
                        void *stream);
 
+/*
+ * coarse_deflate -- multi-RHS deflation with n_ev eigenpairs of the operator (Eq. 7-10; "applied to
+ * multiple right-hand sides"):  C = Vev^H B;  QBpar = Vev (C / lambda) = (sum_i |i><i| / lambda_i) b;
+ * Bperp = B - Vev C = (1 - sum_i |i><i|) b.  Two tall-skinny products: a deterministic two-stage reduction (complex128
+ * sums) and one pass over Vev and B.
+ *   Vev_dev     : [V*nbasis][nev] device block of the operator's dtype, eigenvector index fastest, orthonormal columns
+ *   lambda_host : [nev] HOST doubles, all > 0;  1 <= nev <= nrhs_max (<= 64) this round
+ *   B_dev       : [V][nb][nrhs];  QBpar_dev, Bperp_dev: outputs of the same shape, QBpar != B, QBpar != Bperp (Bperp may alias B)
+ * coarse_cheby_defl_solve -- the paper's stationary coarse solve  X = Defl(b_par) + P^Cheby(b_perp)  (Eq. 11-12), P as in
+ * coarse_cheby_apply.  Asynchronous on `stream`; both use the handle's block-CG workspace.
+ * Errors: COARSE_INVALID_ARG (NULL, aliasing, nev / nrhs / lambda / lo / hi / order out of range), launch errors.
+ */
+int coarse_deflate(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
+                   void *QBpar_dev, void *Bperp_dev, int32_t nrhs, void *stream);
+int coarse_cheby_defl_solve(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
+                            void *X_dev, int32_t nrhs, double lo, double hi, int32_t order, void *stream);
+
 /* Same with HOST buffers for B (in) and X (in: X0, out: solution). */
 int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
                         int32_t maxiter, block_cg_result *res, void *stream);

@@ -24,7 +24,7 @@ EXPORTS = [
     "block_cg_solve_host", "block_cg_begin", "block_cg_step", "block_cg_end", "coarse_block_gram", "coarse_small_cholesky", "coarse_small_hpd_inverse",
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
-    "coarse_cheby_apply",
+    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve",
 ]
 
 
@@ -77,6 +77,8 @@ def lib():
             "coarse_op_profile": (C.c_int, [vp, i32]),
             "coarse_op_profile_read": (C.c_int, [vp, C.POINTER(dbl), i32, C.POINTER(i32)]),
             "coarse_cheby_apply": (C.c_int, [vp, vp, vp, i32, dbl, dbl, i32, vp]),
+            "coarse_deflate": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, vp, i32, vp]),
+            "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -176,6 +178,31 @@ class CoarseOperator:
             X = torch.empty_like(B)
         self._block_ok(X)
         _check(lib().coarse_cheby_apply(self._h, _dev(B), _dev(X), s, float(lo), float(hi), int(order), _stream(stream)))
+        return X
+
+    def _evecs_ok(self, Vev: torch.Tensor, lam):
+        n = self.V * self.nbasis
+        if Vev.dtype != self.dtype or not Vev.is_cuda or not Vev.is_contiguous() or Vev.dim() != 2 or Vev.shape[0] != n:
+            raise ValueError(f"Vev must be a contiguous device tensor [{n}][nev] of dtype {self.dtype}")
+        nev = int(Vev.shape[1])
+        if len(lam) != nev:
+            raise ValueError("one eigenvalue per column of Vev")
+        return nev, (C.c_double * nev)(*[float(x) for x in lam])
+
+    def deflate(self, Vev: torch.Tensor, lam, B: torch.Tensor, stream=None):
+        """coarse_deflate: (Q b_par, b_perp) for a block B (Eq. 7-10)."""
+        s = self._block_ok(B)
+        nev, lam_c = self._evecs_ok(Vev, lam)
+        q, perp = torch.empty_like(B), torch.empty_like(B)
+        _check(lib().coarse_deflate(self._h, _dev(Vev), lam_c, nev, _dev(B), _dev(q), _dev(perp), s, _stream(stream)))
+        return q, perp
+
+    def cheby_defl_solve(self, Vev: torch.Tensor, lam, B: torch.Tensor, lo: float, hi: float, order: int, stream=None) -> torch.Tensor:
+        """coarse_cheby_defl_solve: X = Defl(b_par) + P^Cheby(b_perp) (Eq. 11-12)."""
+        s = self._block_ok(B)
+        nev, lam_c = self._evecs_ok(Vev, lam)
+        X = torch.empty_like(B)
+        _check(lib().coarse_cheby_defl_solve(self._h, _dev(Vev), lam_c, nev, _dev(B), _dev(X), s, float(lo), float(hi), int(order), _stream(stream)))
         return X
 
     def apply_host(self, X: torch.Tensor, Y: torch.Tensor, stream=None) -> torch.Tensor:

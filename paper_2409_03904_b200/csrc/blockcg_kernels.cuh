@@ -454,6 +454,95 @@ __global__ void cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *
     }
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Multi-RHS deflation (Eq. 7-10, 325-329): two tall-skinny products with the n x m block of eigenvectors.
+//   stage 1: C = Vev^H B (m x s) -- per-CTA partials in double, summed by gram_reduce_kernel (deterministic)
+//   stage 2: Qb_par = Vev (C / lambda),  b_perp = B - Vev C        (one pass over Vev and B)
+// ------------------------------------------------------------------------------------------------------
+struct DeflLambda { double inv[COARSE_MAX_NRHS]; };      // 1 / lambda_i, passed by value
+
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads)
+rgram_partial_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict__ B, int64_t n, int m, int s, int rows_per_tile,
+                     zdouble *__restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sV = reinterpret_cast<cplx<T> *>(smem_raw);
+    cplx<T> *sB = sV + (size_t)rows_per_tile * m;
+    constexpr int MAXE = (COARSE_MAX_NRHS * COARSE_MAX_NRHS) / kLaThreads;      // entries of C per thread
+    const int ms = m * s;
+    double accr[MAXE], acci[MAXE];
+    int ei[MAXE], er[MAXE];
+#pragma unroll
+    for (int j = 0; j < MAXE; ++j) {
+        const int e = threadIdx.x + j * kLaThreads;
+        accr[j] = 0.0; acci[j] = 0.0;
+        ei[j] = e < ms ? e / s : -1;
+        er[j] = e < ms ? e % s : 0;
+    }
+    const int64_t chunk = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t r_begin = blockIdx.x * chunk;
+    const int64_t r_end = (r_begin + chunk < n) ? r_begin + chunk : n;
+    for (int64_t r0 = r_begin; r0 < r_end; r0 += rows_per_tile) {
+        const int nrow = (int)((r_end - r0 < rows_per_tile) ? (r_end - r0) : rows_per_tile);
+        __syncthreads();
+        for (int e = threadIdx.x; e < nrow * m; e += kLaThreads) sV[e] = Vev[r0 * m + e];
+        for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) sB[e] = B[r0 * s + e];
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < MAXE; ++j) {
+            if (ei[j] < 0) continue;
+            double re = 0.0, im = 0.0;
+            for (int k = 0; k < nrow; ++k) {
+                const cplx<T> v = sV[k * m + ei[j]], b = sB[k * s + er[j]];
+                re += (double)v.re * (double)b.re + (double)v.im * (double)b.im;       // conj(v) * b
+                im += (double)v.re * (double)b.im - (double)v.im * (double)b.re;
+            }
+            accr[j] += re; acci[j] += im;
+        }
+    }
+    zdouble *out = partial + (size_t)blockIdx.x * ms;
+#pragma unroll
+    for (int j = 0; j < MAXE; ++j)
+        if (ei[j] >= 0) out[threadIdx.x + j * kLaThreads] = {accr[j], acci[j]};
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads)
+deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict__ B, const zdouble *__restrict__ Cm, const DeflLambda lam,
+                      cplx<T> *__restrict__ QBpar, cplx<T> *__restrict__ Bperp, int64_t n, int m, int s, int rows_per_tile)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sC = reinterpret_cast<cplx<T> *>(smem_raw);          // [m][s]   <i|b>
+    cplx<T> *sCl = sC + m * s;                                     // [m][s]   <i|b> / lambda_i
+    cplx<T> *sV = sCl + m * s;                                     // [rows_per_tile][m]
+    for (int e = threadIdx.x; e < m * s; e += kLaThreads) {
+        const double il = lam.inv[e / s];
+        sC[e].re = (T)Cm[e].re; sC[e].im = (T)Cm[e].im;
+        sCl[e].re = (T)(Cm[e].re * il); sCl[e].im = (T)(Cm[e].im * il);
+    }
+    const int64_t ntiles = (n + rows_per_tile - 1) / rows_per_tile;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t r0 = t * rows_per_tile;
+        const int nrow = (int)((n - r0 < rows_per_tile) ? (n - r0) : rows_per_tile);
+        __syncthreads();
+        for (int e = threadIdx.x; e < nrow * m; e += kLaThreads) sV[e] = Vev[r0 * m + e];
+        __syncthreads();
+        for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) {
+            const int k = e / s, r = e - k * s;
+            cplx<T> par = {0, 0}, q = {0, 0};
+            for (int i = 0; i < m; ++i) {
+                const cplx<T> v = sV[k * m + i];
+                cmac(par, v, sC[i * s + r]);
+                cmac(q, v, sCl[i * s + r]);
+            }
+            const cplx<T> b = B[r0 * s + e];
+            QBpar[r0 * s + e] = q;
+            Bperp[r0 * s + e] = {b.re - par.re, b.im - par.im};
+        }
+    }
+}
+
 // out = a*U + b*W elementwise (used for R = B - H X and copies)
 template <typename T>
 __global__ void axpby_kernel(const cplx<T> *U, const cplx<T> *W, cplx<T> *out, T a, T b, int64_t total)

@@ -861,15 +861,20 @@ extern "C" int block_cg_end(coarse_op_t *op, block_cg_result *res, void *stream)
 
 // ---- per-launch timing of the stencil kernel, for bench.py's roofline object --------------------------------
 // ---- Chebyshev polynomial coarse solve ------------------------------------------------
-extern "C" int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double lo, double hi, int32_t order,
-                                  void *stream_v)
+static int cheby_check(const coarse_op *op, const void *B_dev, const void *X_dev, int nrhs, double lo, double hi, int order)
 {
     if (!op || !B_dev || !X_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
     if (B_dev == X_dev) { set_error("X must not alias B"); return COARSE_INVALID_ARG; }
     if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
     if (!(lo > 0.0) || !(hi > lo) || order < 1 || order > 100000) { set_error("need 0 < lo < hi and 1 <= order <= 100000"); return COARSE_INVALID_ARG; }
-    if (op->bcg_active) { set_error("coarse_cheby_apply inside an active block_cg_begin/end solve"); return COARSE_INVALID_ARG; }
-    cudaStream_t stream = (cudaStream_t)stream_v;
+    if (op->bcg_active) { set_error("polynomial solve inside an active block_cg_begin/end solve"); return COARSE_INVALID_ARG; }
+    return COARSE_OK;
+}
+
+// X = (accumulate ? X : 0) + P(H) B
+static int cheby_impl(coarse_op *op, const void *B_dev, void *X_dev, int nrhs, double lo, double hi, int order, bool accumulate,
+                      cudaStream_t stream)
+{
     // c_j = (2/n) sum_k f(x_k) cos(pi j (k + 1/2) / n), f = 1/x at the first-kind Chebyshev points of [lo, hi]
     const int n = order;
     std::vector<double> c((size_t)n), fk((size_t)n);
@@ -895,10 +900,12 @@ extern "C" int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_de
         CMRHS_LAUNCH_CHECK();
         return COARSE_OK;
     };
-    if (n == 1) return axpby_dispatch(op, B_dev, B_dev, X_dev, 0.5 * c[0], 0.0, total, stream);          // X = (c_0 / 2) B
-    // T_0 = B ;  T_1 = y(H) B -> Ta ;  X = (c_0/2) T_0 + c_1 T_1
+    const void *x_in = accumulate ? X_dev : B_dev;                  // (with b = 0 the second operand is only read)
+    const double keep = accumulate ? 1.0 : 0.0;
+    if (n == 1) return axpby_dispatch(op, B_dev, x_in, X_dev, 0.5 * c[0], keep, total, stream);          // X = (c_0 / 2) B [+ X]
+    // T_0 = B ;  T_1 = y(H) B -> Ta ;  X = (c_0/2) T_0 + c_1 T_1 [+ X]
     CMRHS_STEP(apply_impl(op, B_dev, Z, nrhs, stream));
-    CMRHS_STEP(axpby_dispatch(op, B_dev, B_dev, X_dev, 0.5 * c[0], 0.0, total, stream));
+    CMRHS_STEP(axpby_dispatch(op, B_dev, x_in, X_dev, 0.5 * c[0], keep, total, stream));
     CMRHS_STEP(step(Z, B_dev, Ta, alpha, beta, 0.0, 1.0, c[1]));
     if (n == 2) return COARSE_OK;
     CMRHS_CUDA(cudaMemcpyAsync(Tb, B_dev, blk_bytes, cudaMemcpyDeviceToDevice, stream));               // T_prev = T_0
@@ -909,6 +916,78 @@ extern "C" int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_de
         void *t = tc; tc = tp; tp = t;
     }
     return COARSE_OK;
+}
+
+extern "C" int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double lo, double hi, int32_t order,
+                                  void *stream)
+{
+    CMRHS_STEP(cheby_check(op, B_dev, X_dev, nrhs, lo, hi, order));
+    return cheby_impl(op, B_dev, X_dev, nrhs, lo, hi, order, false, (cudaStream_t)stream);
+}
+
+// ---- multi-RHS deflation and the composite Defl + Cheby coarse solve (Eq. 7-12) ------------------
+static int deflate_check(const coarse_op *op, const void *Vev, const double *lambda, int nev, int nrhs)
+{
+    if (!Vev || !lambda) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (nev < 1 || nev > op->nrhs_max || nev > COARSE_MAX_NRHS) { set_error("nev %d outside 1..nrhs_max (%d)", nev, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
+    for (int i = 0; i < nev; ++i)
+        if (!(lambda[i] > 0.0)) { set_error("lambda[%d] is not positive", i); return COARSE_INVALID_ARG; }
+    return COARSE_OK;
+}
+
+template <typename T>
+static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, int m, const void *B, void *QBpar, void *Bperp, int s,
+                        cudaStream_t stream)
+{
+    const int64_t n = op->dims.V * op->nb;
+    zdouble *Cm = small_view(op).G;                     // m x s <= 64 x 64 complex128
+    // stage 1: C = Vev^H B
+    int rows = (int)(32768 / ((size_t)(m + s) * sizeof(cplx<T>)));
+    if (rows < 1) rows = 1;
+    int blocks = op->gram_blocks;
+    if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
+    const size_t smem1 = (size_t)rows * (m + s) * sizeof(cplx<T>);
+    rgram_partial_kernel<T><<<blocks, kLaThreads, smem1, stream>>>((const cplx<T> *)Vev, (const cplx<T> *)B, n, m, s, rows, op->gram_partial);
+    CMRHS_LAUNCH_CHECK();
+    gram_reduce_kernel<<<(m * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, m * s, Cm);
+    CMRHS_LAUNCH_CHECK();
+    // stage 2: Qb_par = Vev (C / lambda), b_perp = B - Vev C
+    DeflLambda lam;
+    for (int i = 0; i < COARSE_MAX_NRHS; ++i) lam.inv[i] = i < m ? 1.0 / lambda[i] : 0.0;
+    const int rows2 = 64;
+    const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);
+    auto kern = deflate_update_kernel<T>;
+    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem2 > 49152 ? smem2 : 49152)));
+    const int64_t ntiles = ceil_div(n, rows2);
+    const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
+    kern<<<grid, kLaThreads, smem2, stream>>>((const cplx<T> *)Vev, (const cplx<T> *)B, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, rows2);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+extern "C" int coarse_deflate(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
+                              void *QBpar_dev, void *Bperp_dev, int32_t nrhs, void *stream)
+{
+    if (!op || !B_dev || !QBpar_dev || !Bperp_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (B_dev == QBpar_dev || QBpar_dev == Bperp_dev) { set_error("outputs must not alias each other or B's first output"); return COARSE_INVALID_ARG; }
+    CMRHS_STEP(deflate_check(op, Vev_dev, lambda_host, nev, nrhs));
+    if (op->bcg_active) { set_error("coarse_deflate inside an active block_cg_begin/end solve"); return COARSE_INVALID_ARG; }
+    return op->dtype == COARSE_C64 ? deflate_impl<float>(op, Vev_dev, lambda_host, nev, B_dev, QBpar_dev, Bperp_dev, nrhs, (cudaStream_t)stream)
+                                   : deflate_impl<double>(op, Vev_dev, lambda_host, nev, B_dev, QBpar_dev, Bperp_dev, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int coarse_cheby_defl_solve(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
+                                       void *X_dev, int32_t nrhs, double lo, double hi, int32_t order, void *stream_v)
+{
+    CMRHS_STEP(cheby_check(op, B_dev, X_dev, nrhs, lo, hi, order));
+    CMRHS_STEP(deflate_check(op, Vev_dev, lambda_host, nev, nrhs));
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    void *Bperp = op->blk[3];
+    // X = Defl(b_par) ; b_perp -> workspace ; X += P(H) b_perp                                   (Eq. 12)
+    if (op->dtype == COARSE_C64) CMRHS_STEP(deflate_impl<float>(op, Vev_dev, lambda_host, nev, B_dev, X_dev, Bperp, nrhs, stream));
+    else CMRHS_STEP(deflate_impl<double>(op, Vev_dev, lambda_host, nev, B_dev, X_dev, Bperp, nrhs, stream));
+    return cheby_impl(op, Bperp, X_dev, nrhs, lo, hi, order, true, stream);
 }
 
 extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)

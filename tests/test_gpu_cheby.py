@@ -74,3 +74,46 @@ def test_cheby_apply_rejects_bad_arguments():
     with pytest.raises(cm.binding.CoarseError):
         op.cheby_apply(Bd, 1.0, 2.0, 4, X=Bd)
     op.close()
+
+
+# ---- deflation and the composite Defl + Cheby solve (Eq. 7-12) -------------------------------------------------
+def _eigenpairs(dims, nb, seed, nev):
+    """lowest nev eigenpairs of the synthetic operator from a dense eigendecomposition of the brute-force matrix (tiny lattices)."""
+    from helpers import dense_matrix
+    from inputs import synth
+    A, c = synth.make_operator(dims, nb, seed, 1.05)
+    lam, U = np.linalg.eigh(dense_matrix(dims, A.astype(np.complex128)))
+    return A, lam, U[:, :nev].copy(), lam[:nev].copy()
+
+
+@pytest.mark.parametrize("dims,nb,s,nev,dtype", [((2, 2, 2, 2), 8, 4, 6, "c128"), ((2, 2, 2, 3), 8, 16, 16, "c64"),
+                                                 ((2, 2, 2, 2), 4, 5, 3, "c128"), ((2, 2, 2, 2), 8, 64, 33, "c64")])
+def test_deflate_matches_oracle(dims, nb, s, nev, dtype):
+    from inputs import synth
+    A, lam_all, Vev, lam = _eigenpairs(dims, nb, 31, nev)
+    B = synth.make_block(dims, nb, s, 31, synth.TAG_B)
+    n = B.shape[0] * B.shape[1]
+    Vq = Vev.astype(np.complex64).astype(np.complex128) if dtype == "c64" else Vev       # what the device sees
+    q_ref, perp_ref = cheby_oracle.deflate(Vq, lam, B.reshape(n, s))
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), max(s, nev))
+    q, perp = op.deflate(to_dev(Vev, dtype), lam, to_dev(B, dtype))
+    op.close()
+    tol = 1e-12 if dtype == "c128" else 2e-6
+    assert rel_err_cols(to_np(q).reshape(n, 1, s), q_ref.reshape(n, 1, s)) <= tol
+    assert rel_err_cols(to_np(perp).reshape(n, 1, s), perp_ref.reshape(n, 1, s)) <= tol
+
+
+@pytest.mark.parametrize("dims,nb,s,nev,order,dtype", [((2, 2, 2, 2), 8, 4, 6, 10, "c128"), ((2, 2, 2, 3), 8, 16, 12, 8, "c64")])
+def test_cheby_defl_solve_matches_oracle(dims, nb, s, nev, order, dtype):
+    from inputs import synth
+    A, lam_all, Vev, lam = _eigenpairs(dims, nb, 32, nev)
+    B = synth.make_block(dims, nb, s, 32, synth.TAG_B)
+    lo, hi = 0.95 * lam_all[nev], 1.05 * lam_all[-1]
+    Vq = Vev.astype(np.complex64).astype(np.complex128) if dtype == "c64" else Vev
+    ref = cheby_oracle.cheby_defl_solve(dims, A, Vq, lam, B, lo, hi, order)
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), max(s, nev))
+    X = to_np(op.cheby_defl_solve(to_dev(Vev, dtype), lam, to_dev(B, dtype), lo, hi, order))
+    with pytest.raises(cm.binding.CoarseError):
+        op.cheby_defl_solve(to_dev(Vev, dtype), -lam, to_dev(B, dtype), lo, hi, order)          # non-positive eigenvalues
+    op.close()
+    assert rel_err_cols(X, ref) <= TOL[dtype]
