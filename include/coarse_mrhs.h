@@ -176,6 +176,31 @@ int coarse_deflate(coarse_op_t *op, const void *Vev_dev, const double *lambda_ho
 int coarse_cheby_defl_solve(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
                             void *X_dev, int32_t nrhs, double lo, double hi, int32_t order, void *stream);
 
+/*
+ * pblock_cg_solve -- Preconditioned BlockCGrQ (Fig. 2 right) for H X = B with a STATIONARY Hermitian
+ * positive definite preconditioner M^-1: the Chebyshev polynomial of H (coarse_cheby_apply) or the
+ * deflated Chebyshev solve (coarse_cheby_defl_solve).  Statement by statement as printed, with the two readings of
+ * DESIGN.md (the update is X += D_k N_k C_k; one Cholesky factor S per iteration, S^H S = T^H t).  Both the unpreconditioned
+ * (q, z, t) and the preconditioned (Q, Z, T) blocks are rotated; Gram products in the M inner product are Z^H z, D^H z, T^H t.
+ * Stop test: the Euclidean residual r_{k+1} = q_{k+1} C_{k+1} = t_k C_k, max_r ||r[:,r]|| / ||B[:,r]|| <= tol (one extra Gram
+ * t^H t per iteration), taken BEFORE the factorisation of T^H t: once converged that matrix is rounding noise.
+ *   B_dev, X_dev : as block_cg_solve (X in: X_0, out: solution);  M: host struct, its pointers as in coarse_deflate
+ *   res          : host; rel_res_recursive = the stop quantity at the last iteration, rel_res_true from one extra apply
+ * Synchronises the stream every iteration (stop scalar).  Allocates five more workspace blocks on first use.
+ * Returns COARSE_OK, COARSE_NOT_CONVERGED (outputs valid), COARSE_BREAKDOWN, COARSE_INVALID_ARG, COARSE_OUT_OF_MEMORY.
+ */
+enum { COARSE_PRECOND_CHEBY = 0, COARSE_PRECOND_DEFL_CHEBY = 1 };
+typedef struct {
+    int32_t kind;                 /* COARSE_PRECOND_* */
+    int32_t order;                /* Chebyshev order (number of coefficients) */
+    double lo, hi;                /* Chebyshev interval */
+    const void *Vev_dev;          /* DEFL_CHEBY: [V*nbasis][nev] eigenvectors (device), else NULL */
+    const double *lambda_host;    /* DEFL_CHEBY: [nev] eigenvalues (host), else NULL */
+    int32_t nev;
+} coarse_precond;
+int pblock_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
+                    const coarse_precond *M, block_cg_result *res, void *stream);
+
 /* Same with HOST buffers for B (in) and X (in: X0, out: solution). */
 int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
                         int32_t maxiter, block_cg_result *res, void *stream);

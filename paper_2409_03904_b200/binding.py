@@ -24,7 +24,7 @@ EXPORTS = [
     "block_cg_solve_host", "block_cg_begin", "block_cg_step", "block_cg_end", "coarse_block_gram", "coarse_small_cholesky", "coarse_small_hpd_inverse",
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
-    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve",
+    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve",
 ]
 
 
@@ -39,6 +39,13 @@ class BlockCGResult(C.Structure):
                 ("rel_res_recursive", C.c_double * MAX_NRHS), ("rel_res_true", C.c_double * MAX_NRHS),
                 ("history", C.c_double * MAX_HISTORY), ("seconds", C.c_double)]
 
+
+class CoarsePrecond(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("order", C.c_int32), ("lo", C.c_double), ("hi", C.c_double),
+                ("Vev_dev", C.c_void_p), ("lambda_host", C.POINTER(C.c_double)), ("nev", C.c_int32)]
+
+
+PRECOND_CHEBY, PRECOND_DEFL_CHEBY = 0, 1
 
 _lib = None
 
@@ -78,6 +85,7 @@ def lib():
             "coarse_op_profile_read": (C.c_int, [vp, C.POINTER(dbl), i32, C.POINTER(i32)]),
             "coarse_cheby_apply": (C.c_int, [vp, vp, vp, i32, dbl, dbl, i32, vp]),
             "coarse_deflate": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, vp, i32, vp]),
+            "pblock_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(CoarsePrecond), C.POINTER(BlockCGResult), vp]),
             "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
         }
         for name, (res, args) in sig.items():
@@ -229,6 +237,24 @@ class CoarseOperator:
         self._block_ok(X)
         res = BlockCGResult()
         _check(lib().block_cg_solve(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), C.byref(res), _stream(stream)),
+               allow=(NOT_CONVERGED, BREAKDOWN))
+        return self._result(res, s, X)
+
+    def pblock_cg(self, B: torch.Tensor, lo: float, hi: float, order: int, Vev: torch.Tensor | None = None, lam=None,
+                  X: torch.Tensor | None = None, tol: float = 1e-6, maxiter: int = 1000, stream=None):
+        """pblock_cg_solve: Preconditioned BlockCGrQ (Fig. 2 right); preconditioner = Chebyshev polynomial of
+        the operator on [lo, hi], deflated with the eigenpairs (Vev, lam) when given."""
+        s = self._block_ok(B)
+        if X is None:
+            X = torch.zeros_like(B)
+        self._block_ok(X)
+        M = CoarsePrecond(kind=PRECOND_CHEBY, order=int(order), lo=float(lo), hi=float(hi), Vev_dev=None, lambda_host=None, nev=0)
+        keep = None
+        if Vev is not None:
+            nev, keep = self._evecs_ok(Vev, lam)
+            M.kind, M.Vev_dev, M.lambda_host, M.nev = PRECOND_DEFL_CHEBY, _dev(Vev), C.cast(keep, C.POINTER(C.c_double)), nev
+        res = BlockCGResult()
+        _check(lib().pblock_cg_solve(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), C.byref(M), C.byref(res), _stream(stream)),
                allow=(NOT_CONVERGED, BREAKDOWN))
         return self._result(res, s, X)
 

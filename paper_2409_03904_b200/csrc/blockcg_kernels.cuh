@@ -792,6 +792,59 @@ __global__ void bcg_step2_kernel(BcgSmall w, int s)
     }
 }
 
+// ---- Preconditioned BlockCGrQ (Fig. 2 right): the small kernels that differ from the plain ones ----
+// relres[r] = sqrt(G[r][r]) / bnorm[r] from G = z_0^H z_0; stop[0] = max, stop[1] = 0
+__global__ void pbcg_rel0_kernel(BcgSmall w, int s)
+{
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int r = 0; r < s; ++r) {
+            const double rel = sqrt(fmax(w.G[r * s + r].re, 0.0)) / w.bnorm[r];
+            w.relres[r] = rel;
+            m = fmax(m, rel);
+        }
+        w.stop[0] = m;
+        w.stop[1] = 0.0;
+    }
+}
+// G = Z_0^H z_0 = <Z_0|Z_0>_M:  C_0 = chol(G),  K1 = C_0^-1
+__global__ void pbcg_init_kernel(BcgSmall w, int s)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s;
+    __shared__ int flag;
+    if (threadIdx.x == 0) flag = 0;
+    sm_load(m0, w.G, s * s);
+    sm_cholesky_upper(m0, s, &flag);
+    __syncthreads();
+    if (flag) { if (threadIdx.x == 0) w.stop[1] = 1.0; return; }
+    sm_store(w.C, m0, s * s);
+    sm_upper_inverse(m0, m1, s);
+    sm_store(w.K1, m1, s * s);
+}
+// Euclidean residual r_k = q_k C_k:  relres[r] = sqrt((C^H G C)_rr) / bnorm[r] with G = q^H q;  stop[0] = max
+__global__ void pbcg_resid_kernel(BcgSmall w, int s)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s, *m2 = m1 + s * s;
+    sm_load(m0, w.G, s * s);
+    sm_load(m1, w.C, s * s);
+    sm_matmul(m0, m1, m2, s, 0, 0);          // m2 = G C
+    __shared__ double rel[COARSE_MAX_NRHS];
+    for (int r = threadIdx.x; r < s; r += blockDim.x) {
+        double acc = 0.0;                     // Re (C^H G C)_rr = Re sum_a conj(C[a][r]) (G C)[a][r]
+        for (int a = 0; a < s; ++a) acc += m1[a * s + r].re * m2[a * s + r].re + m1[a * s + r].im * m2[a * s + r].im;
+        rel[r] = sqrt(fmax(acc, 0.0)) / w.bnorm[r];
+        w.relres[r] = rel[r];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int r = 0; r < s; ++r) m = fmax(m, rel[r]);
+        w.stop[0] = m;
+    }
+}
+
 // column norms of a block from the diagonal of its Gram matrix: out[r] = sqrt(G[r][r]) / bnorm[r]
 __global__ void bcg_truerel_kernel(BcgSmall w, int s, double *out)
 {

@@ -85,6 +85,7 @@ struct coarse_op {
     unsigned char *Xh = nullptr; // [V] split operand tiles of the current X (pre-pass of the FP16-split kernel)
     uint32_t *amax = nullptr;    // [64] per-column max |x| bit patterns (pre-pass of the FP16-split kernel) + [64] scratch
     int32_t *nbr = nullptr;      // [V][81]
+    void *pblk[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};           // q, Q, D, z, Z of pblock_cg_solve (allocated on first use)
     void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
     zdouble *gram_partial = nullptr;
     int gram_blocks = 0;
@@ -154,6 +155,7 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     if (!op) return COARSE_OK;
     cudaFree(op->At);
     cudaFree(op->Ak);
+    for (int b = 0; b < 5; ++b) cudaFree(op->pblk[b]);
     cudaFree(op->Ah);
     cudaFree(op->Xh);
     cudaFree(op->amax);
@@ -977,17 +979,120 @@ extern "C" int coarse_deflate(coarse_op_t *op, const void *Vev_dev, const double
                                    : deflate_impl<double>(op, Vev_dev, lambda_host, nev, B_dev, QBpar_dev, Bperp_dev, nrhs, (cudaStream_t)stream);
 }
 
-extern "C" int coarse_cheby_defl_solve(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
-                                       void *X_dev, int32_t nrhs, double lo, double hi, int32_t order, void *stream_v)
+// X = Defl(b_par) + P(H) b_perp  (Eq. 12); b_perp goes through workspace block 3
+static int cheby_defl_impl(coarse_op *op, const void *Vev_dev, const double *lambda_host, int nev, const void *B_dev, void *X_dev, int nrhs,
+                           double lo, double hi, int order, cudaStream_t stream)
 {
-    CMRHS_STEP(cheby_check(op, B_dev, X_dev, nrhs, lo, hi, order));
-    CMRHS_STEP(deflate_check(op, Vev_dev, lambda_host, nev, nrhs));
-    cudaStream_t stream = (cudaStream_t)stream_v;
     void *Bperp = op->blk[3];
-    // X = Defl(b_par) ; b_perp -> workspace ; X += P(H) b_perp                                   (Eq. 12)
     if (op->dtype == COARSE_C64) CMRHS_STEP(deflate_impl<float>(op, Vev_dev, lambda_host, nev, B_dev, X_dev, Bperp, nrhs, stream));
     else CMRHS_STEP(deflate_impl<double>(op, Vev_dev, lambda_host, nev, B_dev, X_dev, Bperp, nrhs, stream));
     return cheby_impl(op, Bperp, X_dev, nrhs, lo, hi, order, true, stream);
+}
+
+extern "C" int coarse_cheby_defl_solve(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
+                                       void *X_dev, int32_t nrhs, double lo, double hi, int32_t order, void *stream)
+{
+    CMRHS_STEP(cheby_check(op, B_dev, X_dev, nrhs, lo, hi, order));
+    CMRHS_STEP(deflate_check(op, Vev_dev, lambda_host, nev, nrhs));
+    return cheby_defl_impl(op, Vev_dev, lambda_host, nev, B_dev, X_dev, nrhs, lo, hi, order, (cudaStream_t)stream);
+}
+
+// ---- Preconditioned BlockCGrQ (Fig. 2 right) with a stationary preconditioner -----------------
+static int precond_apply(coarse_op *op, const coarse_precond *M, const void *z, void *Z, int s, cudaStream_t stream)
+{
+    if (M->kind == COARSE_PRECOND_CHEBY) return cheby_impl(op, z, Z, s, M->lo, M->hi, M->order, false, stream);
+    return cheby_defl_impl(op, M->Vev_dev, M->lambda_host, M->nev, z, Z, s, M->lo, M->hi, M->order, stream);
+}
+
+extern "C" int pblock_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
+                               const coarse_precond *M, block_cg_result *res, void *stream_v)
+{
+    if (!op || !B_dev || !X_dev || !M || !res) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (B_dev == X_dev) { set_error("X must not alias B"); return COARSE_INVALID_ARG; }
+    if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (!(tol >= 0.0) || maxiter < 0) { set_error("bad tol / maxiter"); return COARSE_INVALID_ARG; }
+    if (M->kind != COARSE_PRECOND_CHEBY && M->kind != COARSE_PRECOND_DEFL_CHEBY) { set_error("unknown preconditioner kind %d", M->kind); return COARSE_INVALID_ARG; }
+    if (!(M->lo > 0.0) || !(M->hi > M->lo) || M->order < 1 || M->order > 100000) { set_error("preconditioner: need 0 < lo < hi and 1 <= order <= 100000"); return COARSE_INVALID_ARG; }
+    if (M->kind == COARSE_PRECOND_DEFL_CHEBY) CMRHS_STEP(deflate_check(op, M->Vev_dev, M->lambda_host, M->nev, nrhs));
+    if (op->bcg_active) { set_error("pblock_cg_solve inside an active block_cg_begin/end solve"); return COARSE_INVALID_ARG; }
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    const int s = nrhs;
+    const int64_t n = op->dims.V * op->nb, total = n * s;
+    const size_t blk_bytes_max = (size_t)n * op->nrhs_max * op->esize;
+    for (int b = 0; b < 5; ++b)                     // q, Q, D, z, Z: allocated on first use (blocks 0-3 belong to the preconditioner)
+        if (!op->pblk[b]) CMRHS_STEP(alloc_dev(op, &op->pblk[b], blk_bytes_max));
+    void *q = op->pblk[0], *Q = op->pblk[1], *D = op->pblk[2], *z = op->pblk[3], *Z = op->pblk[4];
+    BcgSmall w = small_view(op);
+    const double *h_stop = op->hpin + 64;
+    memset(res, 0, sizeof(*res));
+    for (int k = 0; k < COARSE_MAX_HISTORY; ++k) res->history[k] = -1.0;
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    const auto t0 = std::chrono::steady_clock::now();
+    auto small3 = [&](void (*kern)(BcgSmall, int)) -> int { return small_launch(kern, op, s, 3, stream); };
+    // ||B[:,r]|| ;  z_0 = B - H X_0 ;  relative residual of the start
+    CMRHS_STEP(gram_dispatch(op, B_dev, B_dev, w.G, n, s, stream));
+    bcg_bnorm_kernel<<<1, 64, 0, stream>>>(w, s);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(apply_impl(op, X_dev, Z, s, stream));
+    CMRHS_STEP(axpby_dispatch(op, B_dev, Z, z, 1.0, -1.0, total, stream));
+    CMRHS_STEP(gram_dispatch(op, z, z, w.G, n, s, stream));
+    pbcg_rel0_kernel<<<1, 32, 0, stream>>>(w, s);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(fetch_scalars(op, stream));
+    res->history[0] = h_stop[0];
+    int status = COARSE_NOT_CONVERGED, its = 0;
+    if (h_stop[0] <= tol) status = COARSE_OK;
+    else {
+        // Z_0 = M^-1 z_0 ;  C_0^H C_0 = Z_0^H z_0 ;  q_0 = z_0 C_0^-1 ;  Q_0 = Z_0 C_0^-1 ;  D_0 = Q_0
+        CMRHS_STEP(precond_apply(op, M, z, Z, s, stream));
+        CMRHS_STEP(gram_dispatch(op, Z, z, w.G, n, s, stream));
+        CMRHS_STEP(small3(pbcg_init_kernel));
+        CMRHS_STEP(rotate_dispatch(op, z, w.K1, nullptr, q, 0.0, n, s, stream));
+        CMRHS_STEP(rotate_dispatch(op, Z, w.K1, nullptr, Q, 0.0, n, s, stream));
+        CMRHS_CUDA(cudaMemcpyAsync(D, Q, (size_t)total * op->esize, cudaMemcpyDeviceToDevice, stream));
+        for (int k = 0; k < maxiter; ++k) {
+            CMRHS_STEP(apply_impl(op, D, z, s, stream));                                   // z_k = H D_k
+            CMRHS_STEP(precond_apply(op, M, z, Z, s, stream));                             // Z_k = M^-1 z_k
+            CMRHS_STEP(gram_dispatch(op, D, z, w.G, n, s, stream));                        // D^H z
+            CMRHS_STEP(small3(bcg_step1_kernel));                                          // N ; K1 = N C ; K2 = -N
+            CMRHS_STEP(rotate_dispatch(op, D, w.K1, X_dev, X_dev, 1.0, n, s, stream));     // X += D N C
+            CMRHS_STEP(rotate_dispatch(op, z, w.K2, q, q, 1.0, n, s, stream));             // t = q - z N   (in place)
+            CMRHS_STEP(rotate_dispatch(op, Z, w.K2, Q, Q, 1.0, n, s, stream));             // T = Q - Z N   (in place)
+            // stop test first: the residual of X_{k+1} is r_{k+1} = q_{k+1} C_{k+1} = t_k C_k, so it is available before the
+            // factorisation (near convergence T^H t is dominated by rounding and need not be positive definite any more)
+            CMRHS_STEP(gram_dispatch(op, q, q, w.G, n, s, stream));                        // t^H t -> ||t C_k|| column norms
+            CMRHS_STEP(small3(pbcg_resid_kernel));
+            CMRHS_STEP(fetch_scalars(op, stream));
+            its = k + 1;
+            if (h_stop[1] != 0.0) { status = COARSE_BREAKDOWN; break; }
+            if (its < COARSE_MAX_HISTORY) res->history[its] = h_stop[0];
+            for (int r = 0; r < s; ++r) res->rel_res_recursive[r] = op->hpin[r];
+            if (h_stop[0] <= tol) { status = COARSE_OK; break; }
+            if (its == maxiter) break;
+            CMRHS_STEP(gram_dispatch(op, Q, q, w.G, n, s, stream));                        // T^H t = <T|T>_M
+            CMRHS_STEP(small3(bcg_step2_kernel));                                          // S ; K3 = S^-1 ; K4 = S^H ; C = S C
+            CMRHS_STEP(rotate_dispatch(op, q, w.K3, nullptr, q, 0.0, n, s, stream));       // q = t S^-1    (in place)
+            CMRHS_STEP(rotate_dispatch(op, Q, w.K3, nullptr, Q, 0.0, n, s, stream));       // Q = T S^-1    (in place)
+            CMRHS_STEP(rotate_dispatch(op, D, w.K4, Q, D, 1.0, n, s, stream));             // D = Q + D S^H
+        }
+        if (status == COARSE_NOT_CONVERGED || status == COARSE_OK) {                       // a breakdown inside step1 / step2 shows up here
+            CMRHS_STEP(fetch_scalars(op, stream));
+            if (h_stop[1] != 0.0) status = COARSE_BREAKDOWN;
+        }
+    }
+    if (its == 0) for (int r = 0; r < s; ++r) res->rel_res_recursive[r] = op->hpin[r];
+    // true residual from one extra apply
+    CMRHS_STEP(apply_impl(op, X_dev, Z, s, stream));
+    CMRHS_STEP(axpby_dispatch(op, B_dev, Z, z, 1.0, -1.0, total, stream));
+    CMRHS_STEP(gram_dispatch(op, z, z, w.G, n, s, stream));
+    bcg_truerel_kernel<<<1, 64, 0, stream>>>(w, s, op->dscal + 130);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(fetch_scalars(op, stream));
+    for (int r = 0; r < s; ++r) res->rel_res_true[r] = op->hpin[66 + r];
+    res->iterations = its;
+    res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    res->status = status;
+    return status;
 }
 
 extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)
