@@ -94,7 +94,9 @@ int coarse_op_destroy(coarse_op_t *op);
  * (Eq. 19 summed over the stencil; the paper issues 81 batched GEMMs).
  *   X_dev, Y_dev : device, [V][nbasis][nrhs], dtype of the operator; Y must not alias X
  *   nrhs         : 1..nrhs_max
- * Asynchronous on `stream`; allocates nothing.
+ * Asynchronous on `stream`; allocates nothing.  complex64, nbasis 32, nrhs 4 or a multiple of 8 (the split-FP16 tensor
+ * kernel): two short pre-pass kernels first write the scaled, split copy of X into a scratch block OWNED BY THE HANDLE, so
+ * applies on one handle must be ordered (same stream, or externally synchronised); distinct handles are independent.
  */
 int coarse_op_apply(const coarse_op_t *op, const void *X_dev, void *Y_dev, int32_t nrhs, void *stream);
 

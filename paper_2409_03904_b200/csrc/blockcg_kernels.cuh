@@ -436,10 +436,44 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
 //   Tn = ca * Z + cb * Tc - cp * Tp   (Z = H Tc from the stencil kernel; Tn overwrites Tp)
 //   X  = cx * X + cn * Tn             (cx = 0 on the first call: X need not be initialised)
 template <typename T>
-__global__ void cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Tc, cplx<T> *Tp, cplx<T> *X,
-                                  T ca, T cb, T cp, T cx, T cn, int64_t total)
+__global__ void __launch_bounds__(256)
+cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Tc, cplx<T> *Tp, cplx<T> *X,
+                  T ca, T cb, T cp, T cx, T cn, int64_t total)
 {
-    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+    // 32 bytes per thread and array per trip (4 complex64 / 2 complex128), all loads issued before the arithmetic
+    constexpr int VEC = 32 / (int)sizeof(cplx<T>);
+    const int64_t nvec = total / VEC;
+    for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < nvec; v += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t e0 = v * VEC;
+        cplx<T> z[VEC], tc[VEC], tp[VEC], x[VEC];
+#pragma unroll
+        for (int u = 0; u < VEC; u += 16 / (int)sizeof(cplx<T>)) {
+            *reinterpret_cast<float4 *>(&z[u]) = *reinterpret_cast<const float4 *>(&Z[e0 + u]);
+            *reinterpret_cast<float4 *>(&tc[u]) = *reinterpret_cast<const float4 *>(&Tc[e0 + u]);
+            if (cp != (T)0) *reinterpret_cast<float4 *>(&tp[u]) = *reinterpret_cast<const float4 *>(&Tp[e0 + u]);
+            if (cx != (T)0) *reinterpret_cast<float4 *>(&x[u]) = *reinterpret_cast<const float4 *>(&X[e0 + u]);
+        }
+#pragma unroll
+        for (int u = 0; u < VEC; ++u) {
+            cplx<T> tn;
+            tn.re = ca * z[u].re + cb * tc[u].re;
+            tn.im = ca * z[u].im + cb * tc[u].im;
+            if (cp != (T)0) { tn.re -= cp * tp[u].re; tn.im -= cp * tp[u].im; }
+            cplx<T> xo = {0, 0};
+            if (cx != (T)0) { xo.re = cx * x[u].re; xo.im = cx * x[u].im; }
+            xo.re += cn * tn.re;
+            xo.im += cn * tn.im;
+            tp[u] = tn;
+            x[u] = xo;
+        }
+#pragma unroll
+        for (int u = 0; u < VEC; u += 16 / (int)sizeof(cplx<T>)) {
+            *reinterpret_cast<float4 *>(&Tp[e0 + u]) = *reinterpret_cast<const float4 *>(&tp[u]);
+            *reinterpret_cast<float4 *>(&X[e0 + u]) = *reinterpret_cast<const float4 *>(&x[u]);
+        }
+    }
+    // ragged tail (total not a multiple of VEC)
+    for (int64_t e = nvec * VEC + blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
         const cplx<T> z = Z[e], tc = Tc[e];
         cplx<T> tn;
         tn.re = ca * z.re + cb * tc.re;

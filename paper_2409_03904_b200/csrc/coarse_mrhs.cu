@@ -891,7 +891,8 @@ static int cheby_impl(coarse_op *op, const void *B_dev, void *X_dev, int nrhs, d
     const int64_t total = op->dims.V * op->nb * (int64_t)nrhs;
     const size_t blk_bytes = (size_t)total * op->esize;
     void *Z = op->blk[2], *Ta = op->blk[0], *Tb = op->blk[1];
-    const int grid = (int)(ceil_div(total, 256) < (int64_t)op->num_sms * 16 ? ceil_div(total, 256) : (int64_t)op->num_sms * 16);
+    const int64_t cvec = ceil_div(total, (int64_t)(32 / op->esize) * 256);
+    const int grid = (int)(cvec < (int64_t)op->num_sms * 8 ? (cvec < 1 ? 1 : cvec) : (int64_t)op->num_sms * 8);
     auto step = [&](const void *z, const void *tc, void *tp, double ca, double cb, double cp, double cx, double cn) -> int {
         if (op->dtype == COARSE_C64)
             cheby_step_kernel<float><<<grid, 256, 0, stream>>>((const cplx<float> *)z, (const cplx<float> *)tc, (cplx<float> *)tp,
