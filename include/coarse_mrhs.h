@@ -203,6 +203,18 @@ typedef struct {
 int pblock_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
                     const coarse_precond *M, block_cg_result *res, void *stream);
 
+/*
+ * stacked_cg_solve -- the coarse solve "as an enlarged five dimensional system with a single Krylov solve, albeit with a
+ * block diagonal structure": plain conjugate gradients on (I_nrhs (x) H) vec(X) = vec(B), ONE alpha and
+ * ONE beta per iteration from Frobenius inner products over all right-hand sides.  Per iteration: one apply, two fused
+ * elementwise passes (X += alpha P, R -= alpha Z with <R,R>;  P = R + beta P), one inner product; scalars stay on the device,
+ * one stop scalar goes to the host.  Stop: ||R||_F / ||B||_F <= tol (R18); res->history holds that quantity,
+ * rel_res_recursive its last value in every column, rel_res_true the per-column true residuals from one extra apply.
+ * Arguments and return codes as block_cg_solve.
+ */
+int stacked_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
+                     block_cg_result *res, void *stream);
+
 /* Same with HOST buffers for B (in) and X (in: X0, out: solution). */
 int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
                         int32_t maxiter, block_cg_result *res, void *stream);

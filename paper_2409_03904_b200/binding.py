@@ -24,7 +24,7 @@ EXPORTS = [
     "block_cg_solve_host", "block_cg_begin", "block_cg_step", "block_cg_end", "coarse_block_gram", "coarse_small_cholesky", "coarse_small_hpd_inverse",
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
-    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve",
+    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve", "stacked_cg_solve",
 ]
 
 
@@ -85,6 +85,7 @@ def lib():
             "coarse_op_profile_read": (C.c_int, [vp, C.POINTER(dbl), i32, C.POINTER(i32)]),
             "coarse_cheby_apply": (C.c_int, [vp, vp, vp, i32, dbl, dbl, i32, vp]),
             "coarse_deflate": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, vp, i32, vp]),
+            "stacked_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(BlockCGResult), vp]),
             "pblock_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(CoarsePrecond), C.POINTER(BlockCGResult), vp]),
             "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
         }
@@ -237,6 +238,17 @@ class CoarseOperator:
         self._block_ok(X)
         res = BlockCGResult()
         _check(lib().block_cg_solve(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), C.byref(res), _stream(stream)),
+               allow=(NOT_CONVERGED, BREAKDOWN))
+        return self._result(res, s, X)
+
+    def stacked_cg(self, B: torch.Tensor, X: torch.Tensor | None = None, tol: float = 1e-6, maxiter: int = 1000, stream=None):
+        """stacked_cg_solve: single-Krylov CG on the stacked system."""
+        s = self._block_ok(B)
+        if X is None:
+            X = torch.zeros_like(B)
+        self._block_ok(X)
+        res = BlockCGResult()
+        _check(lib().stacked_cg_solve(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), C.byref(res), _stream(stream)),
                allow=(NOT_CONVERGED, BREAKDOWN))
         return self._result(res, s, X)
 

@@ -577,6 +577,86 @@ deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict
     }
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Stacked single-Krylov CG: one alpha / beta per iteration from Frobenius inner products over the
+// whole block.  Scalars live on the device (sc: 0 rho, 1 alpha, 2 beta, 3 ||B||_F^2, 4 stop = sqrt(rho / ||B||^2)).
+// Reductions: fixed partition over CTAs, fixed order inside (shuffle tree, then warp 0), partials summed by one warp.
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void la_block_sum_store(double v, double *out)
+{
+    __shared__ double wsum[kLaThreads / 32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < kLaThreads / 32; ++k) t += wsum[k];
+        *out = t;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads) fdot_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W, int64_t total,
+                                                                  double *__restrict__ partial)
+{
+    const int64_t chunk = (total + gridDim.x - 1) / gridDim.x;
+    const int64_t e0 = blockIdx.x * chunk, e1 = (e0 + chunk < total) ? e0 + chunk : total;
+    double acc = 0.0;
+    for (int64_t e = e0 + threadIdx.x; e < e1; e += kLaThreads) {
+        const cplx<T> u = U[e], w = W[e];
+        acc += (double)u.re * (double)w.re + (double)u.im * (double)w.im;         // Re conj(u) w
+    }
+    la_block_sum_store(acc, partial + blockIdx.x);
+}
+
+// mode 0: ||B||^2 ; 1: rho_0 (+ stop) ; 2: alpha = rho / <P, Z> ; 3: beta = rho' / rho, rho <- rho' (+ stop)
+__global__ void scg_scalar_kernel(int mode, const double *__restrict__ partial, int nblocks, double *sc)
+{
+    double v = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += 32) v += partial[b];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (threadIdx.x != 0) return;
+    if (mode == 0) sc[3] = v > 0.0 ? v : 1.0;
+    else if (mode == 1) { sc[0] = v; sc[4] = sqrt(v / sc[3]); }
+    else if (mode == 2) sc[1] = sc[0] / v;
+    else { sc[2] = v / sc[0]; sc[0] = v; sc[4] = sqrt(v / sc[3]); }
+}
+
+// X += alpha P ; R -= alpha Z ; partial(<R, R>)
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads) scg_update1_kernel(const cplx<T> *__restrict__ P, const cplx<T> *__restrict__ Z, cplx<T> *X, cplx<T> *R,
+                                                                 const double *__restrict__ sc, int64_t total, double *__restrict__ partial)
+{
+    const T alpha = (T)sc[1];
+    const int64_t chunk = (total + gridDim.x - 1) / gridDim.x;
+    const int64_t e0 = blockIdx.x * chunk, e1 = (e0 + chunk < total) ? e0 + chunk : total;
+    double acc = 0.0;
+    for (int64_t e = e0 + threadIdx.x; e < e1; e += kLaThreads) {
+        const cplx<T> p = P[e], z = Z[e];
+        cplx<T> x = X[e], r = R[e];
+        x.re += alpha * p.re; x.im += alpha * p.im;
+        r.re -= alpha * z.re; r.im -= alpha * z.im;
+        X[e] = x;
+        R[e] = r;
+        acc += (double)r.re * (double)r.re + (double)r.im * (double)r.im;
+    }
+    la_block_sum_store(acc, partial + blockIdx.x);
+}
+
+// P = R + beta P
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads) scg_update2_kernel(const cplx<T> *__restrict__ R, cplx<T> *P, const double *__restrict__ sc, int64_t total)
+{
+    const T beta = (T)sc[2];
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        const cplx<T> r = R[e];
+        cplx<T> p = P[e];
+        p.re = r.re + beta * p.re;
+        p.im = r.im + beta * p.im;
+        P[e] = p;
+    }
+}
+
 // out = a*U + b*W elementwise (used for R = B - H X and copies)
 template <typename T>
 __global__ void axpby_kernel(const cplx<T> *U, const cplx<T> *W, cplx<T> *out, T a, T b, int64_t total)

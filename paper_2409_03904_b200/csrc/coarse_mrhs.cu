@@ -1096,6 +1096,97 @@ extern "C" int pblock_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, 
     return status;
 }
 
+// ---- stacked single-Krylov CG ---------------------------------------------------------------
+template <typename T>
+static int stacked_cg_impl(coarse_op *op, const void *B_dev, void *X_dev, int s, double tol, int maxiter, block_cg_result *res, cudaStream_t stream)
+{
+    const int64_t n = op->dims.V * op->nb, total = n * s;
+    cplx<T> *R = (cplx<T> *)op->blk[0], *P = (cplx<T> *)op->blk[1], *Z = (cplx<T> *)op->blk[2];
+    const cplx<T> *B = (const cplx<T> *)B_dev;
+    cplx<T> *X = (cplx<T> *)X_dev;
+    double *partial = reinterpret_cast<double *>(op->gram_partial), *sc = op->dscal + 200;
+    const int nblk = op->gram_blocks;
+    const int egrid = (int)(ceil_div(total, 256) < (int64_t)op->num_sms * 16 ? ceil_div(total, 256) : (int64_t)op->num_sms * 16);
+    BcgSmall w = small_view(op);
+    auto fetch_stop = [&](double *out) -> int {
+        CMRHS_CUDA(cudaMemcpyAsync(op->hpin + 200, sc, 5 * sizeof(double), cudaMemcpyDeviceToHost, stream));
+        CMRHS_CUDA(cudaStreamSynchronize(stream));
+        *out = op->hpin[204];
+        return COARSE_OK;
+    };
+    // ||B||_F^2 ;  R = B - H X_0 ;  rho_0
+    fdot_partial_kernel<T><<<nblk, kLaThreads, 0, stream>>>(B, B, total, partial);
+    CMRHS_LAUNCH_CHECK();
+    scg_scalar_kernel<<<1, 32, 0, stream>>>(0, partial, nblk, sc);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(apply_impl(op, X, Z, s, stream));
+    CMRHS_STEP(axpby_dispatch(op, B, Z, R, 1.0, -1.0, total, stream));
+    fdot_partial_kernel<T><<<nblk, kLaThreads, 0, stream>>>(R, R, total, partial);
+    CMRHS_LAUNCH_CHECK();
+    scg_scalar_kernel<<<1, 32, 0, stream>>>(1, partial, nblk, sc);
+    CMRHS_LAUNCH_CHECK();
+    double stop = 0.0;
+    CMRHS_STEP(fetch_stop(&stop));
+    res->history[0] = stop;
+    int status = COARSE_NOT_CONVERGED, its = 0;
+    if (stop <= tol) status = COARSE_OK;
+    else {
+        CMRHS_CUDA(cudaMemcpyAsync(P, R, (size_t)total * sizeof(cplx<T>), cudaMemcpyDeviceToDevice, stream));
+        for (int k = 0; k < maxiter; ++k) {
+            CMRHS_STEP(apply_impl(op, P, Z, s, stream));                                        // Z = H P
+            fdot_partial_kernel<T><<<nblk, kLaThreads, 0, stream>>>(P, Z, total, partial);
+            CMRHS_LAUNCH_CHECK();
+            scg_scalar_kernel<<<1, 32, 0, stream>>>(2, partial, nblk, sc);                       // alpha
+            CMRHS_LAUNCH_CHECK();
+            scg_update1_kernel<T><<<nblk, kLaThreads, 0, stream>>>(P, Z, X, R, sc, total, partial);   // X, R, <R, R>
+            CMRHS_LAUNCH_CHECK();
+            scg_scalar_kernel<<<1, 32, 0, stream>>>(3, partial, nblk, sc);                       // beta, rho, stop
+            CMRHS_LAUNCH_CHECK();
+            CMRHS_STEP(fetch_stop(&stop));
+            its = k + 1;
+            if (its < COARSE_MAX_HISTORY) res->history[its] = stop;
+            if (!(stop == stop)) { status = COARSE_BREAKDOWN; break; }
+            if (stop <= tol) { status = COARSE_OK; break; }
+            scg_update2_kernel<T><<<egrid, 256, 0, stream>>>(R, P, sc, total);                   // P = R + beta P
+            CMRHS_LAUNCH_CHECK();
+        }
+    }
+    for (int r = 0; r < s; ++r) res->rel_res_recursive[r] = stop;
+    // per-column true residuals from one extra apply
+    CMRHS_STEP(gram_dispatch(op, B, B, w.G, n, s, stream));
+    bcg_bnorm_kernel<<<1, 64, 0, stream>>>(w, s);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(apply_impl(op, X, Z, s, stream));
+    CMRHS_STEP(axpby_dispatch(op, B, Z, R, 1.0, -1.0, total, stream));
+    CMRHS_STEP(gram_dispatch(op, R, R, w.G, n, s, stream));
+    bcg_truerel_kernel<<<1, 64, 0, stream>>>(w, s, op->dscal + 130);
+    CMRHS_LAUNCH_CHECK();
+    CMRHS_STEP(fetch_scalars(op, stream));
+    for (int r = 0; r < s; ++r) res->rel_res_true[r] = op->hpin[66 + r];
+    res->iterations = its;
+    res->status = status;
+    return status;
+}
+
+extern "C" int stacked_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
+                                block_cg_result *res, void *stream_v)
+{
+    if (!op || !B_dev || !X_dev || !res) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (B_dev == X_dev) { set_error("X must not alias B"); return COARSE_INVALID_ARG; }
+    if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (!(tol >= 0.0) || maxiter < 0) { set_error("bad tol / maxiter"); return COARSE_INVALID_ARG; }
+    if (op->bcg_active) { set_error("stacked_cg_solve inside an active block_cg_begin/end solve"); return COARSE_INVALID_ARG; }
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    memset(res, 0, sizeof(*res));
+    for (int k = 0; k < COARSE_MAX_HISTORY; ++k) res->history[k] = -1.0;
+    CMRHS_CUDA(cudaStreamSynchronize(stream));
+    const auto t0 = std::chrono::steady_clock::now();
+    const int st = op->dtype == COARSE_C64 ? stacked_cg_impl<float>(op, B_dev, X_dev, nrhs, tol, maxiter, res, stream)
+                                           : stacked_cg_impl<double>(op, B_dev, X_dev, nrhs, tol, maxiter, res, stream);
+    res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return st;
+}
+
 extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)
 {
     if (!op) { set_error("NULL argument"); return COARSE_INVALID_ARG; }

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared_symbols():
     text = open(os.path.join(ROOT, "include", "coarse_mrhs.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    names = re.findall(r"\b(coarse_[a-z_0-9]+|p?block_cg_[a-z_0-9]+)\s*\(", text)
+    names = re.findall(r"\b(coarse_[a-z_0-9]+|p?block_cg_[a-z_0-9]+|stacked_cg_[a-z_0-9]+)\s*\(", text)
     return sorted(set(names))
 
 
