@@ -215,6 +215,21 @@ int pblock_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrh
 int stacked_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
                      block_cg_result *res, void *stream);
 
+/*
+ * coarse_block_project / coarse_block_promote -- multi-RHS transfer between grids (section 2.5.1), "one
+ * matrix multiply for each coarse lattice site":
+ *   project (Eq. 14):  C[x] (nbasis x nrhs) = Basis[x]^dagger (nbasis x vblock) . F[x] (vblock x nrhs)
+ *   promote (Eq. 15):  F[x] (vblock x nrhs) = Basis[x] (vblock x nbasis) . C[x] (nbasis x nrhs)
+ * Layouts (device, row-major, interleaved complex of `dtype`): Basis [Vc][vblock][nbasis], fine vectors [Vc][vblock][nrhs]
+ * (the fine field block by block -- the paper's "BLAS ready layout"), coarse vectors [Vc][nbasis][nrhs] (the layout of
+ * coarse_op_apply).  Stateless (no handle), asynchronous on `stream`, allocate nothing.  nbasis, nrhs <= 64.
+ * Errors: COARSE_INVALID_ARG, launch errors.  (SIMT kernels, one CTA per coarse site; not tuned this round.)
+ */
+int coarse_block_project(const void *Basis_dev, const void *F_dev, void *C_dev, int64_t Vc, int32_t vblock, int32_t nbasis,
+                         int32_t nrhs, int32_t dtype, void *stream);
+int coarse_block_promote(const void *Basis_dev, const void *C_dev, void *F_dev, int64_t Vc, int32_t vblock, int32_t nbasis,
+                         int32_t nrhs, int32_t dtype, void *stream);
+
 /* Same with HOST buffers for B (in) and X (in: X0, out: solution). */
 int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
                         int32_t maxiter, block_cg_result *res, void *stream);

@@ -24,7 +24,7 @@ EXPORTS = [
     "block_cg_solve_host", "block_cg_begin", "block_cg_step", "block_cg_end", "coarse_block_gram", "coarse_small_cholesky", "coarse_small_hpd_inverse",
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
-    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve", "stacked_cg_solve",
+    "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve", "stacked_cg_solve", "coarse_block_project", "coarse_block_promote",
 ]
 
 
@@ -85,6 +85,8 @@ def lib():
             "coarse_op_profile_read": (C.c_int, [vp, C.POINTER(dbl), i32, C.POINTER(i32)]),
             "coarse_cheby_apply": (C.c_int, [vp, vp, vp, i32, dbl, dbl, i32, vp]),
             "coarse_deflate": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, vp, i32, vp]),
+            "coarse_block_project": (C.c_int, [vp, vp, vp, i64, i32, i32, i32, i32, vp]),
+            "coarse_block_promote": (C.c_int, [vp, vp, vp, i64, i32, i32, i32, i32, vp]),
             "stacked_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(BlockCGResult), vp]),
             "pblock_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(CoarsePrecond), C.POINTER(BlockCGResult), vp]),
             "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
@@ -347,3 +349,27 @@ def fill_block(dims, nbasis: int, nrhs: int, dtype: torch.dtype, seed: int, tag:
     X = torch.empty((V, nbasis, nrhs), dtype=dtype, device=device)
     _check(lib().coarse_fill_block(_dev(X), _dims(dims), nbasis, nrhs, _dtype_code(X), int(seed), int(tag), _stream(stream)))
     return X
+
+
+def _transfer(fn, Basis: torch.Tensor, src: torch.Tensor, out_rows: int, stream=None) -> torch.Tensor:
+    if Basis.dim() != 3 or src.dim() != 3 or Basis.shape[0] != src.shape[0] or Basis.dtype != src.dtype:
+        raise ValueError("Basis [Vc][vblock][nbasis] and the vector block must share Vc and dtype")
+    dt = C64 if Basis.dtype == torch.complex64 else C128
+    Vc, vb, nb = (int(x) for x in Basis.shape)
+    out = torch.empty((Vc, out_rows, int(src.shape[2])), dtype=src.dtype, device=src.device)
+    _check(fn(_dev(Basis), _dev(src), _dev(out), Vc, vb, nb, int(src.shape[2]), dt, _stream(stream)))
+    return out
+
+
+def block_project(Basis: torch.Tensor, F: torch.Tensor, stream=None) -> torch.Tensor:
+    """coarse_block_project (Eq. 14): C[x] = Basis[x]^dagger F[x]."""
+    if F.shape[1] != Basis.shape[1]:
+        raise ValueError("F must be [Vc][vblock][nrhs]")
+    return _transfer(lib().coarse_block_project, Basis, F, int(Basis.shape[2]), stream)
+
+
+def block_promote(Basis: torch.Tensor, Cc: torch.Tensor, stream=None) -> torch.Tensor:
+    """coarse_block_promote (Eq. 15): F[x] = Basis[x] C[x]."""
+    if Cc.shape[1] != Basis.shape[2]:
+        raise ValueError("C must be [Vc][nbasis][nrhs]")
+    return _transfer(lib().coarse_block_promote, Basis, Cc, int(Basis.shape[1]), stream)

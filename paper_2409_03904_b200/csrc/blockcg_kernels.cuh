@@ -657,6 +657,82 @@ __global__ void __launch_bounds__(kLaThreads) scg_update2_kernel(const cplx<T> *
     }
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Multi-RHS transfer between grids (Eq. 14-15): one small GEMM per coarse site, one CTA per site
+// (grid-stride).  basis [Vc][vb][nb], fine [Vc][vb][s], coarse [Vc][nb][s]; products in T, sums over V_block in double (project).
+// ------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads)
+block_project_kernel(const cplx<T> *__restrict__ Bas, const cplx<T> *__restrict__ F, cplx<T> *__restrict__ Cc, int64_t Vc, int vb, int nb, int s,
+                     int rows_per_tile)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sB = reinterpret_cast<cplx<T> *>(smem_raw);
+    cplx<T> *sF = sB + (size_t)rows_per_tile * nb;
+    constexpr int MAXE = (COARSE_MAX_NBASIS * COARSE_MAX_NRHS) / kLaThreads;
+    const int ms = nb * s;
+    int ek[MAXE], er[MAXE];
+#pragma unroll
+    for (int j = 0; j < MAXE; ++j) {
+        const int e = threadIdx.x + j * kLaThreads;
+        ek[j] = e < ms ? e / s : -1;
+        er[j] = e < ms ? e % s : 0;
+    }
+    for (int64_t x = blockIdx.x; x < Vc; x += gridDim.x) {
+        double accr[MAXE], acci[MAXE];
+#pragma unroll
+        for (int j = 0; j < MAXE; ++j) { accr[j] = 0.0; acci[j] = 0.0; }
+        const cplx<T> *bx = Bas + x * (int64_t)vb * nb, *fx = F + x * (int64_t)vb * s;
+        for (int v0 = 0; v0 < vb; v0 += rows_per_tile) {
+            const int nrow = (vb - v0 < rows_per_tile) ? (vb - v0) : rows_per_tile;
+            __syncthreads();
+            for (int e = threadIdx.x; e < nrow * nb; e += kLaThreads) sB[e] = bx[(int64_t)v0 * nb + e];
+            for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) sF[e] = fx[(int64_t)v0 * s + e];
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < MAXE; ++j) {
+                if (ek[j] < 0) continue;
+                cplx<T> run = {0, 0};
+                for (int v = 0; v < nrow; ++v) cmac_conj(run, sB[v * nb + ek[j]], sF[v * s + er[j]]);
+                accr[j] += (double)run.re; acci[j] += (double)run.im;
+            }
+        }
+        cplx<T> *cx = Cc + x * (int64_t)ms;
+#pragma unroll
+        for (int j = 0; j < MAXE; ++j)
+            if (ek[j] >= 0) cx[threadIdx.x + j * kLaThreads] = {(T)accr[j], (T)acci[j]};
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads)
+block_promote_kernel(const cplx<T> *__restrict__ Bas, const cplx<T> *__restrict__ Cc, cplx<T> *__restrict__ F, int64_t Vc, int vb, int nb, int s,
+                     int rows_per_tile)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sC = reinterpret_cast<cplx<T> *>(smem_raw);          // [nb][s]
+    cplx<T> *sB = sC + nb * s;                                     // [rows_per_tile][nb + 1]
+    const int ld = nb + 1;
+    for (int64_t x = blockIdx.x; x < Vc; x += gridDim.x) {
+        const cplx<T> *bx = Bas + x * (int64_t)vb * nb;
+        cplx<T> *fx = F + x * (int64_t)vb * s;
+        __syncthreads();
+        for (int e = threadIdx.x; e < nb * s; e += kLaThreads) sC[e] = Cc[x * (int64_t)nb * s + e];
+        for (int v0 = 0; v0 < vb; v0 += rows_per_tile) {
+            const int nrow = (vb - v0 < rows_per_tile) ? (vb - v0) : rows_per_tile;
+            __syncthreads();
+            for (int e = threadIdx.x; e < nrow * nb; e += kLaThreads) sB[(e / nb) * ld + e % nb] = bx[(int64_t)v0 * nb + e];
+            __syncthreads();
+            for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) {
+                const int v = e / s, r = e - v * s;
+                cplx<T> acc = {0, 0};
+                for (int k = 0; k < nb; ++k) cmac(acc, sB[v * ld + k], sC[k * s + r]);
+                fx[(int64_t)v0 * s + e] = acc;
+            }
+        }
+    }
+}
+
 // out = a*U + b*W elementwise (used for R = B - H X and copies)
 template <typename T>
 __global__ void axpby_kernel(const cplx<T> *U, const cplx<T> *W, cplx<T> *out, T a, T b, int64_t total)

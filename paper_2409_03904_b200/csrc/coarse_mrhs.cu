@@ -1187,6 +1187,56 @@ extern "C" int stacked_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev,
     return st;
 }
 
+// ---- multi-RHS block project / promote (Eq. 14-15) -----------------------------------------------------
+static int transfer_check(const void *a, const void *b, const void *c, int64_t Vc, int vb, int nb, int s, int dtype)
+{
+    if (!a || !b || !c) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (dtype != COARSE_C64 && dtype != COARSE_C128) { set_error("dtype must be COARSE_C64 or COARSE_C128"); return COARSE_INVALID_ARG; }
+    if (Vc < 1 || vb < 1 || nb < 1 || nb > COARSE_MAX_NBASIS || s < 1 || s > COARSE_MAX_NRHS) { set_error("bad Vc / vblock / nbasis / nrhs"); return COARSE_INVALID_ARG; }
+    return COARSE_OK;
+}
+
+template <typename T>
+static int transfer_launch(bool project, const void *Bas, const void *in, void *out, int64_t Vc, int vb, int nb, int s, cudaStream_t stream)
+{
+    int dev = 0, sms = 0;
+    CMRHS_CUDA(cudaGetDevice(&dev));
+    CMRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int grid = (int)(Vc < (int64_t)sms * 4 ? Vc : (int64_t)sms * 4);
+    if (project) {
+        int rows = (int)(32768 / ((size_t)(nb + s) * sizeof(cplx<T>)));
+        if (rows > vb) rows = vb;
+        if (rows < 1) rows = 1;
+        const size_t smem = (size_t)rows * (nb + s) * sizeof(cplx<T>);
+        block_project_kernel<T><<<grid, kLaThreads, smem, stream>>>((const cplx<T> *)Bas, (const cplx<T> *)in, (cplx<T> *)out, Vc, vb, nb, s, rows);
+    } else {
+        int rows = 32;
+        if (rows > vb) rows = vb;
+        const size_t smem = ((size_t)nb * s + (size_t)rows * (nb + 1)) * sizeof(cplx<T>);
+        auto kern = block_promote_kernel<T>;
+        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152)));
+        kern<<<grid, kLaThreads, smem, stream>>>((const cplx<T> *)Bas, (const cplx<T> *)in, (cplx<T> *)out, Vc, vb, nb, s, rows);
+    }
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+extern "C" int coarse_block_project(const void *Basis_dev, const void *F_dev, void *C_dev, int64_t Vc, int32_t vblock, int32_t nbasis, int32_t nrhs,
+                                    int32_t dtype, void *stream)
+{
+    CMRHS_STEP(transfer_check(Basis_dev, F_dev, C_dev, Vc, vblock, nbasis, nrhs, dtype));
+    return dtype == COARSE_C64 ? transfer_launch<float>(true, Basis_dev, F_dev, C_dev, Vc, vblock, nbasis, nrhs, (cudaStream_t)stream)
+                               : transfer_launch<double>(true, Basis_dev, F_dev, C_dev, Vc, vblock, nbasis, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int coarse_block_promote(const void *Basis_dev, const void *C_dev, void *F_dev, int64_t Vc, int32_t vblock, int32_t nbasis, int32_t nrhs,
+                                    int32_t dtype, void *stream)
+{
+    CMRHS_STEP(transfer_check(Basis_dev, C_dev, F_dev, Vc, vblock, nbasis, nrhs, dtype));
+    return dtype == COARSE_C64 ? transfer_launch<float>(false, Basis_dev, C_dev, F_dev, Vc, vblock, nbasis, nrhs, (cudaStream_t)stream)
+                               : transfer_launch<double>(false, Basis_dev, C_dev, F_dev, Vc, vblock, nbasis, nrhs, (cudaStream_t)stream);
+}
+
 extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)
 {
     if (!op) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
