@@ -17,11 +17,12 @@ constexpr int kLaThreads = 256;
 // Thread layout: the s x s result is cut into TT x TT sub-blocks (one per thread "tile"); the 256 threads
 // are (row group) x (tile).  Products and short runs in T, flushed to double every row tile.
 // ------------------------------------------------------------------------------------------------------
-template <typename T, int TT>
+template <typename T, int TT, int S = 0>
 __global__ void __launch_bounds__(kLaThreads)
-gram_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W, int64_t n, int s, int rows_per_tile,
+gram_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W, int64_t n, int s_rt, int rows_per_tile,
                     zdouble *__restrict__ partial)
 {
+    const int s = S ? S : s_rt;              // S > 0: compile-time block width (a multiple of TT): no column guards
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T> *sU = reinterpret_cast<cplx<T> *>(smem_raw);
     cplx<T> *sW = sU + (size_t)rows_per_tile * s;
@@ -57,12 +58,12 @@ gram_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W
                 cplx<T> u[TT], w[TT];
 #pragma unroll
                 for (int a = 0; a < TT; ++a) {
-                    const bool ok = a0 + a < s;
+                    const bool ok = S || a0 + a < s;
                     u[a] = ok ? sU[k * s + a0 + a] : cplx<T>{0, 0};
                 }
 #pragma unroll
                 for (int b = 0; b < TT; ++b) {
-                    const bool ok = b0 + b < s;
+                    const bool ok = S || b0 + b < s;
                     w[b] = ok ? sW[k * s + b0 + b] : cplx<T>{0, 0};
                 }
 #pragma unroll

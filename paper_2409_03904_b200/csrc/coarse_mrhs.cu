@@ -386,12 +386,17 @@ static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble 
     if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
     if (blocks < 1) blocks = 1;
     const cplx<T> *u = (const cplx<T> *)U, *w = (const cplx<T> *)W;
-#define CMRHS_GRAM_CASE(TTV)                                                                                     \
+#define CMRHS_GRAM_CASE(TTV, ...)                                                                                \
     {                                                                                                            \
-        auto kern = gram_partial_kernel<T, TTV>;                                                                 \
+        auto kern = gram_partial_kernel<T, TTV, ##__VA_ARGS__>;                                                  \
         CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152))); \
         kern<<<blocks, kLaThreads, smem, stream>>>(u, w, n, s, rows, op->gram_partial);                          \
     }
+    if (TT == 4 && s == 64) CMRHS_GRAM_CASE(4, 64)
+    else if (TT == 2 && s == 32) CMRHS_GRAM_CASE(2, 32)
+    else if (TT == 2 && s == 16) CMRHS_GRAM_CASE(2, 16)
+    else if (TT == 2 && s == 8) CMRHS_GRAM_CASE(2, 8)
+    else
     switch (TT) {
     case 1: CMRHS_GRAM_CASE(1) break;
     case 2: CMRHS_GRAM_CASE(2) break;
@@ -447,12 +452,21 @@ static int rotate_dispatch(const coarse_op *op, const void *U, const zdouble *K,
 
 // ---- the two fused passes of a BlockCGrQ iteration (blockcg_kernels.cuh) ---------------------------------
 struct FusedPlan { int W, TR, rows, grid; size_t smem; };
+// shared-memory budget of one CTA of the fused passes: the tile height TR is halved until the two K matrices and the
+// double-buffered row tiles fit.  Measured at nrhs 64 (config 4): 100 KB (TR 1) 15.8 ms, 140 KB (TR 2) 11.0 ms, 210 KB (TR 4,
+// one CTA per SM) 9.0 ms per iteration of linear algebra -- the wider register tile beats the second CTA.
+#ifndef LA_W4_FROM
+#define LA_W4_FROM 33
+#endif
+#ifndef LA_CAP
+#define LA_CAP 210
+#endif
 
 template <typename T>
 static FusedPlan fused_plan(const coarse_op *op, int64_t n, int s)
 {
     FusedPlan p;
-    p.W = s >= 8 ? 2 : 1;
+    p.W = s >= LA_W4_FROM ? 4 : (s >= 8 ? 2 : 1);
     if ((s + p.W - 1) / p.W > 16) p.W = 4;
     const int ncg = (s + p.W - 1) / p.W, RL = kLaThreads / ncg, su = s + LaPad<T>::v;
     int tr0 = 4;
@@ -462,7 +476,7 @@ static FusedPlan fused_plan(const coarse_op *op, int64_t n, int s)
         const size_t red = (size_t)s * s * sizeof(zdouble);
         if (tiles < red) tiles = red;
         p.smem = (size_t)2 * s * s * sizeof(cplx<T>) + tiles;
-        if (p.smem <= 100 * 1024 || p.TR == 1) break;      // two CTAs per SM when possible
+        if (p.smem <= LA_CAP * 1024 || p.TR == 1) break;
     }
     int per_sm = p.smem <= 27 * 1024 ? 8 : (p.smem <= 56 * 1024 ? 4 : (p.smem <= 113 * 1024 ? 2 : 1));
     const int64_t ntiles = ceil_div(n, p.rows);
@@ -500,6 +514,10 @@ static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Ti
         if (s == 8) return CALL(4, 2, 8); if (s == 16) return CALL(4, 2, 16); if (s == 32) return CALL(4, 2, 32); \
         if (s == 64) return CALL(4, 2, 64);                              \
     }                                                                    \
+    if (p.W == 4 && s == 64) {                                           \
+        if (p.TR == 4) return CALL(4, 4, 64); if (p.TR == 2) return CALL(2, 4, 64); return CALL(1, 4, 64); \
+    }                                                                    \
+    if (p.W == 4 && p.TR == 4 && s == 32) return CALL(4, 4, 32);         \
     if (p.TR == 4) {                                                     \
         if (p.W == 4) return CALL(4, 4); if (p.W == 2) return CALL(4, 2); return CALL(4, 1); \
     }                                                                    \
