@@ -234,6 +234,15 @@ int coarse_block_promote(const void *Basis_dev, const void *C_dev, void *F_dev, 
 int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
                         int32_t maxiter, block_cg_result *res, void *stream);
 
+/* The same two solves with options.  COARSE_SOLVE_ZERO_GUESS: "X arbitrary" taken as X_0 = 0 -- X is an output
+ * only (its contents on entry are ignored; the host variant does not copy it to the device), R_0 = B and the application of
+ * the operator to X_0 is skipped.  Unknown flag bits: COARSE_INVALID_ARG. */
+enum { COARSE_SOLVE_ZERO_GUESS = 1u << 0 };
+int block_cg_solve_ex(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter, uint32_t flags,
+                      block_cg_result *res, void *stream);
+int block_cg_solve_host_ex(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol, int32_t maxiter,
+                           uint32_t flags, block_cg_result *res, void *stream);
+
 /*
  * The block-CG building blocks, exported so that each can be checked against the oracle on its own.
  * n = number of rows (V*nbasis), s = nrhs (1..64); blocks are [n][s] in `dtype`; s x s matrices are

@@ -18,6 +18,7 @@ C64, C128 = 0, 1
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY, NOT_CONVERGED, BREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 FLAG_FORCE_GENERIC, FLAG_NO_TENSOR, FLAG_TENSOR_ONLY, FLAG_TF32, FLAG_UNFUSED_LINALG = 1, 2, 4, 8, 16
 MAX_NRHS, MAX_HISTORY = 64, 256
+SOLVE_ZERO_GUESS = 1
 
 EXPORTS = [
     "coarse_op_create", "coarse_op_destroy", "coarse_op_apply", "coarse_op_apply_host", "block_cg_solve",
@@ -25,6 +26,7 @@ EXPORTS = [
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
     "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve", "stacked_cg_solve", "coarse_block_project", "coarse_block_promote",
+    "block_cg_solve_ex", "block_cg_solve_host_ex",
 ]
 
 
@@ -87,6 +89,8 @@ def lib():
             "coarse_deflate": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, vp, i32, vp]),
             "coarse_block_project": (C.c_int, [vp, vp, vp, i64, i32, i32, i32, i32, vp]),
             "coarse_block_promote": (C.c_int, [vp, vp, vp, i64, i32, i32, i32, i32, vp]),
+            "block_cg_solve_ex": (C.c_int, [vp, vp, vp, i32, dbl, i32, u32, C.POINTER(BlockCGResult), vp]),
+            "block_cg_solve_host_ex": (C.c_int, [vp, vp, vp, i32, dbl, i32, u32, C.POINTER(BlockCGResult), vp]),
             "stacked_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(BlockCGResult), vp]),
             "pblock_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(CoarsePrecond), C.POINTER(BlockCGResult), vp]),
             "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
@@ -232,15 +236,17 @@ class CoarseOperator:
                     rel_res_recursive=[res.rel_res_recursive[r] for r in range(s)],
                     rel_res_true=[res.rel_res_true[r] for r in range(s)])
 
-    def block_cg(self, B: torch.Tensor, X: torch.Tensor | None = None, tol: float = 1e-6, maxiter: int = 1000, stream=None):
-        """block_cg_solve: BlockCGrQ (Fig. 2 left).  X in: X0 (zeros if None), out: solution."""
+    def block_cg(self, B: torch.Tensor, X: torch.Tensor | None = None, tol: float = 1e-6, maxiter: int = 1000, stream=None,
+                 zero_guess: bool = False):
+        """block_cg_solve(_ex): BlockCGrQ (Fig. 2 left, PAPER.md:132-153).  X in: X0 (zeros if None), out: solution;
+        zero_guess: X is an output only (X_0 = 0: R_0 = B, one application of the operator less)."""
         s = self._block_ok(B)
         if X is None:
-            X = torch.zeros_like(B)
+            X = torch.empty_like(B) if zero_guess else torch.zeros_like(B)
         self._block_ok(X)
         res = BlockCGResult()
-        _check(lib().block_cg_solve(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), C.byref(res), _stream(stream)),
-               allow=(NOT_CONVERGED, BREAKDOWN))
+        _check(lib().block_cg_solve_ex(self._h, _dev(B), _dev(X), s, float(tol), int(maxiter), SOLVE_ZERO_GUESS if zero_guess else 0,
+                                       C.byref(res), _stream(stream)), allow=(NOT_CONVERGED, BREAKDOWN))
         return self._result(res, s, X)
 
     def stacked_cg(self, B: torch.Tensor, X: torch.Tensor | None = None, tol: float = 1e-6, maxiter: int = 1000, stream=None):
@@ -291,14 +297,16 @@ class CoarseOperator:
         B, X = self._bcg_keep
         return self._result(res, int(B.shape[2]), X)
 
-    def block_cg_host(self, B: torch.Tensor, X: torch.Tensor, tol: float = 1e-6, maxiter: int = 1000, stream=None):
+    def block_cg_host(self, B: torch.Tensor, X: torch.Tensor, tol: float = 1e-6, maxiter: int = 1000, stream=None, zero_guess: bool = False):
+        """block_cg_solve_host(_ex): B, X are (pinned) HOST tensors; zero_guess: X is an output only (X_0 = 0, no copy in)."""
         s = self._block_ok(B)
         self._block_ok(X)
         if B.is_cuda or X.is_cuda:
             raise ValueError("block_cg_host takes host tensors")
         res = BlockCGResult()
-        _check(lib().block_cg_solve_host(self._h, B.data_ptr(), X.data_ptr(), s, float(tol), int(maxiter), C.byref(res),
-                                         _stream(stream)), allow=(NOT_CONVERGED, BREAKDOWN))
+        _check(lib().block_cg_solve_host_ex(self._h, B.data_ptr(), X.data_ptr(), s, float(tol), int(maxiter),
+                                            SOLVE_ZERO_GUESS if zero_guess else 0, C.byref(res), _stream(stream)),
+               allow=(NOT_CONVERGED, BREAKDOWN))
         return self._result(res, s, X)
 
     # ---- block-CG building blocks (each parity-tested on its own) ----

@@ -640,7 +640,7 @@ static int fetch_scalars(const coarse_op *op, cudaStream_t stream)
 
 // The solve is split into begin / step / poll / end so that a caller (bench.py) can time exactly K iterations
 // on the device without the per-iteration host read of block_cg_solve.  State lives in the handle.
-static int bcg_begin(coarse_op *op, const void *B, void *X, int s, double tol, cudaStream_t stream)
+static int bcg_begin(coarse_op *op, const void *B, void *X, int s, double tol, cudaStream_t stream, bool zero_guess = false)
 {
     const int64_t n = op->dims.V * op->nb, total = n * s;
     const size_t blk_bytes = (size_t)total * op->esize;
@@ -651,9 +651,14 @@ static int bcg_begin(coarse_op *op, const void *B, void *X, int s, double tol, c
     CMRHS_STEP(gram_dispatch(op, B, B, w.G, n, s, stream));
     bcg_bnorm_kernel<<<1, 64, 0, stream>>>(w, s);
     CMRHS_LAUNCH_CHECK();
-    // R_0 = B - H X_0  (held in T)
-    CMRHS_STEP(apply_impl(op, X, Z, s, stream));
-    CMRHS_STEP(axpby_dispatch(op, B, Z, T, 1.0, -1.0, total, stream));
+    // R_0 = B - H X_0  (held in T); with a zero initial guess R_0 = B and the apply is skipped
+    if (zero_guess) {
+        CMRHS_CUDA(cudaMemsetAsync(X, 0, blk_bytes, stream));
+        CMRHS_CUDA(cudaMemcpyAsync(T, B, blk_bytes, cudaMemcpyDeviceToDevice, stream));
+    } else {
+        CMRHS_STEP(apply_impl(op, X, Z, s, stream));
+        CMRHS_STEP(axpby_dispatch(op, B, Z, T, 1.0, -1.0, total, stream));
+    }
     // Q_0 C_0 = R_0 by Cholesky of R^H R
     CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));
     {
@@ -725,14 +730,14 @@ static int bcg_end(coarse_op *op, block_cg_result *res, cudaStream_t stream)
 }
 
 static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double tol, int maxiter, block_cg_result *res,
-                         cudaStream_t stream)
+                         cudaStream_t stream, bool zero_guess = false)
 {
     const double *h_stop = op->hpin + 64;
     memset(res, 0, sizeof(*res));
     for (int k = 0; k < COARSE_MAX_HISTORY; ++k) res->history[k] = -1.0;
     CMRHS_CUDA(cudaStreamSynchronize(stream));
     const auto t0 = std::chrono::steady_clock::now();
-    int status = bcg_begin(op, B, X, s, tol, stream);
+    int status = bcg_begin(op, B, X, s, tol, stream, zero_guess);
     if (status != COARSE_OK && status != COARSE_NOT_CONVERGED && status != COARSE_BREAKDOWN) return status;
     res->history[0] = h_stop[0];
     if (status == COARSE_NOT_CONVERGED) {
@@ -768,20 +773,37 @@ extern "C" int block_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, i
     return block_cg_impl(op, B_dev, X_dev, nrhs, tol, maxiter, res, (cudaStream_t)stream);
 }
 
-extern "C" int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
-                                   int32_t maxiter, block_cg_result *res, void *stream_v)
+extern "C" int block_cg_solve_host_ex(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol, int32_t maxiter,
+                                      uint32_t flags, block_cg_result *res, void *stream_v)
 {
     int st = check_solve_args(op, B_host, X_host, nrhs, tol, maxiter, res);
     if (st != COARSE_OK) return st;
+    if (flags & ~(uint32_t)COARSE_SOLVE_ZERO_GUESS) { set_error("unknown solve flags 0x%x", flags); return COARSE_INVALID_ARG; }
+    const bool zero = (flags & COARSE_SOLVE_ZERO_GUESS) != 0;
     cudaStream_t stream = (cudaStream_t)stream_v;
     const size_t bytes = (size_t)op->dims.V * op->nb * nrhs * op->esize;
     CMRHS_CUDA(cudaMemcpyAsync(op->blk[4], B_host, bytes, cudaMemcpyHostToDevice, stream));
-    CMRHS_CUDA(cudaMemcpyAsync(op->blk[5], X_host, bytes, cudaMemcpyHostToDevice, stream));
-    st = block_cg_impl(op, op->blk[4], op->blk[5], nrhs, tol, maxiter, res, stream);
+    if (!zero) CMRHS_CUDA(cudaMemcpyAsync(op->blk[5], X_host, bytes, cudaMemcpyHostToDevice, stream));
+    st = block_cg_impl(op, op->blk[4], op->blk[5], nrhs, tol, maxiter, res, stream, zero);
     if (st != COARSE_OK && st != COARSE_NOT_CONVERGED) return st;
     CMRHS_CUDA(cudaMemcpyAsync(X_host, op->blk[5], bytes, cudaMemcpyDeviceToHost, stream));
     CMRHS_CUDA(cudaStreamSynchronize(stream));
     return st;
+}
+
+extern "C" int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol,
+                                   int32_t maxiter, block_cg_result *res, void *stream)
+{
+    return block_cg_solve_host_ex(op, B_host, X_host, nrhs, tol, maxiter, 0u, res, stream);
+}
+
+extern "C" int block_cg_solve_ex(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter, uint32_t flags,
+                                 block_cg_result *res, void *stream)
+{
+    int st = check_solve_args(op, B_dev, X_dev, nrhs, tol, maxiter, res);
+    if (st != COARSE_OK) return st;
+    if (flags & ~(uint32_t)COARSE_SOLVE_ZERO_GUESS) { set_error("unknown solve flags 0x%x", flags); return COARSE_INVALID_ARG; }
+    return block_cg_impl(op, B_dev, X_dev, nrhs, tol, maxiter, res, (cudaStream_t)stream, (flags & COARSE_SOLVE_ZERO_GUESS) != 0);
 }
 
 // ---- synthetic inputs (bench convenience) --------------------------------

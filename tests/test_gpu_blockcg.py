@@ -230,3 +230,27 @@ def test_fused_passes_equal_the_unfused_kernel_sequence(dims, nb, s, dtype, tol)
     k = outs[0]["iterations"]
     h0, h1 = np.array(outs[0]["history"][:k + 1]), np.array(outs[1]["history"][:k + 1])
     assert np.allclose(h0, h1, rtol=1e-9 if dtype == "c128" else 2e-2)
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_zero_guess_option_equals_an_explicit_zero_start(dtype):
+    # COARSE_SOLVE_ZERO_GUESS: X is an output only, R_0 = B, one apply less -- same iterates as X_0 = 0 passed explicitly
+    dims, nb, s = (4, 4, 4, 4), 32, 16
+    tol = 1e-10 if dtype == "c128" else 1e-6
+    A, c, _, B = host_case(dims, nb, s, seed=55, factor=1.03)
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), s)
+    Bd = to_dev(B, dtype)
+    ref = op.block_cg(Bd, torch.zeros_like(Bd), tol=tol, maxiter=100)
+    l0 = cm.launch_count()
+    garbage = torch.full_like(Bd, float("nan"))
+    out = op.block_cg(Bd, garbage, tol=tol, maxiter=100, zero_guess=True)
+    assert out["status"] == ref["status"] == 0 and out["iterations"] == ref["iterations"]
+    assert torch.equal(out["X"], ref["X"])
+    assert np.array_equal(out["history"], ref["history"])
+    # host entry point: X_host is not read
+    Bh, Xh = Bd.cpu().pin_memory(), torch.full_like(Bd, float("nan")).cpu().pin_memory()
+    outh = op.block_cg_host(Bh, Xh, tol=tol, maxiter=100, zero_guess=True)
+    assert outh["iterations"] == ref["iterations"] and torch.equal(Xh, ref["X"].cpu())
+    with pytest.raises(cm.binding.CoarseError):
+        cm.binding._check(cm.lib().block_cg_solve_ex(op._h, Bd.data_ptr(), garbage.data_ptr(), s, tol, 10, 2, None, None))
+    op.close()
