@@ -92,7 +92,7 @@ int coarse_op_destroy(coarse_op_t *op);
 /*
  * coarse_op_apply -- Y(x) = sum_{p=0}^{80} A^p(x) . X(x + delta_p) for all sites, one launch
  * (Eq. 19 summed over the stencil; the paper issues 81 batched GEMMs).
- *   X_dev, Y_dev : device, [V][nbasis][nrhs], dtype of the operator; Y must not alias X
+ *   X_dev, Y_dev : device, [V][nbasis][nrhs], dtype of the operator, 16-byte aligned; Y must not alias X
  *   nrhs         : 1..nrhs_max
  * Asynchronous on `stream`; allocates nothing.  complex64, nbasis 32, nrhs 4 or a multiple of 8 (the split-FP16 tensor
  * kernel): two short pre-pass kernels first write the scaled, split copy of X into a scratch block OWNED BY THE HANDLE, so
