@@ -344,10 +344,15 @@ def run_ours(args, cfg):
             t_ms = ev[0].elapsed_time(ev[1]) / reps
             r = roofline_tflops(V, nb, sv, dtype, peaks, op.kernel_name(sv), sustained=True)
             tf = apply_flops(V, nb, sv) / (t_ms * 1e-3) / 1e12
+            # block-CG solve seconds at this Nrhs (the metric's second half): device-resident, X_0 = 0, to the config's tolerance
+            Bs = cm.fill_block(dims, nb, sv, tdt, seed, synth.TAG_B)
+            sol_s = op.block_cg(Bs, tol=cfg["tol"], maxiter=100, zero_guess=True)
             sweep.append(dict(nrhs=sv, ms=t_ms, tflops=tf, hbm_gbs=apply_bytes(V, nb, sv, esize) / (t_ms * 1e-3) / 1e9,
                               roof_tflops=r["roof_tflops"], bound=r["bound"], frac=tf / r["roof_tflops"],
-                              kernel=op.kernel_name(sv)))
-            del Xs, Ys
+                              kernel=op.kernel_name(sv),
+                              block_cg=dict(seconds=sol_s["seconds"], iterations=sol_s["iterations"], status=sol_s["status"],
+                                            max_true_rel_res=max(sol_s["rel_res_true"]))))
+            del Xs, Ys, Bs, sol_s
 
     # ---- block-CG solve seconds (the metric's second half), device-resident -----------------------------------
     Xs = torch.zeros_like(B)

@@ -209,7 +209,10 @@ def test_begin_step_end_equals_solve(cfg1):
     ((3, 3, 3, 5), 24, 8, "c128", 1e-10),
     ((3, 3, 2, 4), 13, 5, "c128", 1e-10),       # odd s: 8-byte cp.async chunks do not apply to complex128; ragged column groups
     ((3, 3, 2, 4), 16, 7, "c64", 1e-6),         # odd s in complex64: 8-byte chunks, ragged column groups
-    ((3, 3, 3, 3), 32, 64, "c64", 1e-6),        # widest block
+    ((3, 3, 3, 3), 32, 64, "c64", 1e-6),        # widest block: 4 x 4 register tiles, width-specialised kernels
+    ((3, 3, 3, 3), 32, 48, "c64", 1e-6),        # 4 x 4 tiles with a run-time width
+    ((3, 3, 3, 3), 24, 40, "c64", 1e-6),        # same, TF32 stencil kernel underneath
+    ((3, 3, 3, 3), 8, 64, "c128", 1e-10),       # widest block in complex128 (tile height limited by shared memory)
     ((3, 3, 3, 3), 8, 33, "c128", 1e-10),       # s > 32 in complex128
 ])
 def test_fused_passes_equal_the_unfused_kernel_sequence(dims, nb, s, dtype, tol):
