@@ -377,8 +377,15 @@ bcg_fused1_kernel(const cplx<T> *__restrict__ D, const cplx<T> *__restrict__ Z, 
 template <typename T, int TR, int W, int S = 0>
 __global__ void __launch_bounds__(kLaThreads)
 bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, const zdouble *__restrict__ K3, const zdouble *__restrict__ K4,
-                  int64_t n, int s_rt)
+                  int64_t n, int s_rt, uint32_t *__restrict__ colmax)
 {
+    // colmax (may be NULL; zeroed by the caller): per-column max |Re|, |Im| of the new D as float bit patterns -- the first
+    // pre-pass of the FP16-split stencil kernel, which reads this D next, fused into its producer (order independent: atomicMax)
+    __shared__ uint32_t scm[COARSE_MAX_NRHS];
+    uint32_t cm[W];
+#pragma unroll
+    for (int c = 0; c < W; ++c) cm[c] = 0u;
+    if (threadIdx.x < COARSE_MAX_NRHS) scm[threadIdx.x] = 0u;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int s = S ? S : s_rt;
     const int su = s + LaPad<T>::v;
@@ -425,12 +432,25 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
                             v.re = q[tt][c].re + d[tt][c].re;
                             v.im = q[tt][c].im + d[tt][c].im;
                             D[e] = v;                                            // D = Q + D S^H (this CTA staged its rows of D first)
+                            if (sizeof(T) == 4) {
+                                const uint32_t a = __float_as_uint((float)v.re) & 0x7FFFFFFFu, b = __float_as_uint((float)v.im) & 0x7FFFFFFFu;
+                                if (a <= 0x7F800000u) cm[c] = max(cm[c], a);
+                                if (b <= 0x7F800000u) cm[c] = max(cm[c], b);
+                            }
                         }
             }
         }
         __syncthreads();                                   // this stage's buffers may be restaged by the next iteration
     }
     cp_async_wait<0>();
+    if (sizeof(T) == 4 && colmax != nullptr) {
+        if (rl < RL)
+#pragma unroll
+            for (int c = 0; c < W; ++c)
+                if ((S || c0 + c < s) && cm[c]) atomicMax(&scm[c0 + c], cm[c]);
+        __syncthreads();
+        if (threadIdx.x < s && scm[threadIdx.x]) atomicMax(&colmax[threadIdx.x], scm[threadIdx.x]);
+    }
 }
 
 // Chebyshev recurrence, one fused elementwise pass:

@@ -83,6 +83,7 @@ struct coarse_op {
     bool h16_ok = false;
     float inv_sA = 1.0f;         // 1 / (power-of-two operator scale of Ah)
     unsigned char *Xh = nullptr; // [V] split operand tiles of the current X (pre-pass of the FP16-split kernel)
+    bool d_colmax_ready = false; // inside a begin/step/end solve: op->amax holds the column maxima of D (written by fused pass 2)
     uint32_t *amax = nullptr;    // [64] per-column max |x| bit patterns (pre-pass of the FP16-split kernel) + [64] scratch
     int32_t *nbr = nullptr;      // [V][81]
     void *pblk[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};           // q, Q, D, z, Z of pblock_cg_solve (allocated on first use)
@@ -302,23 +303,27 @@ extern "C" const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs
     return v ? v->name : (op->dtype == COARSE_C64 ? "stencil_generic<float>" : "stencil_generic<double>");
 }
 
-static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream);
+static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream, bool have_colmax);
 
-static int apply_impl(const coarse_op *op_c, const void *X, void *Y, int nrhs, cudaStream_t stream)
+// have_colmax: the caller guarantees that op->amax holds the column maxima of X (only bcg_step, for D after fused pass 2)
+static int apply_impl(const coarse_op *op_c, const void *X, void *Y, int nrhs, cudaStream_t stream, bool have_colmax = false)
 {
     coarse_op *op = const_cast<coarse_op *>(op_c);
-    if (!op->prof_on || op->prof_n >= 64) return apply_launch(op, X, Y, nrhs, stream);
+    if (!op->prof_on || op->prof_n >= 64) return apply_launch(op, X, Y, nrhs, stream, have_colmax);
     const int k = op->prof_n;
     CMRHS_CUDA(cudaEventRecord(op->prof_ev[2 * k], stream));
-    int st = apply_launch(op, X, Y, nrhs, stream);
+    int st = apply_launch(op, X, Y, nrhs, stream, have_colmax);
     CMRHS_CUDA(cudaEventRecord(op->prof_ev[2 * k + 1], stream));
     op->prof_n = k + 1;
     return st;
 }
 
-static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream)
+static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, cudaStream_t stream, bool have_colmax)
 {
-    if (use_h16(op, nrhs)) return launch_stencil_h16(op->Ah, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream);
+    if (use_h16(op, nrhs)) {
+        if (!have_colmax) const_cast<coarse_op *>(op)->d_colmax_ready = false;     // this apply's own pre-pass overwrites op->amax
+        return launch_stencil_h16(op->Ah, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream, have_colmax);
+    }
     if (use_tc(op, nrhs)) {
         switch (op->nb) {
         case 8: return launch_stencil_tc<8>(op->Ak, op->dims, X, Y, nrhs, op->num_sms, stream);
@@ -503,7 +508,11 @@ static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Ti
 {
     auto kern = bcg_fused2_kernel<T, TR, W, S>;
     CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
-    kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)Tin, (cplx<T> *)D, (cplx<T> *)Qout, K3, K4, n, s);
+    // the next reader of D is the stencil kernel: if that is the FP16-split one, its column-maxima pre-pass is done here
+    uint32_t *colmax = (sizeof(T) == 4 && op->h16_ok && h16_supported(op->nb, s)) ? op->amax : nullptr;
+    if (colmax) CMRHS_CUDA(cudaMemsetAsync(colmax, 0, 64 * sizeof(uint32_t), stream));
+    kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)Tin, (cplx<T> *)D, (cplx<T> *)Qout, K3, K4, n, s, colmax);
+    const_cast<coarse_op *>(op)->d_colmax_ready = colmax != nullptr;
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
@@ -647,6 +656,7 @@ static int bcg_begin(coarse_op *op, const void *B, void *X, int s, double tol, c
     void *Q = op->blk[0], *D = op->blk[1], *Z = op->blk[2], *T = op->blk[3];
     BcgSmall w = small_view(op);
     op->bcg_B = B; op->bcg_X = X; op->bcg_s = s; op->bcg_its = 0; op->bcg_active = false;
+    op->d_colmax_ready = false;
     // ||B[:,r]||
     CMRHS_STEP(gram_dispatch(op, B, B, w.G, n, s, stream));
     bcg_bnorm_kernel<<<1, 64, 0, stream>>>(w, s);
@@ -684,7 +694,8 @@ static int bcg_step(coarse_op *op, cudaStream_t stream)
     const int64_t n = op->dims.V * op->nb;
     void *Q = op->blk[0], *D = op->blk[1], *Z = op->blk[2], *T = op->blk[3], *X = op->bcg_X;
     BcgSmall w = small_view(op);
-    CMRHS_STEP(apply_impl(op, D, Z, s, stream));                                   // Z_k = H D_k
+    CMRHS_STEP(apply_impl(op, D, Z, s, stream, op->d_colmax_ready));               // Z_k = H D_k
+    op->d_colmax_ready = false;
     CMRHS_STEP(gram_dispatch(op, D, Z, w.G, n, s, stream));                        // D^H Z
     CMRHS_STEP(small_launch(bcg_step1_kernel, op, s, 3, stream));                  // M, K1 = M C, K2 = -M
     if (op->flags & COARSE_FLAG_UNFUSED_LINALG) {

@@ -533,7 +533,7 @@ __global__ void __launch_bounds__(256) xsplit_kernel(const float *__restrict__ X
 inline int h16_xo_bytes(int s) { return (4 * s <= 64) ? 4096 : 2 * ((2 * s + 63) / 64) * 4096; }
 
 inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *amax_dev, unsigned char *Xh, const LatticeDims &d, const void *X,
-                              void *Y, int s, int num_sms, cudaStream_t stream)
+                              void *Y, int s, int num_sms, cudaStream_t stream, bool have_colmax = false)
 {
     if ((reinterpret_cast<uintptr_t>(X) & 15u) || (reinterpret_cast<uintptr_t>(Y) & 15u)) {
         set_error("tensor path: X and Y must be 16-byte aligned");
@@ -576,12 +576,15 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     const size_t smem = (size_t)fixed + (size_t)P.sa * kHTile + (size_t)P.sxo * P.xo_bytes;
 
     // pre-passes over X: per-column max |x| (-> power-of-two column scales), then the split operand tiles
-    CMRHS_CUDA(cudaMemsetAsync(amax_dev, 0, 64 * sizeof(uint32_t), stream));
-    const int64_t n = d.V * 32;
-    const int rpp = 256 / s;
-    const int cgrid = (int)(ceil_div(n, rpp) < (int64_t)num_sms * 8 ? ceil_div(n, rpp) : (int64_t)num_sms * 8);
-    colmax_kernel<<<cgrid, 256, 0, stream>>>(static_cast<const float2 *>(X), n, s, amax_dev);
-    CMRHS_LAUNCH_CHECK();
+    // (have_colmax: the kernel that produced X -- pass 2 of a block-CG iteration -- has already left them in amax_dev)
+    if (!have_colmax) {
+        CMRHS_CUDA(cudaMemsetAsync(amax_dev, 0, 64 * sizeof(uint32_t), stream));
+        const int64_t n = d.V * 32;
+        const int rpp = 256 / s;
+        const int cgrid = (int)(ceil_div(n, rpp) < (int64_t)num_sms * 8 ? ceil_div(n, rpp) : (int64_t)num_sms * 8);
+        colmax_kernel<<<cgrid, 256, 0, stream>>>(static_cast<const float2 *>(X), n, s, amax_dev);
+        CMRHS_LAUNCH_CHECK();
+    }
     const int xgrid = (int)(d.V < (int64_t)num_sms * 8 ? d.V : (int64_t)num_sms * 8);
     xsplit_kernel<<<xgrid, 256, 0, stream>>>(static_cast<const float *>(X), Xh, amax_dev, d.V, s, P.LO, P.xo_bytes);
     CMRHS_LAUNCH_CHECK();

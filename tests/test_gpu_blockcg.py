@@ -257,3 +257,22 @@ def test_zero_guess_option_equals_an_explicit_zero_start(dtype):
     with pytest.raises(cm.binding.CoarseError):
         cm.binding._check(cm.lib().block_cg_solve_ex(op._h, Bd.data_ptr(), garbage.data_ptr(), s, tol, 10, 2, None, None))
     op.close()
+
+
+def test_steps_interleaved_with_other_applies_on_the_same_handle():
+    # pass 2 of an iteration leaves the column maxima of D for the next stencil launch (FP16-split kernel); an unrelated apply
+    # on the same handle in between must not corrupt them
+    dims, nb, s = (4, 4, 4, 4), 32, 16
+    A, c, X, B = host_case(dims, nb, s, seed=61, factor=1.03)
+    ref = oracle.block_cg(dims, A, B, tol=1e-6, maxiter=100)
+    op = cm.CoarseOperator(dims, to_dev(A, "c64"), s)
+    Bd, Xd = to_dev(B, "c64"), to_dev(np.zeros_like(B), "c64")
+    big = to_dev(1e6 * X, "c64")
+    st, r0 = op.block_cg_begin(Bd, Xd, tol=1e-6)
+    for k in range(ref["iterations"]):
+        op.block_cg_step(1)
+        Y = op.apply(big)                      # very different column maxima
+    out = op.block_cg_end()
+    op.close()
+    assert out["status"] == 0 and max(out["rel_res_true"]) <= 1e-6 + 3e-7
+    assert rel_err_cols(to_np(Xd), ref["X"]) <= 1e-5
