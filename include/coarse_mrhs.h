@@ -236,7 +236,9 @@ int block_cg_solve_host(coarse_op_t *op, const void *B_host, void *X_host, int32
 
 /* The same two solves with options.  COARSE_SOLVE_ZERO_GUESS: "X arbitrary" taken as X_0 = 0 -- X is an output
  * only (its contents on entry are ignored; the host variant does not copy it to the device), R_0 = B and the application of
- * the operator to X_0 is skipped.  Unknown flag bits: COARSE_INVALID_ARG. */
+ * the operator to X_0 is skipped.  Unknown flag bits: COARSE_INVALID_ARG.
+ * The host variants start the device->host copy of the solution as soon as the iteration has stopped, on a stream of the
+ * handle's own, so that it overlaps the extra apply of the true residual; they return after both have finished. */
 enum { COARSE_SOLVE_ZERO_GUESS = 1u << 0 };
 int block_cg_solve_ex(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter, uint32_t flags,
                       block_cg_result *res, void *stream);

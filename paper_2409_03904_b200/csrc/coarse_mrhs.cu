@@ -83,6 +83,8 @@ struct coarse_op {
     bool h16_ok = false;
     float inv_sA = 1.0f;         // 1 / (power-of-two operator scale of Ah)
     unsigned char *Xh = nullptr; // [V] split operand tiles of the current X (pre-pass of the FP16-split kernel)
+    cudaStream_t copy_stream = nullptr;   // device->host copy of the solution overlapping the true-residual apply (block_cg_solve_host*)
+    cudaEvent_t copy_event = nullptr;
     bool d_colmax_ready = false; // inside a begin/step/end solve: op->amax holds the column maxima of D (written by fused pass 2)
     uint32_t *amax = nullptr;    // [64] per-column max |x| bit patterns (pre-pass of the FP16-split kernel) + [64] scratch
     int32_t *nbr = nullptr;      // [V][81]
@@ -156,6 +158,8 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     if (!op) return COARSE_OK;
     cudaFree(op->At);
     cudaFree(op->Ak);
+    if (op->copy_stream) cudaStreamDestroy(op->copy_stream);
+    if (op->copy_event) cudaEventDestroy(op->copy_event);
     for (int b = 0; b < 5; ++b) cudaFree(op->pblk[b]);
     cudaFree(op->Ah);
     cudaFree(op->Xh);
@@ -740,8 +744,10 @@ static int bcg_end(coarse_op *op, block_cg_result *res, cudaStream_t stream)
     return COARSE_OK;
 }
 
+// X_host_out (optional): the solution is final when the loop ends, so its copy to the host is started then, on the handle's
+// copy stream, and overlaps the extra apply that evaluates the true residual
 static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double tol, int maxiter, block_cg_result *res,
-                         cudaStream_t stream, bool zero_guess = false)
+                         cudaStream_t stream, bool zero_guess = false, void *X_host_out = nullptr)
 {
     const double *h_stop = op->hpin + 64;
     memset(res, 0, sizeof(*res));
@@ -760,7 +766,17 @@ static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double to
             if (h_stop[0] <= tol) { status = COARSE_OK; break; }
         }
     }
-    CMRHS_STEP(bcg_end(op, res, stream));
+    if (X_host_out) {
+        if (!op->copy_stream) {
+            CMRHS_CUDA(cudaStreamCreateWithFlags(&op->copy_stream, cudaStreamNonBlocking));
+            CMRHS_CUDA(cudaEventCreateWithFlags(&op->copy_event, cudaEventDisableTiming));
+        }
+        CMRHS_CUDA(cudaEventRecord(op->copy_event, stream));
+        CMRHS_CUDA(cudaStreamWaitEvent(op->copy_stream, op->copy_event, 0));
+        CMRHS_CUDA(cudaMemcpyAsync(X_host_out, X, (size_t)op->dims.V * op->nb * s * op->esize, cudaMemcpyDeviceToHost, op->copy_stream));
+    }
+    CMRHS_STEP(bcg_end(op, res, stream));                                                  // reads X only
+    if (X_host_out) CMRHS_CUDA(cudaStreamSynchronize(op->copy_stream));
     res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
     res->status = status;
     return status;
@@ -795,9 +811,7 @@ extern "C" int block_cg_solve_host_ex(coarse_op_t *op, const void *B_host, void 
     const size_t bytes = (size_t)op->dims.V * op->nb * nrhs * op->esize;
     CMRHS_CUDA(cudaMemcpyAsync(op->blk[4], B_host, bytes, cudaMemcpyHostToDevice, stream));
     if (!zero) CMRHS_CUDA(cudaMemcpyAsync(op->blk[5], X_host, bytes, cudaMemcpyHostToDevice, stream));
-    st = block_cg_impl(op, op->blk[4], op->blk[5], nrhs, tol, maxiter, res, stream, zero);
-    if (st != COARSE_OK && st != COARSE_NOT_CONVERGED) return st;
-    CMRHS_CUDA(cudaMemcpyAsync(X_host, op->blk[5], bytes, cudaMemcpyDeviceToHost, stream));
+    st = block_cg_impl(op, op->blk[4], op->blk[5], nrhs, tol, maxiter, res, stream, zero, X_host);      // copies X back itself
     CMRHS_CUDA(cudaStreamSynchronize(stream));
     return st;
 }
