@@ -564,8 +564,8 @@ rgram_partial_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict_
 
 template <typename T>
 __global__ void __launch_bounds__(kLaThreads)
-deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict__ B, const zdouble *__restrict__ Cm, const DeflLambda lam,
-                      cplx<T> *__restrict__ QBpar, cplx<T> *__restrict__ Bperp, int64_t n, int m, int s, int rows_per_tile)
+deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *B, const zdouble *__restrict__ Cm, const DeflLambda lam,
+                      cplx<T> *__restrict__ QBpar, cplx<T> *Bperp, int64_t n, int m, int s, int rows_per_tile)      // Bperp may alias B
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T> *sC = reinterpret_cast<cplx<T> *>(smem_raw);          // [m][s]   <i|b>
@@ -909,7 +909,7 @@ struct BcgSmall {
     zdouble *K4;      // S^H
     double *bnorm;    // ||B[:,r]||  (1 where the source column is zero)
     double *relres;   // [s] recursive relative residuals
-    double *stop;     // [0] = max_r relres, [1] = status flag (0 ok, 1 breakdown)
+    double *stop;     // [0] = max_r relres, [1] = 0 ok, else where the FIRST breakdown happened: 1 initial QR, 2 D^H Z, 3 T^H T
 };
 
 // bnorm[r] = sqrt(G[r][r]) from G = B^H B
@@ -956,11 +956,17 @@ __global__ void bcg_step1_kernel(BcgSmall w, int s)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s, *m2 = m1 + s * s;
     __shared__ int flag;
-    if (threadIdx.x == 0) flag = 0;
+    if (threadIdx.x == 0) flag = (w.stop[1] != 0.0) ? 1 : 0;       // an earlier breakdown freezes the iteration
     sm_load(m0, w.G, s * s);
-    sm_cholesky_upper(m0, s, &flag);
+    if (!flag) sm_cholesky_upper(m0, s, &flag);
     __syncthreads();
-    if (flag) { if (threadIdx.x == 0) w.stop[1] = 1.0; return; }
+    if (flag) {
+        // breakdown contract (coarse_mrhs.h): the block passes already enqueued behind this kernel must leave X at the last
+        // valid iterate: K1 = K2 = 0  =>  X += 0,  T = Q
+        for (int e = threadIdx.x; e < s * s; e += blockDim.x) { w.K1[e] = {0.0, 0.0}; w.K2[e] = {0.0, 0.0}; }
+        if (threadIdx.x == 0 && w.stop[1] == 0.0) w.stop[1] = 2.0;      // 2: D^H Z not positive definite (statement 9)
+        return;
+    }
     sm_upper_inverse(m0, m1, s);
     sm_matmul(m1, m1, m0, s, 0, 1);          // m0 = M
     sm_load(m2, w.C, s * s);
@@ -975,11 +981,19 @@ __global__ void bcg_step2_kernel(BcgSmall w, int s)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     zdouble *m0 = reinterpret_cast<zdouble *>(smem_raw), *m1 = m0 + s * s, *m2 = m1 + s * s;
     __shared__ int flag;
-    if (threadIdx.x == 0) flag = 0;
+    if (threadIdx.x == 0) flag = (w.stop[1] != 0.0) ? 1 : 0;
     sm_load(m0, w.G, s * s);
-    sm_cholesky_upper(m0, s, &flag);
+    if (!flag) sm_cholesky_upper(m0, s, &flag);
     __syncthreads();
-    if (flag) { if (threadIdx.x == 0) w.stop[1] = 1.0; return; }
+    if (flag) {
+        // breakdown contract: K3 = I, K4 = 0  =>  Q = T, D = Q (well defined, X untouched); C and the residuals keep their last values
+        for (int e = threadIdx.x; e < s * s; e += blockDim.x) {
+            w.K3[e] = {(e / s == e % s) ? 1.0 : 0.0, 0.0};
+            w.K4[e] = {0.0, 0.0};
+        }
+        if (threadIdx.x == 0 && w.stop[1] == 0.0) w.stop[1] = 3.0;      // 3: T^H T not positive definite (statement 11)
+        return;
+    }
     sm_upper_inverse(m0, m1, s);
     sm_store(w.K3, m1, s * s);
     for (int e = threadIdx.x; e < s * s; e += blockDim.x) {

@@ -5,7 +5,10 @@
 #include <cstdarg>
 #include <cstring>
 #include <atomic>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 #include <cmath>
 
@@ -30,6 +33,22 @@ void set_error(const char *fmt, ...)
     va_end(ap);
 }
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+cudaError_t ensure_dyn_smem(const void *func, size_t bytes)
+{
+    if (bytes <= 48 * 1024) return cudaSuccess;                 // the default limit needs no opt-in
+    static std::mutex mu;
+    static std::map<std::pair<int, const void *>, size_t> seen;  // (device, kernel) -> bytes already granted
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t &have = seen[{dev, func}];
+    if (have >= bytes) return cudaSuccess;
+    e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) have = bytes;
+    return e;
+}
 
 // ---- tiled SIMT variants: (dtype, nbasis, nrhs) -> kernel ---------------------------------------------
 //                      T      NB TM TN GC KSPLIT STAGES WARPS
@@ -75,6 +94,7 @@ struct coarse_op {
     int nb = 0, nrhs_max = 0, dtype = 0;
     uint32_t flags = 0;
     int num_sms = 0;
+    int device = 0;              // the CUDA device the handle (its memory, its kernel attributes) belongs to
     size_t esize = 0;            // bytes per complex element
     void *At = nullptr;          // [V][81][nb(k)][nb(i)]
     float *Ak = nullptr;         // planar k-major [V][81][part][nb(k)][nb(i)] for the tensor path (complex64 only)
@@ -196,6 +216,7 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
     op->dtype = dtype;
     op->flags = flags;
     op->esize = dtype == COARSE_C64 ? sizeof(cplx<float>) : sizeof(cplx<double>);
+    op->device = dev;
     cudaError_t ce = cudaDeviceGetAttribute(&op->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (ce != cudaSuccess) { set_error("cudaDeviceGetAttribute: %s", cudaGetErrorString(ce)); delete op; return COARSE_CUDA_ERROR; }
 
@@ -349,12 +370,25 @@ static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, c
                                           op->dims.V, op->nb, nrhs, op->num_sms, stream);
 }
 
-static int check_apply_args(const coarse_op *op, const void *X, const void *Y, int nrhs)
+// the handle's device must be the current one (its buffers and kernel attributes live there)
+static int check_device(const coarse_op *op)
+{
+    int dev = -1;
+    CMRHS_CUDA(cudaGetDevice(&dev));
+    if (dev != op->device) { set_error("handle was created on device %d, current device is %d", op->device, dev); return COARSE_INVALID_ARG; }
+    return COARSE_OK;
+}
+
+// device blocks must be 16-byte aligned: bulk-TMA loads, cp.async and float4 accesses (coarse_mrhs.h)
+static bool misaligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+static int check_apply_args(const coarse_op *op, const void *X, const void *Y, int nrhs, bool device_ptrs = true)
 {
     if (!op || !X || !Y) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
     if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..nrhs_max=%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
     if (X == Y) { set_error("Y must not alias X"); return COARSE_INVALID_ARG; }
-    return COARSE_OK;
+    if (device_ptrs && (misaligned16(X) || misaligned16(Y))) { set_error("X and Y must be 16-byte aligned"); return COARSE_INVALID_ARG; }
+    return check_device(op);
 }
 
 extern "C" int coarse_op_apply(const coarse_op_t *op, const void *X_dev, void *Y_dev, int32_t nrhs, void *stream)
@@ -366,7 +400,7 @@ extern "C" int coarse_op_apply(const coarse_op_t *op, const void *X_dev, void *Y
 
 extern "C" int coarse_op_apply_host(coarse_op_t *op, const void *X_host, void *Y_host, int32_t nrhs, void *stream_v)
 {
-    int st = check_apply_args(op, X_host, Y_host, nrhs);
+    int st = check_apply_args(op, X_host, Y_host, nrhs, false);
     if (st != COARSE_OK) return st;
     cudaStream_t stream = (cudaStream_t)stream_v;
     const size_t bytes = (size_t)op->dims.V * op->nb * nrhs * op->esize;
@@ -398,7 +432,7 @@ static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble 
 #define CMRHS_GRAM_CASE(TTV, ...)                                                                                \
     {                                                                                                            \
         auto kern = gram_partial_kernel<T, TTV, ##__VA_ARGS__>;                                                  \
-        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152))); \
+        CMRHS_SMEM_ATTR(kern, smem); \
         kern<<<blocks, kLaThreads, smem, stream>>>(u, w, n, s, rows, op->gram_partial);                          \
     }
     if (TT == 4 && s == 64) CMRHS_GRAM_CASE(4, 64)
@@ -438,7 +472,7 @@ static int rotate_impl(const coarse_op *op, const void *U, const zdouble *K, con
 #define CMRHS_ROT_CASE(TCV)                                                                                      \
     {                                                                                                            \
         auto kern = rotate_kernel<T, TCV>;                                                                       \
-        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152))); \
+        CMRHS_SMEM_ATTR(kern, smem); \
         kern<<<grid, kLaThreads, smem, stream>>>((const cplx<T> *)U, K, (const cplx<T> *)Vin, (cplx<T> *)out, (T)beta, n, s, rows); \
     }
     switch (TC) {
@@ -500,7 +534,7 @@ static int fused1_launch(const coarse_op *op, const FusedPlan &p, const void *D,
                          const zdouble *K1, const zdouble *K2, int64_t n, int s, cudaStream_t stream)
 {
     auto kern = bcg_fused1_kernel<T, TR, W, S>;
-    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
+    CMRHS_SMEM_ATTR(kern, p.smem);
     kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)D, (const cplx<T> *)Z, (const cplx<T> *)Q, (cplx<T> *)X, (cplx<T> *)Tout, K1, K2,
                                                   n, s, op->gram_partial);
     CMRHS_LAUNCH_CHECK();
@@ -511,7 +545,7 @@ static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Ti
                          int64_t n, int s, cudaStream_t stream)
 {
     auto kern = bcg_fused2_kernel<T, TR, W, S>;
-    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(p.smem > 49152 ? p.smem : 49152)));
+    CMRHS_SMEM_ATTR(kern, p.smem);
     // the next reader of D is the stencil kernel: if that is the FP16-split one, its column-maxima pre-pass is done here
     uint32_t *colmax = (sizeof(T) == 4 && op->h16_ok && h16_supported(op->nb, s)) ? op->amax : nullptr;
     if (colmax) CMRHS_CUDA(cudaMemsetAsync(colmax, 0, 64 * sizeof(uint32_t), stream));
@@ -582,7 +616,7 @@ static int axpby_dispatch(const coarse_op *op, const void *U, const void *W, voi
 static int small_smem_attr(const void *kern, int s, int nmat, size_t *smem)
 {
     *smem = (size_t)nmat * s * s * sizeof(zdouble);
-    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(*smem > 49152 ? *smem : 49152)));
+    CMRHS_SMEM_ATTR(kern, *smem);
     return COARSE_OK;
 }
 
@@ -761,7 +795,12 @@ static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double to
         for (int k = 0; k < maxiter; ++k) {
             CMRHS_STEP(bcg_step(op, stream));
             CMRHS_STEP(fetch_scalars(op, stream));                                         // stop scalar -> host
-            if (h_stop[1] != 0.0) { status = COARSE_BREAKDOWN; break; }
+            if (h_stop[1] != 0.0) {
+                // D^H Z failed (statement 9): the iteration did nothing (the s x s kernels froze X, blockcg_kernels.cuh): it does not count
+                if (h_stop[1] == 2.0) op->bcg_its -= 1;
+                status = COARSE_BREAKDOWN;
+                break;
+            }
             if (op->bcg_its < COARSE_MAX_HISTORY) res->history[op->bcg_its] = h_stop[0];
             if (h_stop[0] <= tol) { status = COARSE_OK; break; }
         }
@@ -783,13 +822,15 @@ static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double to
 }
 
 static int check_solve_args(const coarse_op *op, const void *B, const void *X, int nrhs, double tol, int maxiter,
-                            const block_cg_result *res)
+                            const block_cg_result *res, bool device_ptrs = true)
 {
     if (!op || !B || !X || !res) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
     if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..nrhs_max=%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
     if (!(tol > 0.0) || maxiter < 0) { set_error("tol must be > 0 and maxiter >= 0"); return COARSE_INVALID_ARG; }
     if (B == X) { set_error("X must not alias B"); return COARSE_INVALID_ARG; }
-    return COARSE_OK;
+    if (device_ptrs && (misaligned16(B) || misaligned16(X))) { set_error("B and X must be 16-byte aligned"); return COARSE_INVALID_ARG; }
+    if (op->bcg_active) { set_error("a block_cg_begin/step/end solve is active on this handle"); return COARSE_INVALID_ARG; }
+    return check_device(op);
 }
 
 extern "C" int block_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nrhs, double tol, int32_t maxiter,
@@ -803,7 +844,7 @@ extern "C" int block_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, i
 extern "C" int block_cg_solve_host_ex(coarse_op_t *op, const void *B_host, void *X_host, int32_t nrhs, double tol, int32_t maxiter,
                                       uint32_t flags, block_cg_result *res, void *stream_v)
 {
-    int st = check_solve_args(op, B_host, X_host, nrhs, tol, maxiter, res);
+    int st = check_solve_args(op, B_host, X_host, nrhs, tol, maxiter, res, false);
     if (st != COARSE_OK) return st;
     if (flags & ~(uint32_t)COARSE_SOLVE_ZERO_GUESS) { set_error("unknown solve flags 0x%x", flags); return COARSE_INVALID_ARG; }
     const bool zero = (flags & COARSE_SOLVE_ZERO_GUESS) != 0;
@@ -897,6 +938,7 @@ extern "C" int block_cg_begin(coarse_op_t *op, const void *B_dev, void *X_dev, i
                               void *stream)
 {
     block_cg_result dummy;
+    if (op) op->bcg_active = false;                      // a new begin abandons an unfinished begin/step/end solve
     int st = check_solve_args(op, B_dev, X_dev, nrhs, tol, 0, &dummy);
     if (st != COARSE_OK) return st;
     st = bcg_begin(op, B_dev, X_dev, nrhs, tol, (cudaStream_t)stream);
@@ -1026,7 +1068,7 @@ static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, in
     const int rows2 = 64;
     const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);
     auto kern = deflate_update_kernel<T>;
-    CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem2 > 49152 ? smem2 : 49152)));
+    CMRHS_SMEM_ATTR(kern, smem2);
     const int64_t ntiles = ceil_div(n, rows2);
     const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
     kern<<<grid, kLaThreads, smem2, stream>>>((const cplx<T> *)Vev, (const cplx<T> *)B, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, rows2);
@@ -1279,7 +1321,7 @@ static int transfer_launch(bool project, const void *Bas, const void *in, void *
         if (rows > vb) rows = vb;
         const size_t smem = ((size_t)nb * s + (size_t)rows * (nb + 1)) * sizeof(cplx<T>);
         auto kern = block_promote_kernel<T>;
-        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 49152 ? smem : 49152)));
+        CMRHS_SMEM_ATTR(kern, smem);
         kern<<<grid, kLaThreads, smem, stream>>>((const cplx<T> *)Bas, (const cplx<T> *)in, (cplx<T> *)out, Vc, vb, nb, s, rows);
     }
     CMRHS_LAUNCH_CHECK();

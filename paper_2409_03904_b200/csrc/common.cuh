@@ -22,6 +22,10 @@ __host__ __device__ __forceinline__ int stencil_point_in_order(int q) { return q
 void set_error(const char *fmt, ...);
 extern thread_local char g_err[512];
 void count_launch(int n = 1);
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: remembered per (device, kernel), set only when it has to grow
+// (thread-safe; no driver call on the launch path once a kernel has been seen on the current device)
+cudaError_t ensure_dyn_smem(const void *func, size_t bytes);
+#define CMRHS_SMEM_ATTR(kern, bytes) CMRHS_CUDA(cmrhs::ensure_dyn_smem(reinterpret_cast<const void *>(kern), (size_t)(bytes)))
 
 #define CMRHS_CUDA(expr)                                                                         \
     do {                                                                                         \

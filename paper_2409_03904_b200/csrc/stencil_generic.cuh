@@ -69,7 +69,7 @@ int launch_stencil_generic(const cplx<T> *At, const int32_t *nbr, const cplx<T> 
 #define CMRHS_GENERIC_CASE(MO)                                                                                       \
     {                                                                                                                \
         auto kern = stencil_generic_kernel<T, MO>;                                                                   \
-        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));              \
+        CMRHS_SMEM_ATTR(kern, smem);                                                                                 \
         kern<<<grid, kGenericThreads, smem, stream>>>(At, nbr, X, Y, V, nb, s);                                      \
     }
     if (nout <= 1) CMRHS_GENERIC_CASE(1)

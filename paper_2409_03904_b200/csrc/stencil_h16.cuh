@@ -589,14 +589,10 @@ inline int launch_stencil_h16(const unsigned char *Ah, float inv_sA, uint32_t *a
     xsplit_kernel<<<xgrid, 256, 0, stream>>>(static_cast<const float *>(X), Xh, amax_dev, d.V, s, P.LO, P.xo_bytes);
     CMRHS_LAUNCH_CHECK();
 
-    static bool attr_set = false;
-    if (!attr_set) {
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
-        CMRHS_CUDA(cudaFuncSetAttribute(stencil_h16_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
-        attr_set = true;
-    }
+    if (P.tr) CMRHS_SMEM_ATTR((stencil_h16_kernel<2, true>), 113 * 1024);
+    else if (cps == 3) CMRHS_SMEM_ATTR((stencil_h16_kernel<3, false>), 74 * 1024);
+    else if (cps == 2) CMRHS_SMEM_ATTR((stencil_h16_kernel<2, false>), 113 * 1024);
+    else CMRHS_SMEM_ATTR((stencil_h16_kernel<1, false>), 227 * 1024);
     const int slots = cps * num_sms;
     const int grid = P.ngroups < slots ? P.ngroups : slots;
     float2 *Yp = static_cast<float2 *>(Y);

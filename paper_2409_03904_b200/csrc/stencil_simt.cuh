@@ -205,11 +205,7 @@ int launch_stencil_simt(const void *At, const int32_t *nbr, const void *X, void 
 {
     using Z = cplx<typename C::real>;
     auto kern = stencil_simt_kernel<C>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-        attr_set = true;
-    }
+    CMRHS_SMEM_ATTR(kern, C::SMEM_BYTES);
     const int64_t nctas = (V + C::WARPS - 1) / C::WARPS;
     const int grid = (int)(nctas < num_sms ? nctas : num_sms);
     kern<<<grid, C::THREADS, C::SMEM_BYTES, stream>>>(static_cast<const Z *>(At), nbr, static_cast<const Z *>(X),

@@ -543,11 +543,7 @@ int launch_stencil_tc(const float *Ak, const LatticeDims &d, const void *X, void
     if (st != COARSE_OK) return st;
 
     auto kern = stencil_tc_kernel<NB>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CMRHS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
-        attr_set = true;
-    }
+    CMRHS_SMEM_ATTR(kern, 227 * 1024);
     const int grid = P.ngroups < num_sms ? P.ngroups : num_sms;
     kern<<<grid, kTcThreads, smem, stream>>>(Ak, tmX, static_cast<float2 *>(Y), P);
     CMRHS_LAUNCH_CHECK();

@@ -106,6 +106,54 @@ __device__ __forceinline__ void tmem_ld_x16(uint32_t taddr, uint32_t (&v)[16])
         : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld_x8(uint32_t taddr, uint32_t (&v)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+
+// ---- tcgen05.cp: shared memory -> tensor memory, all 128 lanes (SASS: UTCCP) ----------------------------------
+// The source is a matrix of 128 rows described by a K-major shared-memory descriptor (8-row x 16-byte core matrices:
+// stride byte offset between 8-row groups, leading byte offset between the 16-byte chunks of a row);
+// .128x256b gives every lane 32 bytes (8 TMEM columns: one K = 16 slab of binary16), .128x128b 16 bytes (4 columns).
+// Issued by one thread; ordered with the tcgen05.mma instructions the same thread issues afterwards.
+__device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t sdesc)
+{
+    asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+__device__ __forceinline__ void tmem_cp_128x128b(uint32_t taddr, uint64_t sdesc)
+{
+    asm volatile("tcgen05.cp.cta_group::1.128x128b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+
+// ---- tcgen05.mma, kind::f16, cta_group::1, D[tmem] (+)= A[tmem] . B[smem descriptor] --------------------------
+// A: 128 lanes x 16 binary16 (8 columns, two per 32-bit cell, K-major); B through a shared-memory descriptor.
+__device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// instruction descriptor, kind::f16: D = F32, A = B = F16, A K-major (tensor memory), B K-major
+__host__ __device__ constexpr uint32_t umma_idesc_f16_kk(int M, int N)
+{
+    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+// K-major shared-memory descriptor without swizzle ("interleave"): core matrices of 8 rows x 16 bytes, each 128
+// contiguous bytes; lbo = distance between the two 16-byte K chunks of a K = 16 slab, sbo = distance between 8-row groups
+__device__ __forceinline__ uint64_t umma_desc_kmajor_noswz(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) |
+           (1ull << 46);
+}
+
 // ---- tcgen05.mma, kind::tf32, cta_group::1, D[tmem] (+)= A[tmem] . B[smem descriptor] -----------------------
 // One thread issues on behalf of the CTA.  `accumulate` = 0 overwrites D.
 __device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)

@@ -46,3 +46,16 @@ def rel_err_cols(Y, Yref):
     d = (Y - Yref).reshape(-1, s)
     r = Yref.reshape(-1, s)
     return float(np.max(np.linalg.norm(d, axis=0) / np.linalg.norm(r, axis=0)))
+
+
+def stress_operator(dims, nb, seed, delta):
+    """The synthetic stencil matrices with the diagonal shift taken from the SPECTRUM instead of the loose Frobenius bound
+    ("optional stress operator"): c = (1 + delta) |lambda_min(off-diagonal part)|, lambda_min from a
+    dense eigvalsh of the brute-force matrix (small lattices only).  Returns (A complex64 float32-exact, c, lambda_min(H),
+    lambda_max(H)); kappa(H) ~ (lambda_max - lambda_min) / (delta |lambda_min|): delta 0.02 -> ~100, 0.001 -> ~2000."""
+    from inputs import synth
+    A, _ = synth.make_operator(dims, nb, seed, 0.0)
+    lam = np.linalg.eigvalsh(dense_matrix(dims, A.astype(np.complex128)))
+    c = float(np.float32((1.0 + delta) * abs(lam[0])))
+    synth.add_shift(A, c)
+    return A, c, float(lam[0] + c), float(lam[-1] + c)

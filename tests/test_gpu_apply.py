@@ -138,6 +138,21 @@ def test_errors_are_reported_not_swallowed():
     X = torch.zeros((16, nb, 4), dtype=torch.complex64, device="cuda")
     with pytest.raises(cm.CoarseError):
         op.apply(X, X)                               # aliasing
+    # blocks that are not 16-byte aligned are refused before any kernel could fault on them (every kernel variant)
+    for kind in ("c64", "c128"):
+        dt = torch.complex64 if kind == "c64" else torch.complex128
+        op2 = cm.CoarseOperator(dims, A.to(dt), 4)
+        n = 16 * nb * 4
+        odd = torch.zeros(n + 1, dtype=dt, device="cuda")[1:].view(16, nb, 4) if kind == "c64" else None
+        if odd is not None:                          # complex64 offset by one element: 8-byte aligned only
+            for args in ((odd, torch.zeros_like(X)), (X, odd)):
+                with pytest.raises(cm.CoarseError) as e:
+                    op2.apply(*args)
+                assert e.value.status == cm.binding.INVALID_ARG
+            with pytest.raises(cm.CoarseError) as e:
+                op2.block_cg(odd, torch.zeros_like(X))
+            assert e.value.status == cm.binding.INVALID_ARG
+        op2.close()
     op.close()
 
 

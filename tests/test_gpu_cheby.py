@@ -3,7 +3,7 @@
 Tolerances: the polynomial is evaluated by a three-term recurrence with order - 1 applications of the operator; rounding
 errors of the apply (1e-15 complex128, ~1.5e-7 complex64 per application) accumulate at most linearly in
 the order while the terms T_j(y(H)) B stay bounded by ||B|| (spectrum inside [lo, hi]); the result is compared norm-wise per
-column: <= 1e-12 (complex128), <= 1e-5 (complex64) -- north_star's figures -- for orders up to 32.
+column: <= 1e-12 (complex128), <= 1e-5 (complex64) -- north_star's figures -- for orders up to 120 (the paper's coarse solve).
 """
 import numpy as np
 import pytest
@@ -45,6 +45,40 @@ def test_cheby_apply_matches_oracle(dims, nb, s, dtype, order):
     X, name = _gpu(dims, A, B, dtype, lo, hi, order)
     ref = cheby_oracle.cheby_apply(dims, A, B, lo, hi, order)
     assert rel_err_cols(X, ref) <= TOL[dtype], (name, rel_err_cols(X, ref))
+
+
+@pytest.mark.parametrize("dims,nb,s,dtype", [((4, 4, 4, 4), 8, 4, "c128"), ((4, 4, 2, 2), 32, 16, "c64")])
+def test_cheby_order_120_on_an_ill_conditioned_operator(dims, nb, s, dtype):
+    # the paper's coarse solve is P^Cheby of order 120 on an eigenspan of ratio 2000 ([0.02, 40]); here: the
+    # stress operator (kappa ~ 100, no dominant diagonal), [lo, hi] = [0.9 lambda_min, 1.1 lambda_max], order 120 = 119 applications
+    from helpers import stress_operator
+    from inputs import synth
+    A, c, lmin, lmax = stress_operator(dims, nb, 123, 0.02)
+    B = synth.make_block(dims, nb, s, 123, synth.TAG_B)
+    lo, hi = 0.9 * lmin, 1.1 * lmax
+    X, name = _gpu(dims, A, B, dtype, lo, hi, 120)
+    ref = cheby_oracle.cheby_apply(dims, A, B, lo, hi, 120)
+    err = rel_err_cols(X, ref)
+    # the apply's own error on this operator (no dominant diagonal), measured here against the oracle
+    Xv = synth.make_block(dims, nb, s, 124, synth.TAG_X)
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), s)
+    e_apply = rel_err_cols(to_np(op.apply(to_dev(Xv, dtype))), oracle.apply(dims, A, Xv))
+    op.close()
+    kappa = lmax / lmin
+    print(f"cheby order 120 {dtype}: kernel={name} kappa={kappa:.0f} e_apply={e_apply:.2e} err={err:.2e}")
+    assert e_apply <= TOL[dtype]
+    # P approximates 1/x: a perturbed operator H~ = H + E, ||E|| <= e ||H||, moves P(H) B by ~ kappa e relative (d(1/x) = -dx/x^2);
+    # the tensor kernels' error is systematic (FP32 accumulator truncation), so it does not average out over the 119 applications:
+    # bar = 2 kappa e_apply with e_apply measured above (and never below the apply's own bar)
+    assert err <= max(TOL[dtype], 2.0 * kappa * e_apply), (name, err, e_apply)
+    # and the polynomial is the approximate inverse it should be: ||B - H X|| <= ||B|| / |T_n(y(0))| + rounding
+    R = B - oracle.apply(dims, A, X)
+    y0 = (hi + lo) / (hi - lo)
+    bound = 1.0 / np.cosh(120 * np.arccosh(y0))
+    rel = np.linalg.norm(R.reshape(-1, s), axis=0) / np.linalg.norm(B.reshape(-1, s), axis=0)
+    # (complex64: plus ||H (X - X_oracle)|| <= lambda_max ||X - X_oracle||, the part of the residual the perturbed operator explains)
+    dx = np.linalg.norm((X - ref).reshape(-1, s), axis=0) / np.linalg.norm(B.reshape(-1, s), axis=0)
+    assert np.all(rel <= bound + (1e-12 if dtype == "c128" else lmax * dx + 1e-7)), (rel.max(), bound)
 
 
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
@@ -101,6 +135,29 @@ def test_deflate_matches_oracle(dims, nb, s, nev, dtype):
     tol = 1e-12 if dtype == "c128" else 2e-6
     assert rel_err_cols(to_np(q).reshape(n, 1, s), q_ref.reshape(n, 1, s)) <= tol
     assert rel_err_cols(to_np(perp).reshape(n, 1, s), perp_ref.reshape(n, 1, s)) <= tol
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_deflate_in_place_Bperp_aliases_B(dtype):
+    # coarse_mrhs.h: "Bperp may alias B" -- the projection written over its own input
+    from inputs import synth
+    dims, nb, s, nev = (2, 2, 2, 2), 8, 8, 5
+    A, lam_all, Vev, lam = _eigenpairs(dims, nb, 33, nev)
+    B = synth.make_block(dims, nb, s, 33, synth.TAG_B)
+    n = B.shape[0] * B.shape[1]
+    Vq = Vev.astype(np.complex64).astype(np.complex128) if dtype == "c64" else Vev
+    q_ref, perp_ref = cheby_oracle.deflate(Vq, lam, B.reshape(n, s))
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), max(s, nev))
+    Bd, Vd = to_dev(B, dtype), to_dev(Vev, dtype)
+    q = torch.empty_like(Bd)
+    lam_c = (cm.binding.C.c_double * nev)(*[float(x) for x in lam])
+    st = cm.lib().coarse_deflate(op._h, Vd.data_ptr(), lam_c, nev, Bd.data_ptr(), q.data_ptr(), Bd.data_ptr(), s, None)
+    torch.cuda.synchronize()
+    op.close()
+    assert st == 0
+    tol = 1e-12 if dtype == "c128" else 2e-6
+    assert rel_err_cols(to_np(q).reshape(n, 1, s), q_ref.reshape(n, 1, s)) <= tol
+    assert rel_err_cols(to_np(Bd).reshape(n, 1, s), perp_ref.reshape(n, 1, s)) <= tol
 
 
 @pytest.mark.parametrize("dims,nb,s,nev,order,dtype", [((2, 2, 2, 2), 8, 4, 6, 10, "c128"), ((2, 2, 2, 3), 8, 16, 12, 8, "c64")])
