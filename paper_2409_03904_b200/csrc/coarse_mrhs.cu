@@ -36,17 +36,26 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 cudaError_t ensure_dyn_smem(const void *func, size_t bytes)
 {
-    if (bytes <= 48 * 1024) return cudaSuccess;                 // the default limit needs no opt-in
+    if (bytes <= 16 * 1024) return cudaSuccess;                 // far below the default limit even with the kernel's static part
+    struct Seen { size_t static_bytes = 0, have = 0; bool known = false; };
     static std::mutex mu;
-    static std::map<std::pair<int, const void *>, size_t> seen;  // (device, kernel) -> bytes already granted
+    static std::map<std::pair<int, const void *>, Seen> seen;    // (device, kernel) -> static bytes, dynamic bytes already granted
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     std::lock_guard<std::mutex> lock(mu);
-    size_t &have = seen[{dev, func}];
-    if (have >= bytes) return cudaSuccess;
+    Seen &k = seen[{dev, func}];
+    if (!k.known) {
+        cudaFuncAttributes fa;
+        e = cudaFuncGetAttributes(&fa, func);
+        if (e != cudaSuccess) return e;
+        k.static_bytes = fa.sharedSizeBytes;
+        k.known = true;
+    }
+    // without opt-in, static + dynamic shared memory together must fit the default 48 KB
+    if (k.have >= bytes || (k.have == 0 && k.static_bytes + bytes <= 48 * 1024)) return cudaSuccess;
     e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e == cudaSuccess) have = bytes;
+    if (e == cudaSuccess) k.have = bytes;
     return e;
 }
 

@@ -277,3 +277,26 @@ def test_steps_interleaved_with_other_applies_on_the_same_handle():
     op.close()
     assert out["status"] == 0 and max(out["rel_res_true"]) <= 1e-6 + 3e-7
     assert rel_err_cols(to_np(Xd), ref["X"]) <= 1e-5
+
+
+@pytest.mark.parametrize("s", [32, 64])
+def test_first_solve_of_a_fresh_process_at_this_width(s):
+    # Kernel attributes (dynamic shared memory opt-in) are set lazily per (device, kernel): a width whose s x s kernels sit
+    # exactly at the 48 KB default (s = 32: 3 matrices x 16 KB + the kernel's static part) must work as the FIRST launch of
+    # a process, not only after a wider solve has raised the limit (bench.py's Nrhs sweep runs 1, 4, 8, 16, 32, 64 in order).
+    import subprocess
+    import sys
+    code = (
+        "import sys, numpy as np, torch\n"
+        f"sys.path.insert(0, {repr(str(__import__('os').path.dirname(__import__('os').path.dirname(__import__('os').path.abspath(__file__)))))})\n"
+        "import paper_2409_03904_b200 as cm\n"
+        "from inputs import synth\n"
+        f"dims, nb, s = (4, 4, 2, 2), 32, {s}\n"
+        "A, c = synth.make_operator(dims, nb, 5, 1.02)\n"
+        "B = synth.make_block(dims, nb, s, 5, synth.TAG_B)\n"
+        "op = cm.CoarseOperator(dims, torch.from_numpy(A.astype(np.complex64)).cuda(), 64)\n"
+        "out = op.block_cg(torch.from_numpy(B.astype(np.complex64)).cuda(), tol=1e-6, maxiter=50)\n"
+        "assert out['status'] == 0 and max(out['rel_res_true']) <= 1.3e-6, out\n"
+        "print('ok', out['iterations'])\n")
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "ok" in r.stdout, r.stdout + r.stderr
