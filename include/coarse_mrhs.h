@@ -63,8 +63,11 @@ enum {
                                             instead of the default split-FP16 kernel (operator stored pre-split as two
                                             binary16 numbers per real: 22-23 significant bits, elements below 2^-29 of the
                                             operator's largest element lose relative precision) */
-    COARSE_FLAG_UNFUSED_LINALG = 1u << 4 /* block_cg_*: run the block rotations and Gram products of an iteration as six
+    COARSE_FLAG_UNFUSED_LINALG = 1u << 4, /* block_cg_*: run the block rotations and Gram products of an iteration as six
                                             separate kernels instead of the two fused passes (cross-check / debugging aid) */
+    COARSE_FLAG_H16X = 1u << 5           /* complex64, nbasis 32: keep the operator in the layout of the split-FP16 kernel that
+                                            holds the X operand in tensor memory (stencil_h16x: the default for nbasis 8, 16, 24)
+                                            instead of the paired-site kernel's (stencil_h16) */
 };
 
 #define COARSE_MAX_NRHS 64

@@ -36,7 +36,7 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS, "-o", str(LIB), *map(str, SOURCES)]
+    cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("CMRHS_NVCC_EXTRA", "").split(), "-o", str(LIB), *map(str, SOURCES)]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

@@ -19,6 +19,7 @@
 #include "stencil_simt.cuh"
 #include "stencil_tc.cuh"
 #include "stencil_h16.cuh"
+#include "stencil_h16x.cuh"
 
 namespace cmrhs {
 
@@ -110,6 +111,8 @@ struct coarse_op {
     bool tc_ok = false;
     unsigned char *Ah = nullptr; // pre-split FP16 tiles [V][81][hi 4 KB | lo 4 KB] for the FP16-split tensor kernel (complex64, nbasis 32)
     bool h16_ok = false;
+    unsigned char *Ax = nullptr; // pre-split FP16 tiles, K-major core-matrix image [V][81][8 nb^2 bytes] (stencil_h16x.cuh: any nbasis in {8,16,24,32})
+    bool h16x_ok = false;
     float inv_sA = 1.0f;         // 1 / (power-of-two operator scale of Ah)
     unsigned char *Xh = nullptr; // [V] split operand tiles of the current X (pre-pass of the FP16-split kernel)
     cudaStream_t copy_stream = nullptr;   // device->host copy of the solution overlapping the true-residual apply (block_cg_solve_host*)
@@ -191,6 +194,7 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     if (op->copy_event) cudaEventDestroy(op->copy_event);
     for (int b = 0; b < 5; ++b) cudaFree(op->pblk[b]);
     cudaFree(op->Ah);
+    cudaFree(op->Ax);
     cudaFree(op->Xh);
     cudaFree(op->amax);
     cudaFree(op->nbr);
@@ -243,11 +247,20 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
         }                                    \
     } while (0)
     const bool want_tc = dtype == COARSE_C64 && !(flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) && tc_supported(nbasis, 8);
-    const bool want_h16 = want_tc && !(flags & COARSE_FLAG_TF32) && h16_supported(nbasis, 8);
+    const bool want_split16 = want_tc && !(flags & COARSE_FLAG_TF32);
+    const bool want_h16x = want_split16 && h16x_supported(nbasis, 8) && (nbasis != 32 || (flags & COARSE_FLAG_H16X));
+    const bool want_h16 = want_split16 && !want_h16x && h16_supported(nbasis, 8);
     const bool want_simt = !(want_tc && (flags & COARSE_FLAG_TENSOR_ONLY));
     if (want_simt) CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
-    if (want_tc && !want_h16) CMRHS_TRY(alloc_dev(op, (void **)&op->Ak, a_bytes));
+    if (want_tc && !want_h16 && !want_h16x) CMRHS_TRY(alloc_dev(op, (void **)&op->Ak, a_bytes));
+    if (want_h16x) {
+        CMRHS_TRY(alloc_dev(op, (void **)&op->Ax, a_bytes));
+        CMRHS_TRY(alloc_dev(op, (void **)&op->amax, 128 * sizeof(uint32_t)));
+        const size_t xh_bytes = (size_t)V * h16x_site_bytes(nbasis, nrhs_max);
+        CMRHS_TRY(alloc_dev(op, (void **)&op->Xh, xh_bytes));
+        CMRHS_CUDA(cudaMemsetAsync(op->Xh, 0, xh_bytes, stream));       // padding rows of the chunks are never written again
+    }
     if (want_h16) {
         CMRHS_TRY(alloc_dev(op, (void **)&op->Ah, a_bytes));
         CMRHS_TRY(alloc_dev(op, (void **)&op->amax, 128 * sizeof(uint32_t)));
@@ -279,12 +292,12 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
             relayout_transpose_kernel<double><<<rgrid, 128, 0, stream>>>((const cplx<double> *)A_dev, (cplx<double> *)op->At, ntiles, nbasis);
         count_launch();
     }
-    if (want_tc && !want_h16) {
+    if (want_tc && !want_h16 && !want_h16x) {
         relayout_planar_kernel<<<rgrid, 128, 0, stream>>>((const cplx<float> *)A_dev, op->Ak, ntiles, nbasis);
         count_launch();
         op->tc_ok = true;
     }
-    if (want_h16) {
+    if (want_h16 || want_h16x) {
         // operator scale: the power of two that maps max |Re a|, |Im a| into [2^14, 2^15) (stencil_h16.cuh)
         uint32_t bits = 0;
         ce = cudaMemsetAsync(op->amax, 0, 128 * sizeof(uint32_t), stream);
@@ -301,9 +314,14 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
         }
         const float sA = h_scale_from_bits(bits);
         op->inv_sA = 1.0f / sA;
-        relayout_h16_kernel<<<rgrid, 256, 0, stream>>>((const cplx<float> *)A_dev, op->Ah, ntiles, sA);
+        if (want_h16) {
+            relayout_h16_kernel<<<rgrid, 256, 0, stream>>>((const cplx<float> *)A_dev, op->Ah, ntiles, sA);
+            op->h16_ok = true;
+        } else {
+            relayout_h16x_kernel<<<rgrid, 256, 0, stream>>>((const cplx<float> *)A_dev, op->Ax, ntiles, nbasis, sA);
+            op->h16x_ok = true;
+        }
         count_launch();
-        op->h16_ok = true;
     }
     ce = cudaGetLastError();
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(stream);
@@ -326,11 +344,20 @@ static const SimtVariant *select_variant(const coarse_op *op, int nrhs)
 
 static bool use_tc(const coarse_op *op, int nrhs) { return op->tc_ok && tc_supported(op->nb, nrhs); }
 static bool use_h16(const coarse_op *op, int nrhs) { return op->h16_ok && h16_supported(op->nb, nrhs); }
+// the X-in-tensor-memory kernel covers every nrhs; a single column (or a pair) is left to a tuned SIMT variant when there is one
+static bool use_h16x(const coarse_op *op, int nrhs)
+{
+    if (!op->h16x_ok || !h16x_supported(op->nb, nrhs)) return false;
+    return nrhs >= 4 || !op->At || !find_variant(op->dtype, op->nb, nrhs);
+}
+// the kernels whose X operand is scaled by per-column powers of two (column maxima in op->amax)
+static bool use_split16(const coarse_op *op, int nrhs) { return use_h16(op, nrhs) || use_h16x(op, nrhs); }
 
 extern "C" const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs)
 {
     if (!op) return "";
     if (use_h16(op, nrhs)) return "stencil_h16<fp16x3>";
+    if (use_h16x(op, nrhs)) return "stencil_h16x<fp16x3>";
     if (use_tc(op, nrhs)) return "stencil_tc<tf32x3>";
     if (!op->At) return "unsupported";
     const SimtVariant *v = select_variant(op, nrhs);
@@ -357,6 +384,15 @@ static int apply_launch(const coarse_op *op, const void *X, void *Y, int nrhs, c
     if (use_h16(op, nrhs)) {
         if (!have_colmax) const_cast<coarse_op *>(op)->d_colmax_ready = false;     // this apply's own pre-pass overwrites op->amax
         return launch_stencil_h16(op->Ah, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream, have_colmax);
+    }
+    if (use_h16x(op, nrhs)) {
+        if (!have_colmax) const_cast<coarse_op *>(op)->d_colmax_ready = false;
+        switch (op->nb) {
+        case 8: return launch_stencil_h16x<8>(op->Ax, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream, have_colmax);
+        case 16: return launch_stencil_h16x<16>(op->Ax, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream, have_colmax);
+        case 24: return launch_stencil_h16x<24>(op->Ax, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream, have_colmax);
+        default: return launch_stencil_h16x<32>(op->Ax, op->inv_sA, op->amax, op->Xh, op->dims, X, Y, nrhs, op->num_sms, stream, have_colmax);
+        }
     }
     if (use_tc(op, nrhs)) {
         switch (op->nb) {
@@ -556,7 +592,7 @@ static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Ti
     auto kern = bcg_fused2_kernel<T, TR, W, S>;
     CMRHS_SMEM_ATTR(kern, p.smem);
     // the next reader of D is the stencil kernel: if that is the FP16-split one, its column-maxima pre-pass is done here
-    uint32_t *colmax = (sizeof(T) == 4 && op->h16_ok && h16_supported(op->nb, s)) ? op->amax : nullptr;
+    uint32_t *colmax = (sizeof(T) == 4 && use_split16(op, s)) ? op->amax : nullptr;
     if (colmax) CMRHS_CUDA(cudaMemsetAsync(colmax, 0, 64 * sizeof(uint32_t), stream));
     kern<<<p.grid, kLaThreads, p.smem, stream>>>((const cplx<T> *)Tin, (cplx<T> *)D, (cplx<T> *)Qout, K3, K4, n, s, colmax);
     const_cast<coarse_op *>(op)->d_colmax_ready = colmax != nullptr;

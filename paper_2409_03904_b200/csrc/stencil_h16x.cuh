@@ -1,0 +1,474 @@
+// Tensor-core stencil-GEMM kernel for complex64 on sm_100a, split-FP16, X OPERAND IN TENSOR MEMORY, any nbasis in {8,16,24,32}.
+//   Y(x) = sum_{p=0}^{80} A^p(x) . X(x + delta_p)                       (Eq. 19)
+//
+// Same numbers as stencil_h16.cuh (a = hi + 2^-11 lo in binary16 after a power-of-two scaling, three tensor products,
+// FP32 accumulators D and C in tensor memory, Y = (D + 2^-11 C) / (sA sX_r)), in the TRANSPOSED form
+//   D_x[(r,c)][(h,part,i)] += sum_k X(y)[k][(r,c)] . A^p(x)_{h,part}[i][k]          y = x + delta_p
+// * M side (the 128 TMEM lanes) = the 2 nrhs real columns (r, re/im) of the neighbour's X tile, held IN TENSOR MEMORY
+//   (tcgen05.mma with the A operand from TMEM): lane m, 16-bit pairs along k.  Loader warps read the pre-split tile
+//   (one coalesced 16-byte load per lane and 8 k) from L2 and write it with tcgen05.st -- the tile never touches shared
+//   memory, and the tensor core reads only the stencil matrix through the shared-memory pipe.  (stencil_h16.cuh reads both
+//   operands of every MMA from shared memory and is bound by that pipe from nrhs 32 up.)
+// * N side = the stencil matrix, K-major without swizzle: 8 x 8 core matrices of binary16 (128 contiguous bytes), the
+//   tile stored in HBM as [k chunk of 8][n group of 8] with n = (hi/lo, Re/Im, row i): 8 nb^2 bytes for ANY nb that is a
+//   multiple of 8 (no padding bytes in HBM: same size as complex64); one 1-D bulk copy per stencil matrix.
+//   MMA 1: X_hi^T . [A_hi | A_lo] -> D | C (N = 4 nb), MMA 2: X_lo^T . A_hi -> C (N = 2 nb), per K = 16 slab.
+//   nb = 8, 24: the last K = 16 slab is half empty: the X operand holds zeros there, the ring stage a zero chunk.
+// * One accumulator of 4 nb columns PER SITE (slots rotate: the epilogue of a site overlaps the MMAs of the next ones);
+//   two x-adjacent sites still share each X tile (110 tile loads per pair instead of 162).
+// * One persistent CTA per SM: loader warps (kXTurns per lane quarter, taking turns tile by tile, two tiles in
+//   registers each), 4 epilogue warps, one bulk-copy producer, one MMA issuer.  The ring of stencil matrices takes
+//   almost all of shared memory (the HBM stream needs ~100 KB in flight per SM).
+#pragma once
+
+#include "stencil_h16.cuh"
+
+namespace cmrhs {
+
+constexpr int kXTurns = 2;                    // loader warps per TMEM lane quarter
+constexpr int kXThreads = 32 * (4 * kXTurns + 6);
+constexpr int kXMaxStagesA = 64;
+constexpr int kXMaxBuf = 8;
+
+template <int NB> struct XCfg {
+    static_assert(NB % 8 == 0 && NB >= 8 && NB <= 32, "h16x: nbasis in {8,16,24,32}");
+    static constexpr int KSTEPS = (NB + 15) / 16;               // K = 16 slabs per stencil matrix
+    static constexpr int NCH = NB / 8;                           // 8-wide k chunks that carry data
+    static constexpr uint32_t LBO = 64u * NB;                    // bytes between k chunks: 4 nb / 8 core matrices of 128 B
+    static constexpr uint32_t SBO = 128u;                        // bytes between n groups
+    static constexpr uint32_t TILE_BYTES = 8u * NB * NB;         // one stencil matrix, [A_hi | A_lo]
+    static constexpr uint32_t STAGE_BYTES = 2u * KSTEPS * LBO;   // ring stage (>= TILE_BYTES; the rest stays zero)
+    static constexpr int ACC_COLS = 4 * NB;                      // D (2 nb) | C (2 nb) per site
+    static constexpr int XHALF = 8 * KSTEPS;                     // TMEM columns of X_hi (or X_lo) of one tile
+    static constexpr int XCOLS = 2 * XHALF;
+    static constexpr int NACC = NB == 32 ? 3 : 4;                // accumulator slots
+    static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS < kXMaxBuf ? (512 - NACC * ACC_COLS) / XCOLS : kXMaxBuf;
+    static constexpr int XBASE = NACC * ACC_COLS;
+    static_assert(XBASE + NXB * XCOLS <= 512 && NXB >= 3, "tensor memory plan");
+};
+
+struct XParams {
+    int32_t L[4];
+    int32_t ng0, ngroups;
+    int32_t s, N2;            // nrhs, 2 nrhs = real columns of an X tile = M rows in use
+    int32_t m32;              // N2 rounded up to a multiple of 32: rows of one chunk of the split X tile
+    int32_t nq;               // TMEM lane quarters in use = m32 / 32
+    int32_t sa;               // ring depth (stencil matrices)
+    int32_t xh_site_bytes;    // bytes of one split X tile: 2 (hi, lo) x NCH x m32 x 16
+    uint32_t idesc_wide, idesc_lo;
+    float inv_sA;
+    const uint32_t *amax;
+};
+
+// position in the sequence of X tiles (= MMA steps) a CTA walks: groups g, g + grid, ...; steps 0 .. nsteps-1 of each
+struct XCursor {
+    int g, step;
+    TcGroup grp;
+};
+
+template <int NB>
+__global__ void __launch_bounds__(kXThreads, 1)
+stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *__restrict__ Xh, float *__restrict__ Y, const XParams P)
+{
+    using C = XCfg<NB>;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char *smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+    unsigned char *ringA = smem;
+    uint32_t *tab2 = reinterpret_cast<uint32_t *>(ringA + (size_t)P.sa * C::STAGE_BYTES);
+    uint32_t *tab1 = tab2 + kTcMaxSteps;
+    int32_t *last = reinterpret_cast<int32_t *>(tab1 + kTcMaxSteps);     // [0,1]: last step of site 0 / 1 in a pair, [2]: single site
+    float *inv = reinterpret_cast<float *>(last + 4);                    // [128] per real column: 1 / (sA sX_r)
+    uint64_t *bars = reinterpret_cast<uint64_t *>(inv + 128);
+    uint64_t *a_full = bars, *a_empty = a_full + kXMaxStagesA;
+    uint64_t *x_full = a_empty + kXMaxStagesA, *x_empty = x_full + kXMaxBuf;
+    uint64_t *acc_full = x_empty + kXMaxBuf, *acc_empty = acc_full + kXMaxBuf;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_empty + kXMaxBuf);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int kWEpi = 4 * kXTurns, kWProd = kWEpi + 4, kWMma = kWEpi + 5;
+#ifdef CMRHS_TC_TRACE
+    long long wt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long t_begin = clock64();
+#endif
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
+        for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[i], (uint32_t)P.nq); mbar_init(&x_empty[i], 1); }
+        for (int i = 0; i < C::NACC; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 4); }
+        mbar_fence_init();
+    }
+    if (threadIdx.x == 32) {
+        const int n = tc_build_schedule(2, tab2);
+        int l0 = 0, l1 = 0;
+        for (int k = 0; k < n; ++k) {
+            if ((tab2[k] >> 8) & 1u) l0 = k;
+            if ((tab2[k] >> 9) & 1u) l1 = k;
+        }
+        last[0] = l0;
+        last[1] = l1;
+    }
+    if (threadIdx.x == 64) last[2] = tc_build_schedule(1, tab1) - 1;
+    if (threadIdx.x >= 128 && threadIdx.x < 256) {
+        const int col = threadIdx.x - 128;
+        const float sc = col < P.N2 ? h_scale_from_bits(P.amax[col >> 1]) : 1.0f;
+        inv[col] = P.inv_sA / sc;
+    }
+    if constexpr (C::STAGE_BYTES != C::TILE_BYTES) {
+        // the half-empty last K slab: the chunk after the data stays zero for the whole kernel (bulk copies never reach it)
+        for (int e = threadIdx.x; e < (int)((size_t)P.sa * C::STAGE_BYTES / 16); e += kXThreads)
+            reinterpret_cast<uint4 *>(ringA)[e] = make_uint4(0u, 0u, 0u, 0u);
+        fence_proxy_async_smem();
+    }
+    if (warp == kWProd) tmem_alloc_cols(tmem_slot, 512u);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+
+    auto group_of = [&](int g) {
+        TcGroup r;
+        const int gx = g % P.ng0;
+        int line = g / P.ng0;
+        r.x0 = gx * 2;
+        r.G = min(2, P.L[0] - r.x0);
+        r.y = line % P.L[1]; line /= P.L[1];
+        r.z = line % P.L[2];
+        r.t = line / P.L[2];
+        r.nsteps = r.G == 2 ? 110 : 81;
+        r.tab = r.G == 2 ? tab2 : tab1;
+        return r;
+    };
+    auto site_of = [&](int x, int y, int z, int t) { return x + (int64_t)P.L[0] * (y + (int64_t)P.L[1] * (z + (int64_t)P.L[2] * t)); };
+    auto x_site_of = [&](const TcGroup &g, uint32_t e) {
+        const int off3 = (int)(e & 31u), j = (int)((e >> 5) & 7u);
+        const int dy = off3 % 3 - 1, dz = (off3 / 3) % 3 - 1, dt = off3 / 9 - 1;
+        return site_of(tc_wrap(g.x0 + j - 1, P.L[0]), tc_wrap(g.y + dy, P.L[1]), tc_wrap(g.z + dz, P.L[2]), tc_wrap(g.t + dt, P.L[3]));
+    };
+
+    if (warp < kWEpi) {
+        // ================= X loaders: pre-split tile (L2) -> registers -> tensor memory =================
+        const int q = warp & 3, turn = warp >> 2;
+        if (q < P.nq) {
+            const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)C::XBASE;
+            const size_t row_off = (size_t)(32 * q + lane) * 16;
+            const size_t chunk_stride = (size_t)P.m32 * 16;
+            XCursor cur;
+            cur.g = blockIdx.x;
+            cur.step = 0;
+            bool more = cur.g < P.ngroups;
+            if (more) cur.grp = group_of(cur.g);
+            auto skip = [&](int n) {              // advance the cursor by n tiles
+                for (int k = 0; k < n && more; ++k) {
+                    if (++cur.step == cur.grp.nsteps) {
+                        cur.step = 0;
+                        cur.g += gridDim.x;
+                        more = cur.g < P.ngroups;
+                        if (more) cur.grp = group_of(cur.g);
+                    }
+                }
+            };
+            skip(turn);
+            auto load_next = [&](uint4 (&r)[2 * C::NCH]) -> bool {
+                if (!more) return false;
+                const unsigned char *src = Xh + x_site_of(cur.grp, cur.grp.tab[cur.step]) * (int64_t)P.xh_site_bytes + row_off;
+#pragma unroll
+                for (int c = 0; c < 2 * C::NCH; ++c) r[c] = __ldg(reinterpret_cast<const uint4 *>(src + (size_t)c * chunk_stride));
+                skip(kXTurns);
+                return true;
+            };
+            uint32_t t = (uint32_t)turn;          // sequence number of the tile held in the register set about to be stored
+            auto store = [&](const uint4 (&r)[2 * C::NCH]) {
+                const uint32_t b = t % (uint32_t)C::NXB, ph = (t / (uint32_t)C::NXB) & 1u;
+                TW(0, mbar_wait(&x_empty[b], ph ^ 1u));
+                tc_fence_after_sync();
+                TW_BEGIN();
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    uint32_t w[C::XHALF];
+#pragma unroll
+                    for (int c = 0; c < C::XHALF / 4; ++c) {
+                        if (c < C::NCH) {
+                            w[4 * c + 0] = r[h * C::NCH + c].x; w[4 * c + 1] = r[h * C::NCH + c].y;
+                            w[4 * c + 2] = r[h * C::NCH + c].z; w[4 * c + 3] = r[h * C::NCH + c].w;
+                        } else {
+                            w[4 * c + 0] = 0u; w[4 * c + 1] = 0u; w[4 * c + 2] = 0u; w[4 * c + 3] = 0u;
+                        }
+                    }
+                    tmem_st<C::XHALF>(lane_base + b * (uint32_t)C::XCOLS + (uint32_t)(h * C::XHALF), w);
+                }
+                tmem_wait_st();
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&x_full[b]);
+                TW_END(1);
+                t += kXTurns;
+            };
+            uint4 ra[2 * C::NCH], rb[2 * C::NCH];
+            bool va = load_next(ra), vb = load_next(rb);
+            for (;;) {
+                if (!va) break;
+                store(ra);
+                va = load_next(ra);
+                if (!vb) break;
+                store(rb);
+                vb = load_next(rb);
+            }
+        }
+    } else if (warp < kWEpi + 4) {
+        // ================= epilogue: Y = combine((D + 2^-11 C) / (sA sX)) -> global, one site per accumulator slot =================
+        // lanes = real columns n = (r, re/im), columns = (hi/lo, part, i):  Y_re = P[(r,0)] - Q[(r,1)],  Y_im = P[(r,1)] + Q[(r,0)]
+        const int q = warp - kWEpi;                       // = warp % 4: the TMEM lane quarter this warp may access
+        const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
+        const int n = 32 * q + lane, c = n & 1;
+        const bool live = n < P.N2;
+        const float sc = live ? inv[n] : 0.0f;
+        TcRing rc;
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const TcGroup grp = group_of(g);
+            for (int i = 0; i < grp.G; ++i) {
+                TW(0, mbar_wait(&acc_full[rc.stage], rc.phase));
+                tc_fence_after_sync();
+                TW_BEGIN();
+                if (q < P.nq) {
+                    const uint32_t ds = lane_base + (uint32_t)(rc.stage * C::ACC_COLS);
+                    float *yrow = Y + site_of(grp.x0 + i, grp.y, grp.z, grp.t) * (int64_t)(NB * P.N2) + n;
+#pragma unroll
+                    for (int ic = 0; ic < NB / 8; ++ic) {
+                        uint32_t dp[8], dq[8], cp[8], cq[8];
+                        tmem_ld_x8(ds + (uint32_t)(8 * ic), dp);
+                        tmem_ld_x8(ds + (uint32_t)(NB + 8 * ic), dq);
+                        tmem_ld_x8(ds + (uint32_t)(2 * NB + 8 * ic), cp);
+                        tmem_ld_x8(ds + (uint32_t)(3 * NB + 8 * ic), cq);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) {
+                            const float pv = (__uint_as_float(dp[k]) + __uint_as_float(cp[k]) * (1.0f / 2048.0f)) * sc;
+                            const float qv = (__uint_as_float(dq[k]) + __uint_as_float(cq[k]) * (1.0f / 2048.0f)) * sc;
+                            const float qo = __shfl_xor_sync(0xffffffffu, qv, 1);
+                            const float val = c == 0 ? pv - qo : pv + qo;
+                            if (live) yrow[(int64_t)(8 * ic + k) * P.N2] = val;
+                        }
+                    }
+                }
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[rc.stage]);
+                TW_END(1);
+                rc.advance(C::NACC);
+            }
+        }
+    } else if (warp == kWProd) {
+        // ================= A producer: one pre-split stencil matrix (contiguous) per stage, in the order the MMA warp uses them =================
+        const uint64_t pol = l2_policy_evict_first();
+        TcRing ra;
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const TcGroup grp = group_of(g);
+            const int64_t site0 = site_of(grp.x0, grp.y, grp.z, grp.t);
+            for (int step = 0; step < grp.nsteps; ++step) {
+                const uint32_t e = grp.tab[step];
+                const int off3 = (int)(e & 31u);
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    if (!((e >> (8 + i)) & 1u)) continue;
+                    const int p = (int)((e >> (10 + 2 * i)) & 3u) + 3 * off3;
+                    const unsigned char *src = Ax + ((site0 + i) * kNPoint + p) * (int64_t)C::TILE_BYTES;
+                    TW(0, mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u));
+                    if (elect_one_sync()) {
+                        mbar_arrive_expect_tx(&a_full[ra.stage], C::TILE_BYTES);
+                        bulk_g2s(ringA + (size_t)ra.stage * C::STAGE_BYTES, src, C::TILE_BYTES, &a_full[ra.stage], pol);
+                    }
+                    __syncwarp();
+                    ra.advance(P.sa);
+                }
+            }
+        }
+    } else if (warp == kWMma) {
+        // ================= MMA issuer (whole warp walks the schedule, one elected lane issues) =================
+        const uint32_t ring0 = smem_u32(ringA);
+        TcRing ra, rc;
+        uint32_t t = 0;                           // X tile sequence number
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const TcGroup grp = group_of(g);
+            TcRing slot[2];
+            slot[0] = rc;
+            rc.advance(C::NACC);
+            slot[1] = rc;
+            if (grp.G == 2) rc.advance(C::NACC);
+            const int last0 = grp.G == 2 ? last[0] : last[2], last1 = last[1];
+            uint32_t seen = 0u;
+            for (int step = 0; step < grp.nsteps; ++step, ++t) {
+                const uint32_t um = (grp.tab[step] >> 8) & 3u;
+                const uint32_t b = t % (uint32_t)C::NXB, xph = (t / (uint32_t)C::NXB) & 1u;
+                TW(2, mbar_wait(&x_full[b], xph));
+                const uint32_t x_hi = tmem + (uint32_t)C::XBASE + b * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XHALF;
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    if (!((um >> i) & 1u)) continue;
+                    const bool first = !((seen >> i) & 1u);
+                    if (first) TW(0, mbar_wait(&acc_empty[slot[i].stage], slot[i].phase ^ 1u));
+                    TW(1, mbar_wait(&a_full[ra.stage], ra.phase));
+                    tc_fence_after_sync();
+                    TW_BEGIN();
+                    if (elect_one_sync()) {
+                        const uint32_t ds = tmem + (uint32_t)(slot[i].stage * C::ACC_COLS);
+                        const uint32_t tile = ring0 + (uint32_t)ra.stage * C::STAGE_BYTES;
+#ifdef CMRHS_TC_TRACE
+                        const long long q0 = clock64();
+#endif
+#pragma unroll
+                        for (int ks = 0; ks < C::KSTEPS; ++ks) {
+                            const uint64_t bd = umma_desc_kmajor_noswz(tile + (uint32_t)ks * 2u * C::LBO, C::LBO, C::SBO);
+                            umma_f16_ts(ds, x_hi + 8u * ks, bd, P.idesc_wide, (!first || ks) ? 1u : 0u);      // X_hi^T . [A_hi | A_lo] -> D | C
+#ifdef CMRHS_TC_TRACE
+                            if (ks == 0) wt[4] += clock64() - q0;
+#endif
+                            umma_f16_ts(ds + 2u * NB, x_lo + 8u * ks, bd, P.idesc_lo, 1u);                     // X_lo^T . A_hi -> C
+                        }
+#ifdef CMRHS_TC_TRACE
+                        const long long q1 = clock64();
+                        wt[5] += q1 - q0;
+#endif
+                        umma_commit(&a_empty[ra.stage]);
+                        if (step == (i == 0 ? last0 : last1)) umma_commit(&acc_full[slot[i].stage]);
+#ifdef CMRHS_TC_TRACE
+                        wt[6] += clock64() - q1;
+#endif
+                    }
+                    __syncwarp();
+                    TW_END(3);
+                    ra.advance(P.sa);
+                }
+                if (elect_one_sync()) umma_commit(&x_empty[b]);
+                __syncwarp();
+                seen |= um;
+            }
+        }
+    }
+#ifdef CMRHS_TC_TRACE
+    if (lane == 0 && blockIdx.x < 160) {
+        wt[7] = clock64() - t_begin;
+        for (int k = 0; k < 8; ++k) g_tc_trace[blockIdx.x][warp][k] = wt[k];
+    }
+#endif
+    // ---- teardown ----
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    if (warp == kWProd) tmem_dealloc_cols(tmem, 512u);
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------
+inline bool h16x_supported(int nb, int s) { return (nb == 8 || nb == 16 || nb == 24 || nb == 32) && s >= 1 && s <= 64; }
+inline int h16x_m32(int s) { return (2 * s + 31) / 32 * 32; }
+// bytes of one split X tile
+inline int h16x_site_bytes(int nb, int s) { return 2 * (nb / 8) * h16x_m32(s) * 16; }
+
+// create-time re-layout: canonical A[t][i][k] (complex64) -> Ax[t] = [k chunk c][n group][n % 8][k % 8] binary16, n = (h, part, i):
+// the K-major, unswizzled shared-memory image of the N x K operand [A_hi | A_lo] (8 x 8 core matrices, 128 B each).
+// One thread per (c, part, i): 8 consecutive complex values in, one 16-byte row of a hi core matrix and of a lo core matrix out.
+__global__ void __launch_bounds__(256) relayout_h16x_kernel(const cplx<float> *__restrict__ A, unsigned char *__restrict__ Ax, int64_t ntiles, int nb,
+                                                            float sA)
+{
+    const int nch = nb / 8, items = nch * 2 * nb;
+    const int64_t tile_bytes = 8ll * nb * nb;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const cplx<float> *src = A + t * nb * nb;
+        unsigned char *dst = Ax + t * tile_bytes;
+        for (int e = threadIdx.x; e < items; e += 256) {
+            const int c = e / (2 * nb), pi = e - c * 2 * nb, part = pi / nb, i = pi - part * nb;
+            uint32_t hw[4], lw[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const cplx<float> v0 = src[i * nb + 8 * c + 2 * u], v1 = src[i * nb + 8 * c + 2 * u + 1];
+                const float a0 = (part ? v0.im : v0.re) * sA, a1 = (part ? v1.im : v1.re) * sA;
+                const __half2 h = __floats2half2_rn(a0, a1);
+                const float2 hf = __half22float2(h);
+                const __half2 l = __floats2half2_rn((a0 - hf.x) * 2048.0f, (a1 - hf.y) * 2048.0f);
+                hw[u] = *reinterpret_cast<const uint32_t *>(&h);
+                lw[u] = *reinterpret_cast<const uint32_t *>(&l);
+            }
+            const int n_hi = pi, n_lo = 2 * nb + pi;
+            unsigned char *base = dst + (int64_t)c * 64 * nb;
+            *reinterpret_cast<uint4 *>(base + (n_hi >> 3) * 128 + (n_hi & 7) * 16) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+            *reinterpret_cast<uint4 *>(base + (n_lo >> 3) * 128 + (n_lo & 7) * 16) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+        }
+    }
+}
+
+// per-apply pre-pass: X (fp32, [site][k][2 s real columns]) -> Xh[site][h][k chunk][m32 rows] of 16 bytes: the 8 binary16 values
+// k = 8 c .. 8 c + 7 of real column n, scaled by the column's power of two and split (hi = fp16(x), lo = fp16(2^11 (x - hi))).
+// Rows n >= 2 s of a chunk are never written (zeroed once at create).
+__global__ void __launch_bounds__(256) xsplit_x_kernel(const float *__restrict__ X, unsigned char *__restrict__ Xh, const uint32_t *__restrict__ amax,
+                                                       int64_t nsites, int nb, int s, int m32, int site_bytes)
+{
+    __shared__ float scl[128];
+    const int N2 = 2 * s, nch = nb / 8, items = nch * N2;
+    if (threadIdx.x < 128) scl[threadIdx.x] = threadIdx.x < N2 ? h_scale_from_bits(amax[threadIdx.x >> 1]) : 1.0f;
+    __syncthreads();
+    for (int64_t site = blockIdx.x; site < nsites; site += gridDim.x) {
+        const float *src = X + site * (int64_t)(nb * N2);
+        unsigned char *dst = Xh + site * (int64_t)site_bytes;
+        for (int e = threadIdx.x; e < items; e += 256) {
+            const int c = e / N2, n = e - c * N2;
+            const float sc = scl[n];
+            uint32_t hw[4], lw[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float x0 = src[(8 * c + 2 * u) * N2 + n] * sc, x1 = src[(8 * c + 2 * u + 1) * N2 + n] * sc;
+                const __half2 h = __floats2half2_rn(x0, x1);
+                const float2 hf = __half22float2(h);
+                const __half2 l = __floats2half2_rn((x0 - hf.x) * 2048.0f, (x1 - hf.y) * 2048.0f);
+                hw[u] = *reinterpret_cast<const uint32_t *>(&h);
+                lw[u] = *reinterpret_cast<const uint32_t *>(&l);
+            }
+            *reinterpret_cast<uint4 *>(dst + ((int64_t)c * m32 + n) * 16) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+            *reinterpret_cast<uint4 *>(dst + ((int64_t)(nch + c) * m32 + n) * 16) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+        }
+    }
+}
+
+template <int NB>
+int launch_stencil_h16x(const unsigned char *Ax, float inv_sA, uint32_t *amax_dev, unsigned char *Xh, const LatticeDims &d, const void *X,
+                        void *Y, int s, int num_sms, cudaStream_t stream, bool have_colmax)
+{
+    using C = XCfg<NB>;
+    XParams P;
+    for (int k = 0; k < 4; ++k) P.L[k] = d.L[k];
+    P.ng0 = (d.L[0] + 1) / 2;
+    P.ngroups = (int32_t)((int64_t)P.ng0 * d.L[1] * d.L[2] * d.L[3]);
+    P.s = s;
+    P.N2 = 2 * s;
+    P.m32 = h16x_m32(s);
+    P.nq = P.m32 / 32;
+    P.xh_site_bytes = h16x_site_bytes(NB, s);
+    const int64_t fixed = 128 /* alignment */ + 2 * kTcMaxSteps * 4 + 16 + 512 /* scales */ + (2 * kXMaxStagesA + 4 * kXMaxBuf) * 8 + 16;
+    const int64_t budget = 200 * 1024 - fixed;
+    P.sa = (int32_t)(budget / C::STAGE_BYTES);
+    if (P.sa > kXMaxStagesA) P.sa = kXMaxStagesA;
+    P.idesc_wide = umma_idesc_f16_kk(128, 4 * NB);
+    P.idesc_lo = umma_idesc_f16_kk(128, 2 * NB);
+    P.inv_sA = inv_sA;
+    P.amax = amax_dev;
+    const size_t smem = (size_t)fixed + (size_t)P.sa * C::STAGE_BYTES;
+
+    if (!have_colmax) {
+        CMRHS_CUDA(cudaMemsetAsync(amax_dev, 0, 64 * sizeof(uint32_t), stream));
+        const int64_t n = d.V * NB;
+        const int rpp = 256 / s;
+        const int cgrid = (int)(ceil_div(n, rpp) < (int64_t)num_sms * 8 ? ceil_div(n, rpp) : (int64_t)num_sms * 8);
+        colmax_kernel<<<cgrid, 256, 0, stream>>>(static_cast<const float2 *>(X), n, s, amax_dev);
+        CMRHS_LAUNCH_CHECK();
+    }
+    const int xgrid = (int)(d.V < (int64_t)num_sms * 8 ? d.V : (int64_t)num_sms * 8);
+    xsplit_x_kernel<<<xgrid, 256, 0, stream>>>(static_cast<const float *>(X), Xh, amax_dev, d.V, NB, s, P.m32, P.xh_site_bytes);
+    CMRHS_LAUNCH_CHECK();
+
+    auto kern = stencil_h16x_kernel<NB>;
+    CMRHS_SMEM_ATTR(kern, smem);
+    const int grid = P.ngroups < num_sms ? P.ngroups : num_sms;
+    kern<<<grid, kXThreads, smem, stream>>>(Ax, Xh, static_cast<float *>(Y), P);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+}  // namespace cmrhs
