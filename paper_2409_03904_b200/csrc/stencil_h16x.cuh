@@ -7,18 +7,23 @@
 // * M side (the 128 TMEM lanes) = the 2 nrhs real columns (r, re/im) of the neighbour's X tile, held IN TENSOR MEMORY
 //   (tcgen05.mma with the A operand from TMEM): lane m, 16-bit pairs along k.  Loader warps read the pre-split tile
 //   (one coalesced 16-byte load per lane and 8 k) from L2 and write it with tcgen05.st -- the tile never touches shared
-//   memory, and the tensor core reads only the stencil matrix through the shared-memory pipe.  (stencil_h16.cuh reads both
-//   operands of every MMA from shared memory and is bound by that pipe from nrhs 32 up.)
+//   memory, and the tensor core reads only the stencil matrix through the shared-memory pipe.
 // * N side = the stencil matrix, K-major without swizzle: 8 x 8 core matrices of binary16 (128 contiguous bytes), the
 //   tile stored in HBM as [k chunk of 8][n group of 8] with n = (hi/lo, Re/Im, row i): 8 nb^2 bytes for ANY nb that is a
 //   multiple of 8 (no padding bytes in HBM: same size as complex64); one 1-D bulk copy per stencil matrix.
 //   MMA 1: X_hi^T . [A_hi | A_lo] -> D | C (N = 4 nb), MMA 2: X_lo^T . A_hi -> C (N = 2 nb), per K = 16 slab.
 //   nb = 8, 24: the last K = 16 slab is half empty: the X operand holds zeros there, the ring stage a zero chunk.
-// * One accumulator of 4 nb columns PER SITE (slots rotate: the epilogue of a site overlaps the MMAs of the next ones);
-//   two x-adjacent sites still share each X tile (110 tile loads per pair instead of 162).
-// * One persistent CTA per SM: loader warps (kXTurns per lane quarter, taking turns tile by tile, two tiles in
-//   registers each), 4 epilogue warps, one bulk-copy producer, one MMA issuer.  The ring of stencil matrices takes
-//   almost all of shared memory (the HBM stream needs ~100 KB in flight per SM).
+// * A GROUP of up to GMAX x-adjacent sites (4; 2 at nbasis 32, where tensor memory holds no more accumulators) shares
+//   every X tile it needs: (G + 2) x 27 tile loads per group instead of 81 G -- the gather of X through L2 is the
+//   largest single cost of this kernel (measured: 21-25 % of the time at nrhs 64).
+// * EVERYTHING THAT SERIALISES IS PER SITE: one accumulator (4 nb TMEM columns), one ring of stencil matrices with its own
+//   producer lane, and one MMA-issuing warp per site of the group.  A single warp's dependent instruction stream
+//   (barrier tests, descriptor arithmetic, 4 MMAs + 2 commits per stencil point: ~600 clk) is what bounds an issuer, not
+//   the tensor pipe (144-192 clk per point): the sites' accumulators are independent, so their streams need no order.
+//   Barriers are per site too: a parity wait cannot tell phases two apart, so every barrier has exactly one waiter
+//   that sees each of its phases.
+// * One persistent CTA per SM: loader warps (kXTurns per lane quarter, taking turns tile by tile, two tiles in registers
+//   each), 4 epilogue warps, one producer warp (lane i feeds site i), GMAX MMA issuers.
 #pragma once
 
 #include "stencil_h16.cuh"
@@ -26,9 +31,11 @@
 namespace cmrhs {
 
 constexpr int kXTurns = 2;                    // loader warps per TMEM lane quarter
-constexpr int kXThreads = 32 * (4 * kXTurns + 6);
-constexpr int kXMaxStagesA = 64;
+constexpr int kXMaxStagesA = 32;              // per site
 constexpr int kXMaxBuf = 8;
+constexpr int kXMaxG = 4;
+constexpr int kXMaxSteps = 168;               // (G + 2) x 27 + G at G = 4: 166
+constexpr int kXViews = kXMaxG * (kXMaxG + 1) / 2;      // per-site views of the schedules of G = 1..4
 
 template <int NB> struct XCfg {
     static_assert(NB % 8 == 0 && NB >= 8 && NB <= 32, "h16x: nbasis in {8,16,24,32}");
@@ -41,10 +48,14 @@ template <int NB> struct XCfg {
     static constexpr int ACC_COLS = 4 * NB;                      // D (2 nb) | C (2 nb) per site
     static constexpr int XHALF = 8 * KSTEPS;                     // TMEM columns of X_hi (or X_lo) of one tile
     static constexpr int XCOLS = 2 * XHALF;
-    static constexpr int NACC = NB == 32 ? 3 : 4;                // accumulator slots
-    static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS < kXMaxBuf ? (512 - NACC * ACC_COLS) / XCOLS : kXMaxBuf;
+    static constexpr int GMAX = NB == 32 ? 2 : 4;                // sites per group
+    static constexpr int NACC = NB == 32 ? 3 : (NB == 24 ? 4 : (NB == 16 ? 6 : 8));      // accumulator slots
+    static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS < kXMaxBuf ? ((512 - NACC * ACC_COLS) / XCOLS >= 4 ? 4 : 2) : kXMaxBuf;
     static constexpr int XBASE = NACC * ACC_COLS;
-    static_assert(XBASE + NXB * XCOLS <= 512 && NXB >= 3, "tensor memory plan");
+    static constexpr int WARPS = 4 * kXTurns + 4 + 1 + GMAX;
+    static constexpr int THREADS = 32 * WARPS;
+    static_assert(XBASE + NXB * XCOLS <= 512 && NXB >= 4 && (NXB & (NXB - 1)) == 0 && NXB % kXTurns == 0, "tensor memory plan");
+    static_assert(NACC >= GMAX, "one accumulator per site of a group");
 };
 
 struct XParams {
@@ -53,69 +64,89 @@ struct XParams {
     int32_t s, N2;            // nrhs, 2 nrhs = real columns of an X tile = M rows in use
     int32_t m32;              // N2 rounded up to a multiple of 32: rows of one chunk of the split X tile
     int32_t nq;               // TMEM lane quarters in use = m32 / 32
-    int32_t sa;               // ring depth (stencil matrices)
+    int32_t sa;               // depth of each site's ring of stencil matrices
     int32_t xh_site_bytes;    // bytes of one split X tile: 2 (hi, lo) x NCH x m32 x 16
     uint32_t idesc_wide, idesc_lo;
     float inv_sA;
     const uint32_t *amax;
 };
 
-// position in the sequence of X tiles (= MMA steps) a CTA walks: groups g, g + grid, ...; steps 0 .. nsteps-1 of each
-struct XCursor {
-    int g, step;
-    TcGroup grp;
-};
+// Schedule of a group of G <= 4 x-adjacent sites x0 .. x0+G-1: one step per X tile, the sites that use it accumulate it.
+// tab entry:  bits 0-3 user mask | 4-6 j (the tile sits at x' = x0 + j - 1) | 8-9 dy+1 | 10-11 dz+1 | 12-13 dt+1
+// view entry (one per stencil point of site i, in the order the site accumulates them):  bits 0-7 step | 16-22 point p
+// Order: the 26 non-centre (dy,dz,dt) offsets first, then the centre offset's dx = -1, +1 points, each site's own centre point
+// (p = 40, which carries c*I) last: the running float32 sums stay small until the large term arrives.
+__device__ inline int hx_build_schedule(int G, uint32_t *tab, uint32_t *view /* [G][84] */)
+{
+    int n = 0, cnt[kXMaxG] = {0, 0, 0, 0};
+    auto emit = [&](int o, int j, bool centre_pass, int only) {
+        uint32_t um = 0;
+        for (int i = 0; i < G; ++i) {
+            const int dx = j - 1 - i;
+            if (dx < -1 || dx > 1) continue;
+            if (only >= 0 ? i != only : (centre_pass && dx == 0)) continue;
+            um |= 1u << i;
+            view[i * 84 + cnt[i]++] = (uint32_t)n | ((uint32_t)((dx + 1) + 3 * o) << 16);
+        }
+        if (um) tab[n++] = um | ((uint32_t)j << 4) | ((uint32_t)(o % 3) << 8) | ((uint32_t)((o / 3) % 3) << 10) | ((uint32_t)(o / 9) << 12);
+    };
+    for (int o = 0; o < 27; ++o) {
+        if (o == 13) continue;
+        for (int j = 0; j < G + 2; ++j) emit(o, j, false, -1);
+    }
+    for (int j = 0; j < G + 2; ++j) emit(13, j, true, -1);
+    for (int i = 0; i < G; ++i) emit(13, i + 1, false, i);
+    return n;
+}
+
+struct XGroup { int x0, G, y, z, t, nsteps; const uint32_t *tab; const uint32_t *view; };
 
 template <int NB>
-__global__ void __launch_bounds__(kXThreads, 1)
+__global__ void __launch_bounds__(XCfg<NB>::THREADS, 1)
 stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *__restrict__ Xh, float *__restrict__ Y, const XParams P)
 {
     using C = XCfg<NB>;
+    constexpr int GMAX = C::GMAX;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-    unsigned char *ringA = smem;
-    uint32_t *tab2 = reinterpret_cast<uint32_t *>(ringA + (size_t)P.sa * C::STAGE_BYTES);
-    uint32_t *tab1 = tab2 + kTcMaxSteps;
-    int32_t *last = reinterpret_cast<int32_t *>(tab1 + kTcMaxSteps);     // [0,1]: last step of site 0 / 1 in a pair, [2]: single site
-    float *inv = reinterpret_cast<float *>(last + 4);                    // [128] per real column: 1 / (sA sX_r)
+    unsigned char *ringA = smem;                 // GMAX rings of P.sa stages: site i's stencil matrices at ring i
+    uint32_t *tabs = reinterpret_cast<uint32_t *>(ringA + (size_t)GMAX * P.sa * C::STAGE_BYTES);      // [G-1][kXMaxSteps]
+    uint32_t *views = tabs + kXMaxG * kXMaxSteps;                        // [G (G-1) / 2 + i][84]
+    int32_t *nsteps = reinterpret_cast<int32_t *>(views + kXViews * 84); // [G-1]
+    float *inv = reinterpret_cast<float *>(nsteps + 4);                  // [128] per real column: 1 / (sA sX_r)
     uint64_t *bars = reinterpret_cast<uint64_t *>(inv + 128);
-    uint64_t *a_full = bars, *a_empty = a_full + kXMaxStagesA;
-    uint64_t *x_full = a_empty + kXMaxStagesA, *x_empty = x_full + kXMaxBuf;
-    uint64_t *acc_full = x_empty + kXMaxBuf, *acc_empty = acc_full + kXMaxBuf;
+    uint64_t *a_full = bars, *a_empty = a_full + kXMaxG * kXMaxStagesA;              // [site][stage]
+    uint64_t *x_full = a_empty + kXMaxG * kXMaxStagesA, *x_empty = x_full + kXMaxG * kXMaxBuf;      // [site][buffer]
+    uint64_t *acc_full = x_empty + kXMaxG * kXMaxBuf, *acc_empty = acc_full + kXMaxBuf;            // [slot]
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_empty + kXMaxBuf);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int kWEpi = 4 * kXTurns, kWProd = kWEpi + 4, kWMma = kWEpi + 5;
+    constexpr int kWEpi = 4 * kXTurns, kWProd = kWEpi + 4, kWMma = kWProd + 1;
 #ifdef CMRHS_TC_TRACE
     long long wt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     const long long t_begin = clock64();
 #endif
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
-        for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[i], (uint32_t)P.nq); mbar_init(&x_empty[i], 1); }
+        for (int j = 0; j < GMAX; ++j) {
+            for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[j * kXMaxStagesA + i], 1); mbar_init(&a_empty[j * kXMaxStagesA + i], 1); }
+            for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[j * kXMaxBuf + i], (uint32_t)P.nq); mbar_init(&x_empty[j * kXMaxBuf + i], 1); }
+        }
         for (int i = 0; i < C::NACC; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 4); }
         mbar_fence_init();
     }
-    if (threadIdx.x == 32) {
-        const int n = tc_build_schedule(2, tab2);
-        int l0 = 0, l1 = 0;
-        for (int k = 0; k < n; ++k) {
-            if ((tab2[k] >> 8) & 1u) l0 = k;
-            if ((tab2[k] >> 9) & 1u) l1 = k;
-        }
-        last[0] = l0;
-        last[1] = l1;
+    if (warp >= 1 && warp <= GMAX && lane == 0) {
+        const int G = warp;
+        nsteps[G - 1] = hx_build_schedule(G, tabs + (G - 1) * kXMaxSteps, views + (G * (G - 1) / 2) * 84);
     }
-    if (threadIdx.x == 64) last[2] = tc_build_schedule(1, tab1) - 1;
-    if (threadIdx.x >= 128 && threadIdx.x < 256) {
-        const int col = threadIdx.x - 128;
+    if (threadIdx.x >= 256 && threadIdx.x < 384) {
+        const int col = threadIdx.x - 256;
         const float sc = col < P.N2 ? h_scale_from_bits(P.amax[col >> 1]) : 1.0f;
         inv[col] = P.inv_sA / sc;
     }
     if constexpr (C::STAGE_BYTES != C::TILE_BYTES) {
         // the half-empty last K slab: the chunk after the data stays zero for the whole kernel (bulk copies never reach it)
-        for (int e = threadIdx.x; e < (int)((size_t)P.sa * C::STAGE_BYTES / 16); e += kXThreads)
+        for (int e = threadIdx.x; e < (int)((size_t)GMAX * P.sa * C::STAGE_BYTES / 16); e += C::THREADS)
             reinterpret_cast<uint4 *>(ringA)[e] = make_uint4(0u, 0u, 0u, 0u);
         fence_proxy_async_smem();
     }
@@ -126,24 +157,20 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     const uint32_t tmem = *tmem_slot;
 
     auto group_of = [&](int g) {
-        TcGroup r;
+        XGroup r;
         const int gx = g % P.ng0;
         int line = g / P.ng0;
-        r.x0 = gx * 2;
-        r.G = min(2, P.L[0] - r.x0);
+        r.x0 = gx * GMAX;
+        r.G = min(GMAX, P.L[0] - r.x0);
         r.y = line % P.L[1]; line /= P.L[1];
         r.z = line % P.L[2];
         r.t = line / P.L[2];
-        r.nsteps = r.G == 2 ? 110 : 81;
-        r.tab = r.G == 2 ? tab2 : tab1;
+        r.nsteps = nsteps[r.G - 1];
+        r.tab = tabs + (r.G - 1) * kXMaxSteps;
+        r.view = views + (r.G * (r.G - 1) / 2) * 84;
         return r;
     };
     auto site_of = [&](int x, int y, int z, int t) { return x + (int64_t)P.L[0] * (y + (int64_t)P.L[1] * (z + (int64_t)P.L[2] * t)); };
-    auto x_site_of = [&](const TcGroup &g, uint32_t e) {
-        const int off3 = (int)(e & 31u), j = (int)((e >> 5) & 7u);
-        const int dy = off3 % 3 - 1, dz = (off3 / 3) % 3 - 1, dt = off3 / 9 - 1;
-        return site_of(tc_wrap(g.x0 + j - 1, P.L[0]), tc_wrap(g.y + dy, P.L[1]), tc_wrap(g.z + dz, P.L[2]), tc_wrap(g.t + dt, P.L[3]));
-    };
 
     if (warp < kWEpi) {
         // ================= X loaders: pre-split tile (L2) -> registers -> tensor memory =================
@@ -152,34 +179,47 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
             const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)C::XBASE;
             const size_t row_off = (size_t)(32 * q + lane) * 16;
             const size_t chunk_stride = (size_t)P.m32 * 16;
-            XCursor cur;
-            cur.g = blockIdx.x;
-            cur.step = 0;
-            bool more = cur.g < P.ngroups;
-            if (more) cur.grp = group_of(cur.g);
+            int cg = blockIdx.x, cstep = 0;       // cursor in the sequence of X tiles this CTA walks
+            bool more = cg < P.ngroups;
+            XGroup grp;
+            if (more) grp = group_of(cg);
             auto skip = [&](int n) {              // advance the cursor by n tiles
                 for (int k = 0; k < n && more; ++k) {
-                    if (++cur.step == cur.grp.nsteps) {
-                        cur.step = 0;
-                        cur.g += gridDim.x;
-                        more = cur.g < P.ngroups;
-                        if (more) cur.grp = group_of(cur.g);
+                    if (++cstep == grp.nsteps) {
+                        cstep = 0;
+                        cg += gridDim.x;
+                        more = cg < P.ngroups;
+                        if (more) grp = group_of(cg);
                     }
                 }
             };
             skip(turn);
-            auto load_next = [&](uint4 (&r)[2 * C::NCH]) -> bool {
+            auto load_next = [&](uint4 (&r)[2 * C::NCH], uint32_t &um) -> bool {
                 if (!more) return false;
-                const unsigned char *src = Xh + x_site_of(cur.grp, cur.grp.tab[cur.step]) * (int64_t)P.xh_site_bytes + row_off;
+                const uint32_t e = grp.tab[cstep];
+                um = e & 15u;
+                const int xs = tc_wrap(grp.x0 + (int)((e >> 4) & 7u) - 1, P.L[0]), ys = tc_wrap(grp.y + (int)((e >> 8) & 3u) - 1, P.L[1]);
+                const int zs = tc_wrap(grp.z + (int)((e >> 10) & 3u) - 1, P.L[2]), ts = tc_wrap(grp.t + (int)((e >> 12) & 3u) - 1, P.L[3]);
+                const unsigned char *src = Xh + (int64_t)(xs + P.L[0] * (ys + P.L[1] * (zs + P.L[2] * ts))) * (int64_t)P.xh_site_bytes + row_off;
 #pragma unroll
                 for (int c = 0; c < 2 * C::NCH; ++c) r[c] = __ldg(reinterpret_cast<const uint4 *>(src + (size_t)c * chunk_stride));
                 skip(kXTurns);
                 return true;
             };
-            uint32_t t = (uint32_t)turn;          // sequence number of the tile held in the register set about to be stored
-            auto store = [&](const uint4 (&r)[2 * C::NCH]) {
-                const uint32_t b = t % (uint32_t)C::NXB, ph = (t / (uint32_t)C::NXB) & 1u;
-                TW(0, mbar_wait(&x_empty[b], ph ^ 1u));
+            // this warp always meets the same buffers (NXB is a multiple of the number of turns): per buffer and site it keeps
+            // who used the tile it stored there last (pend) and the parity of that site's next release (par); bit 4 b + i
+            uint32_t t = (uint32_t)turn, pend = 0u, par = 0u;
+            auto store = [&](const uint4 (&r)[2 * C::NCH], uint32_t um) {
+                const uint32_t b = t & (uint32_t)(C::NXB - 1);
+#pragma unroll
+                for (int i = 0; i < GMAX; ++i) {
+                    const uint32_t bit = 1u << (4u * b + i);
+                    if (pend & bit) {
+                        TW(0, mbar_wait(&x_empty[i * kXMaxBuf + b], (par & bit) ? 1u : 0u));
+                        par ^= bit;
+                    }
+                }
+                pend = (pend & ~(15u << (4u * b))) | (um << (4u * b));
                 tc_fence_after_sync();
                 TW_BEGIN();
 #pragma unroll
@@ -199,22 +239,24 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 tmem_wait_st();
                 tc_fence_before_sync();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&x_full[b]);
+                if (lane < GMAX && ((um >> lane) & 1u)) mbar_arrive(&x_full[lane * kXMaxBuf + b]);
                 TW_END(1);
                 t += kXTurns;
             };
             uint4 ra[2 * C::NCH], rb[2 * C::NCH];
-            bool va = load_next(ra), vb = load_next(rb);
+            uint32_t ua = 0u, ub = 0u;
+            bool va = load_next(ra, ua), vb = load_next(rb, ub);
             for (;;) {
                 if (!va) break;
-                store(ra);
-                va = load_next(ra);
+                store(ra, ua);
+                va = load_next(ra, ua);
                 if (!vb) break;
-                store(rb);
-                vb = load_next(rb);
+                store(rb, ub);
+                vb = load_next(rb, ub);
             }
         }
-    } else if (warp < kWEpi + 4) {
+    }
+    else if (warp < kWEpi + 4) {
         // ================= epilogue: Y = combine((D + 2^-11 C) / (sA sX)) -> global, one site per accumulator slot =================
         // lanes = real columns n = (r, re/im), columns = (hi/lo, part, i):  Y_re = P[(r,0)] - Q[(r,1)],  Y_im = P[(r,1)] + Q[(r,0)]
         const int q = warp - kWEpi;                       // = warp % 4: the TMEM lane quarter this warp may access
@@ -224,9 +266,9 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         const float sc = live ? inv[n] : 0.0f;
         TcRing rc;
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-            const TcGroup grp = group_of(g);
+            const XGroup grp = group_of(g);
             for (int i = 0; i < grp.G; ++i) {
-                TW(0, mbar_wait(&acc_full[rc.stage], rc.phase));
+                TW(0, mbar_wait_long(&acc_full[rc.stage], rc.phase, 256u));
                 tc_fence_after_sync();
                 TW_BEGIN();
                 if (q < P.nq) {
@@ -258,90 +300,103 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
             }
         }
     } else if (warp == kWProd) {
-        // ================= A producer: one pre-split stencil matrix (contiguous) per stage, in the order the MMA warp uses them =================
+        // ================= A producer: ONE warp, LANE i feeds site i's ring (the warp runs one uniform polling loop, every lane on its
+        // own ring, barrier, group cursor and stencil-matrix pointer): the site's 81 pre-split stencil matrices, each one contiguous
+        // bulk copy, in the order the site accumulates them =================
+        const int me = lane;
         const uint64_t pol = l2_policy_evict_first();
+        unsigned char *ring = ringA + (size_t)(me < GMAX ? me : 0) * P.sa * C::STAGE_BYTES;
+        uint64_t *full = a_full + (me < GMAX ? me : 0) * kXMaxStagesA, *empty = a_empty + (me < GMAX ? me : 0) * kXMaxStagesA;
         TcRing ra;
-        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-            const TcGroup grp = group_of(g);
-            const int64_t site0 = site_of(grp.x0, grp.y, grp.z, grp.t);
-            for (int step = 0; step < grp.nsteps; ++step) {
-                const uint32_t e = grp.tab[step];
-                const int off3 = (int)(e & 31u);
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    if (!((e >> (8 + i)) & 1u)) continue;
-                    const int p = (int)((e >> (10 + 2 * i)) & 3u) + 3 * off3;
-                    const unsigned char *src = Ax + ((site0 + i) * kNPoint + p) * (int64_t)C::TILE_BYTES;
-                    TW(0, mbar_wait(&a_empty[ra.stage], ra.phase ^ 1u));
-                    if (elect_one_sync()) {
-                        mbar_arrive_expect_tx(&a_full[ra.stage], C::TILE_BYTES);
-                        bulk_g2s(ringA + (size_t)ra.stage * C::STAGE_BYTES, src, C::TILE_BYTES, &a_full[ra.stage], pol);
-                    }
-                    __syncwarp();
-                    ra.advance(P.sa);
+        int g = blockIdx.x, k = 0;
+        bool active = me < GMAX && g < P.ngroups;
+        const unsigned char *src0 = nullptr;
+        const uint32_t *tm = nullptr;
+        auto enter_group = [&]() {               // skips the groups that have no site `me`
+            while (active) {
+                const XGroup grp = group_of(g);
+                if (me < grp.G) {
+                    tm = grp.view + me * 84;
+                    src0 = Ax + (site_of(grp.x0 + me, grp.y, grp.z, grp.t) * kNPoint) * (int64_t)C::TILE_BYTES;
+                    return;
+                }
+                g += gridDim.x;
+                active = g < P.ngroups;
+            }
+        };
+        enter_group();
+        while (__any_sync(0xffffffffu, active)) {
+            if (active && mbar_test_wait(&empty[ra.stage], ra.phase ^ 1u)) {
+                const uint32_t p = (tm[k] >> 16) & 0x7Fu;
+                mbar_arrive_expect_tx(&full[ra.stage], C::TILE_BYTES);
+                bulk_g2s(ring + (size_t)ra.stage * C::STAGE_BYTES, src0 + (size_t)p * C::TILE_BYTES, C::TILE_BYTES, &full[ra.stage], pol);
+                ra.advance(P.sa);
+                if (++k == kNPoint) {
+                    k = 0;
+                    g += gridDim.x;
+                    active = g < P.ngroups;
+                    enter_group();
                 }
             }
         }
-    } else if (warp == kWMma) {
-        // ================= MMA issuer (whole warp walks the schedule, one elected lane issues) =================
-        const uint32_t ring0 = smem_u32(ringA);
-        TcRing ra, rc;
-        uint32_t t = 0;                           // X tile sequence number
+    } else if (warp < kWMma + GMAX) {
+        // ================= MMA issuers, one warp PER SITE of a group; one elected lane issues.  The barrier tests of the NEXT stencil
+        // point are started before the MMAs of this one (non-blocking test_wait), so their latency overlaps the issue. =================
+        const int me = warp - kWMma;
+        const uint32_t ring0 = smem_u32(ringA + (size_t)me * P.sa * C::STAGE_BYTES);
+        const uint32_t x_base = tmem + (uint32_t)C::XBASE;
+        uint64_t *afull = a_full + me * kXMaxStagesA, *aempty = a_empty + me * kXMaxStagesA;
+        uint64_t *xfull = x_full + me * kXMaxBuf, *xempty = x_empty + me * kXMaxBuf;
+        constexpr uint32_t xmask = (uint32_t)C::NXB - 1u;
+        const uint64_t desc_hi = umma_desc_kmajor_noswz(0u, C::LBO, C::SBO);      // everything but the start address
+        TcRing rc, ra;
+        uint32_t xcnt = 0;                        // X tiles before this group
+        uint32_t xpar = 0u;                       // bit b: parity of this site's next "full" phase of X buffer b
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
-            const TcGroup grp = group_of(g);
-            TcRing slot[2];
-            slot[0] = rc;
-            rc.advance(C::NACC);
-            slot[1] = rc;
-            if (grp.G == 2) rc.advance(C::NACC);
-            const int last0 = grp.G == 2 ? last[0] : last[2], last1 = last[1];
-            uint32_t seen = 0u;
-            for (int step = 0; step < grp.nsteps; ++step, ++t) {
-                const uint32_t um = (grp.tab[step] >> 8) & 3u;
-                const uint32_t b = t % (uint32_t)C::NXB, xph = (t / (uint32_t)C::NXB) & 1u;
-                TW(2, mbar_wait(&x_full[b], xph));
-                const uint32_t x_hi = tmem + (uint32_t)C::XBASE + b * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XHALF;
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    if (!((um >> i) & 1u)) continue;
-                    const bool first = !((seen >> i) & 1u);
-                    if (first) TW(0, mbar_wait(&acc_empty[slot[i].stage], slot[i].phase ^ 1u));
-                    TW(1, mbar_wait(&a_full[ra.stage], ra.phase));
+            const XGroup grp = group_of(g);
+            TcRing slot = rc;
+            for (int i = 0; i < me; ++i) slot.advance(C::NACC);
+            for (int i = 0; i < grp.G; ++i) rc.advance(C::NACC);
+            if (me < grp.G) {
+                const uint32_t *tm = grp.view + me * 84;
+                const uint32_t ds = tmem + (uint32_t)(slot.stage * C::ACC_COLS);
+                TW(0, mbar_wait(&acc_empty[slot.stage], slot.phase ^ 1u));
+                uint32_t xb = (xcnt + (tm[0] & 0xFFu)) & xmask;
+                bool okx = false, oka = false;
+                for (int k = 0; k < kNPoint; ++k) {
+                    if (!okx) TW(2, mbar_wait(&xfull[xb], (xpar >> xb) & 1u));
+                    xpar ^= 1u << xb;
+                    if (!oka) TW(1, mbar_wait(&afull[ra.stage], ra.phase));
                     tc_fence_after_sync();
+                    TcRing rn = ra;
+                    rn.advance(P.sa);
+                    uint32_t xbn = 0u;
+                    if (k + 1 < kNPoint) {
+                        xbn = (xcnt + (tm[k + 1] & 0xFFu)) & xmask;
+                        okx = mbar_test_wait(&xfull[xbn], (xpar >> xbn) & 1u);
+                        oka = mbar_test_wait(&afull[rn.stage], rn.phase);
+                    }
                     TW_BEGIN();
                     if (elect_one_sync()) {
-                        const uint32_t ds = tmem + (uint32_t)(slot[i].stage * C::ACC_COLS);
-                        const uint32_t tile = ring0 + (uint32_t)ra.stage * C::STAGE_BYTES;
-#ifdef CMRHS_TC_TRACE
-                        const long long q0 = clock64();
-#endif
+                        const uint32_t x_hi = x_base + xb * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XHALF;
+                        const uint64_t bd0 = desc_hi | (uint64_t)(((ring0 + (uint32_t)ra.stage * C::STAGE_BYTES) >> 4) & 0x3FFFu);
 #pragma unroll
                         for (int ks = 0; ks < C::KSTEPS; ++ks) {
-                            const uint64_t bd = umma_desc_kmajor_noswz(tile + (uint32_t)ks * 2u * C::LBO, C::LBO, C::SBO);
-                            umma_f16_ts(ds, x_hi + 8u * ks, bd, P.idesc_wide, (!first || ks) ? 1u : 0u);      // X_hi^T . [A_hi | A_lo] -> D | C
-#ifdef CMRHS_TC_TRACE
-                            if (ks == 0) wt[4] += clock64() - q0;
-#endif
-                            umma_f16_ts(ds + 2u * NB, x_lo + 8u * ks, bd, P.idesc_lo, 1u);                     // X_lo^T . A_hi -> C
+                            const uint64_t bd = bd0 + (uint64_t)((uint32_t)ks * 2u * C::LBO >> 4);
+                            umma_f16_ts(ds, x_hi + 8u * ks, bd, P.idesc_wide, (k | ks) ? 1u : 0u);      // X_hi^T . [A_hi | A_lo] -> D | C
+                            umma_f16_ts(ds + 2u * NB, x_lo + 8u * ks, bd, P.idesc_lo, 1u);              // X_lo^T . A_hi -> C
                         }
-#ifdef CMRHS_TC_TRACE
-                        const long long q1 = clock64();
-                        wt[5] += q1 - q0;
-#endif
-                        umma_commit(&a_empty[ra.stage]);
-                        if (step == (i == 0 ? last0 : last1)) umma_commit(&acc_full[slot[i].stage]);
-#ifdef CMRHS_TC_TRACE
-                        wt[6] += clock64() - q1;
-#endif
+                        umma_commit(&aempty[ra.stage]);
+                        umma_commit(&xempty[xb]);
+                        if (k == kNPoint - 1) umma_commit(&acc_full[slot.stage]);
                     }
                     __syncwarp();
                     TW_END(3);
-                    ra.advance(P.sa);
+                    ra = rn;
+                    xb = xbn;
                 }
-                if (elect_one_sync()) umma_commit(&x_empty[b]);
-                __syncwarp();
-                seen |= um;
             }
+            xcnt += (uint32_t)grp.nsteps;
         }
     }
 #ifdef CMRHS_TC_TRACE
@@ -434,22 +489,23 @@ int launch_stencil_h16x(const unsigned char *Ax, float inv_sA, uint32_t *amax_de
     using C = XCfg<NB>;
     XParams P;
     for (int k = 0; k < 4; ++k) P.L[k] = d.L[k];
-    P.ng0 = (d.L[0] + 1) / 2;
+    P.ng0 = (d.L[0] + C::GMAX - 1) / C::GMAX;
     P.ngroups = (int32_t)((int64_t)P.ng0 * d.L[1] * d.L[2] * d.L[3]);
     P.s = s;
     P.N2 = 2 * s;
     P.m32 = h16x_m32(s);
     P.nq = P.m32 / 32;
     P.xh_site_bytes = h16x_site_bytes(NB, s);
-    const int64_t fixed = 128 /* alignment */ + 2 * kTcMaxSteps * 4 + 16 + 512 /* scales */ + (2 * kXMaxStagesA + 4 * kXMaxBuf) * 8 + 16;
-    const int64_t budget = 200 * 1024 - fixed;
-    P.sa = (int32_t)(budget / C::STAGE_BYTES);
+    const int64_t fixed = 128 /* alignment */ + (kXMaxG * kXMaxSteps + kXViews * 84 + 4) * 4 + 512 /* scales */ +
+                          (2 * kXMaxG * kXMaxStagesA + 2 * kXMaxG * kXMaxBuf + 2 * kXMaxBuf) * 8 + 16;
+    const int64_t budget = 226 * 1024 - fixed;
+    P.sa = (int32_t)(budget / (C::GMAX * (int64_t)C::STAGE_BYTES));
     if (P.sa > kXMaxStagesA) P.sa = kXMaxStagesA;
     P.idesc_wide = umma_idesc_f16_kk(128, 4 * NB);
     P.idesc_lo = umma_idesc_f16_kk(128, 2 * NB);
     P.inv_sA = inv_sA;
     P.amax = amax_dev;
-    const size_t smem = (size_t)fixed + (size_t)P.sa * C::STAGE_BYTES;
+    const size_t smem = (size_t)fixed + (size_t)C::GMAX * P.sa * C::STAGE_BYTES;
 
     if (!have_colmax) {
         CMRHS_CUDA(cudaMemsetAsync(amax_dev, 0, 64 * sizeof(uint32_t), stream));
@@ -466,7 +522,7 @@ int launch_stencil_h16x(const unsigned char *Ax, float inv_sA, uint32_t *amax_de
     auto kern = stencil_h16x_kernel<NB>;
     CMRHS_SMEM_ATTR(kern, smem);
     const int grid = P.ngroups < num_sms ? P.ngroups : num_sms;
-    kern<<<grid, kXThreads, smem, stream>>>(Ax, Xh, static_cast<float *>(Y), P);
+    kern<<<grid, C::THREADS, smem, stream>>>(Ax, Xh, static_cast<float *>(Y), P);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }
