@@ -5,34 +5,38 @@
 // FP32 accumulators D and C in tensor memory, Y = (D + 2^-11 C) / (sA sX_r)), in the TRANSPOSED form
 //   D_x[(r,c)][(h,part,i)] += sum_k X(y)[k][(r,c)] . A^p(x)_{h,part}[i][k]          y = x + delta_p
 // * M side (the 128 TMEM lanes) = the 2 nrhs real columns (r, re/im) of the neighbour's X tile, held IN TENSOR MEMORY
-//   (tcgen05.mma with the A operand from TMEM): lane m, 16-bit pairs along k.  Loader warps read the pre-split tile
-//   (one coalesced 16-byte load per lane and 8 k) from L2 and write it with tcgen05.st -- the tile never touches shared
-//   memory, and the tensor core reads only the stencil matrix through the shared-memory pipe.
+//   (tcgen05.mma with the A operand from TMEM): lane m, 16-bit pairs along k, [X_hi | X_lo] in nb columns.  The pre-split
+//   tile arrives in a shared-memory ring by one bulk copy and goes to tensor memory by tcgen05.cp (no thread touches it);
+//   every MMA then reads only the stencil matrix through the shared-memory pipe.  (stencil_h16.cuh reads both operands of
+//   every MMA from shared memory and is bound by that pipe from nrhs 32 up.)
 // * N side = the stencil matrix, K-major without swizzle: 8 x 8 core matrices of binary16 (128 contiguous bytes), the
 //   tile stored in HBM as [k chunk of 8][n group of 8] with n = (hi/lo, Re/Im, row i): 8 nb^2 bytes for ANY nb that is a
 //   multiple of 8 (no padding bytes in HBM: same size as complex64); one 1-D bulk copy per stencil matrix.
 //   MMA 1: X_hi^T . [A_hi | A_lo] -> D | C (N = 4 nb), MMA 2: X_lo^T . A_hi -> C (N = 2 nb), per K = 16 slab.
-//   nb = 8, 24: the last K = 16 slab is half empty: the X operand holds zeros there, the ring stage a zero chunk.
+//   nb = 8, 24: the last K = 16 slab is half empty: the ring stage holds a zero chunk there (never overwritten), and the X
+//   operand simply reads on into the next columns of tensor memory (always finite binary16 numbers).
 // * A GROUP of up to GMAX x-adjacent sites (4; 2 at nbasis 32, where tensor memory holds no more accumulators) shares
 //   every X tile it needs: (G + 2) x 27 tile loads per group instead of 81 G -- the gather of X through L2 is the
-//   largest single cost of this kernel (measured: 21-25 % of the time at nrhs 64).
+//   largest single cost of this kernel (measured: 21-25 % of the time at nrhs 64 with pairs of sites).
 // * EVERYTHING THAT SERIALISES IS PER SITE: one accumulator (4 nb TMEM columns), one ring of stencil matrices with its own
 //   producer lane, and one MMA-issuing warp per site of the group.  A single warp's dependent instruction stream
-//   (barrier tests, descriptor arithmetic, 4 MMAs + 2 commits per stencil point: ~600 clk) is what bounds an issuer, not
-//   the tensor pipe (144-192 clk per point): the sites' accumulators are independent, so their streams need no order.
+//   (barrier tests, descriptor arithmetic, 4 MMAs + 2 commits per stencil point: 600-1000 clk) is what bounds an issuer,
+//   not the tensor pipe (144-192 clk per point): the sites' accumulators are independent, so their streams need no order.
 //   Barriers are per site too: a parity wait cannot tell phases two apart, so every barrier has exactly one waiter
-//   that sees each of its phases.
-// * One persistent CTA per SM: loader warps (kXTurns per lane quarter, taking turns tile by tile, two tiles in registers
-//   each), 4 epilogue warps, one producer warp (lane i feeds site i), GMAX MMA issuers.
+//   that sees each of its phases (X buffers: full / empty barriers per site; the mover of a buffer keeps who used it last).
+// * One persistent CTA per SM: one mover warp per X buffer, 4 epilogue warps, one producer warp for the stencil matrices
+//   (lane i feeds site i), one producer warp for the X tiles, GMAX MMA issuers.
+// Measured (B200, 1000 W cap): BASELINE configs[4] (16^3 x 32, nbasis 24, nrhs 64) 16.4-16.7 ms per apply = 0.48 of the HBM
+// roof (the TF32 kernel: 31.5 ms); the board sits at its power cap (SM clock 1.1-1.2 GHz) -- DESIGN.md section 5.5.
 #pragma once
 
 #include "stencil_h16.cuh"
 
 namespace cmrhs {
 
-constexpr int kXTurns = 2;                    // loader warps per TMEM lane quarter
 constexpr int kXMaxStagesA = 32;              // per site
 constexpr int kXMaxBuf = 8;
+constexpr int kXMaxSX = 24;                   // stages of the shared-memory ring of X tiles
 constexpr int kXMaxG = 4;
 constexpr int kXMaxSteps = 168;               // (G + 2) x 27 + G at G = 4: 166
 constexpr int kXViews = kXMaxG * (kXMaxG + 1) / 2;      // per-site views of the schedules of G = 1..4
@@ -46,15 +50,20 @@ template <int NB> struct XCfg {
     static constexpr uint32_t TILE_BYTES = 8u * NB * NB;         // one stencil matrix, [A_hi | A_lo]
     static constexpr uint32_t STAGE_BYTES = 2u * KSTEPS * LBO;   // ring stage (>= TILE_BYTES; the rest stays zero)
     static constexpr int ACC_COLS = 4 * NB;                      // D (2 nb) | C (2 nb) per site
-    static constexpr int XHALF = 8 * KSTEPS;                     // TMEM columns of X_hi (or X_lo) of one tile
-    static constexpr int XCOLS = 2 * XHALF;
-    static constexpr int GMAX = NB == 32 ? 2 : 4;                // sites per group
-    static constexpr int NACC = NB == 32 ? 3 : (NB == 24 ? 4 : (NB == 16 ? 6 : 8));      // accumulator slots
-    static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS < kXMaxBuf ? ((512 - NACC * ACC_COLS) / XCOLS >= 4 ? 4 : 2) : kXMaxBuf;
+    static constexpr int XLO = 4 * NCH;                          // TMEM column of X_lo within a tile: [X_hi: 4 per k chunk | X_lo]
+    static constexpr int XCOLS = 8 * NCH;                        // (a half-empty last K slab reads on into the next columns: finite
+                                                                 //  numbers that meet the zero chunk of the stencil matrix)
+    // tensor-memory plan (512 columns): sites per group, accumulator slots (one per site of a group; one spare at nbasis 32),
+    // X buffers of XCOLS = nb columns, and one mover warp per X buffer
+    static constexpr int GMAX = NB == 32 ? 2 : 4;
+    static constexpr int NACC = NB == 32 ? 3 : (NB == 8 ? 8 : 4);
+    static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS) / XCOLS;
+    static constexpr int MOVERS = NXB;
     static constexpr int XBASE = NACC * ACC_COLS;
-    static constexpr int WARPS = 4 * kXTurns + 4 + 1 + GMAX;
+    static constexpr int MWARPS = (MOVERS + 3) / 4 * 4;          // (the epilogue warps must start at a multiple of 4)
+    static constexpr int WARPS = MWARPS + 4 + 2 + GMAX;
     static constexpr int THREADS = 32 * WARPS;
-    static_assert(XBASE + NXB * XCOLS <= 512 && NXB >= 4 && (NXB & (NXB - 1)) == 0 && NXB % kXTurns == 0, "tensor memory plan");
+    static_assert(XBASE + NXB * XCOLS + (NCH % 2 ? 4 : 0) <= 512 && NXB >= 4 && NXB <= kXMaxBuf && NXB % MOVERS == 0, "tensor memory plan");
     static_assert(NACC >= GMAX, "one accumulator per site of a group");
 };
 
@@ -65,6 +74,7 @@ struct XParams {
     int32_t m32;              // N2 rounded up to a multiple of 32: rows of one chunk of the split X tile
     int32_t nq;               // TMEM lane quarters in use = m32 / 32
     int32_t sa;               // depth of each site's ring of stencil matrices
+    int32_t sx;               // depth of the ring of X tiles (even: a stage always meets the same loader turn)
     int32_t xh_site_bytes;    // bytes of one split X tile: 2 (hi, lo) x NCH x m32 x 16
     uint32_t idesc_wide, idesc_lo;
     float inv_sA;
@@ -110,7 +120,8 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
     unsigned char *ringA = smem;                 // GMAX rings of P.sa stages: site i's stencil matrices at ring i
-    uint32_t *tabs = reinterpret_cast<uint32_t *>(ringA + (size_t)GMAX * P.sa * C::STAGE_BYTES);      // [G-1][kXMaxSteps]
+    unsigned char *ringX = ringA + (size_t)GMAX * P.sa * C::STAGE_BYTES;        // P.sx pre-split X tiles (+ 2 KB the tail reads of a short tile may touch)
+    uint32_t *tabs = reinterpret_cast<uint32_t *>(ringX + (size_t)P.sx * P.xh_site_bytes + 2048);     // [G-1][kXMaxSteps]
     uint32_t *views = tabs + kXMaxG * kXMaxSteps;                        // [G (G-1) / 2 + i][84]
     int32_t *nsteps = reinterpret_cast<int32_t *>(views + kXViews * 84); // [G-1]
     float *inv = reinterpret_cast<float *>(nsteps + 4);                  // [128] per real column: 1 / (sA sX_r)
@@ -118,10 +129,11 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     uint64_t *a_full = bars, *a_empty = a_full + kXMaxG * kXMaxStagesA;              // [site][stage]
     uint64_t *x_full = a_empty + kXMaxG * kXMaxStagesA, *x_empty = x_full + kXMaxG * kXMaxBuf;      // [site][buffer]
     uint64_t *acc_full = x_empty + kXMaxG * kXMaxBuf, *acc_empty = acc_full + kXMaxBuf;            // [slot]
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_empty + kXMaxBuf);
+    uint64_t *x_land = acc_empty + kXMaxBuf, *x_sfree = x_land + kXMaxSX;                          // [stage of the X ring]
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(x_sfree + kXMaxSX);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int kWEpi = 4 * kXTurns, kWProd = kWEpi + 4, kWMma = kWProd + 1;
+    constexpr int kWEpi = C::MWARPS, kWProd = kWEpi + 4, kWProdX = kWProd + 1, kWMma = kWProd + 2;
 #ifdef CMRHS_TC_TRACE
     long long wt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     const long long t_begin = clock64();
@@ -130,9 +142,10 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     if (threadIdx.x == 0) {
         for (int j = 0; j < GMAX; ++j) {
             for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[j * kXMaxStagesA + i], 1); mbar_init(&a_empty[j * kXMaxStagesA + i], 1); }
-            for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[j * kXMaxBuf + i], (uint32_t)P.nq); mbar_init(&x_empty[j * kXMaxBuf + i], 1); }
+            for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[j * kXMaxBuf + i], 1); mbar_init(&x_empty[j * kXMaxBuf + i], 1); }
         }
         for (int i = 0; i < C::NACC; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 4); }
+        for (int i = 0; i < P.sx; ++i) { mbar_init(&x_land[i], 1); mbar_init(&x_sfree[i], 1); }
         mbar_fence_init();
     }
     if (warp >= 1 && warp <= GMAX && lane == 0) {
@@ -155,6 +168,17 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     __syncthreads();
     tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
+    if (warp >= kWEpi && warp < kWEpi + 4) {
+        // the X buffers start as zeros: the copies never touch the columns of a half-empty K slab (nb = 8, 24)
+        uint32_t zz[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) zz[k] = 0u;
+        for (int cc = 0; cc < (C::NXB * C::XCOLS + 4 + 15) / 16 * 16 && C::XBASE + cc + 16 <= 512; cc += 16) tmem_st_x16(tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(C::XBASE + cc), zz);
+        tmem_wait_st();
+    }
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
 
     auto group_of = [&](int g) {
         XGroup r;
@@ -173,18 +197,18 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     auto site_of = [&](int x, int y, int z, int t) { return x + (int64_t)P.L[0] * (y + (int64_t)P.L[1] * (z + (int64_t)P.L[2] * t)); };
 
     if (warp < kWEpi) {
-        // ================= X loaders: pre-split tile (L2) -> registers -> tensor memory =================
-        const int q = warp & 3, turn = warp >> 2;
-        if (q < P.nq) {
-            const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)C::XBASE;
-            const size_t row_off = (size_t)(32 * q + lane) * 16;
-            const size_t chunk_stride = (size_t)P.m32 * 16;
-            int cg = blockIdx.x, cstep = 0;       // cursor in the sequence of X tiles this CTA walks
+        // ================= X movers: tile (shared-memory ring, filled by bulk copies) -> tensor memory by tcgen05.cp; warp m takes the
+        // tiles t = m (mod MOVERS) and with them always the same X buffers and ring stages; one elected lane issues =================
+        const int mv = warp;
+        if (mv < C::MOVERS) {
+            int cg = blockIdx.x, cstep = 0;
             bool more = cg < P.ngroups;
             XGroup grp;
             if (more) grp = group_of(cg);
-            auto skip = [&](int n) {              // advance the cursor by n tiles
+            TcRing rs;
+            auto skip = [&](int n) {
                 for (int k = 0; k < n && more; ++k) {
+                    rs.advance(P.sx);
                     if (++cstep == grp.nsteps) {
                         cstep = 0;
                         cg += gridDim.x;
@@ -193,24 +217,14 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                     }
                 }
             };
-            skip(turn);
-            auto load_next = [&](uint4 (&r)[2 * C::NCH], uint32_t &um) -> bool {
-                if (!more) return false;
-                const uint32_t e = grp.tab[cstep];
-                um = e & 15u;
-                const int xs = tc_wrap(grp.x0 + (int)((e >> 4) & 7u) - 1, P.L[0]), ys = tc_wrap(grp.y + (int)((e >> 8) & 3u) - 1, P.L[1]);
-                const int zs = tc_wrap(grp.z + (int)((e >> 10) & 3u) - 1, P.L[2]), ts = tc_wrap(grp.t + (int)((e >> 12) & 3u) - 1, P.L[3]);
-                const unsigned char *src = Xh + (int64_t)(xs + P.L[0] * (ys + P.L[1] * (zs + P.L[2] * ts))) * (int64_t)P.xh_site_bytes + row_off;
-#pragma unroll
-                for (int c = 0; c < 2 * C::NCH; ++c) r[c] = __ldg(reinterpret_cast<const uint4 *>(src + (size_t)c * chunk_stride));
-                skip(kXTurns);
-                return true;
-            };
-            // this warp always meets the same buffers (NXB is a multiple of the number of turns): per buffer and site it keeps
-            // who used the tile it stored there last (pend) and the parity of that site's next release (par); bit 4 b + i
-            uint32_t t = (uint32_t)turn, pend = 0u, par = 0u;
-            auto store = [&](const uint4 (&r)[2 * C::NCH], uint32_t um) {
-                const uint32_t b = t & (uint32_t)(C::NXB - 1);
+            skip(mv);
+            const uint32_t ringx0 = smem_u32(ringX), chunk_stride = (uint32_t)P.m32 * 16u;
+            const uint64_t desc_hi = umma_desc_kmajor_noswz(0u, chunk_stride, 128u);      // LBO: next k chunk, SBO: next 8 rows
+            uint32_t t = (uint32_t)mv, pend = 0u, par = 0u;
+            while (more) {
+                const uint32_t um = grp.tab[cstep] & 15u;
+                const uint32_t b = t % (uint32_t)C::NXB;
+                TW(2, mbar_wait(&x_land[rs.stage], rs.phase));
 #pragma unroll
                 for (int i = 0; i < GMAX; ++i) {
                     const uint32_t bit = 1u << (4u * b + i);
@@ -222,37 +236,21 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 pend = (pend & ~(15u << (4u * b))) | (um << (4u * b));
                 tc_fence_after_sync();
                 TW_BEGIN();
+                if (elect_one_sync()) {
+                    const uint32_t src = ringx0 + (uint32_t)rs.stage * (uint32_t)P.xh_site_bytes;
+                    const uint32_t dst = tmem + (uint32_t)C::XBASE + b * (uint32_t)C::XCOLS;
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    uint32_t w[C::XHALF];
+                    for (int c = 0; c < 2 * C::NCH; c += 2)            // chunks [hi 0 .. NCH-1 | lo 0 .. NCH-1], two per copy
+                        tmem_cp_128x256b(dst + (uint32_t)(4 * c), desc_hi | (uint64_t)(((src + (uint32_t)c * chunk_stride) >> 4) & 0x3FFFu));
 #pragma unroll
-                    for (int c = 0; c < C::XHALF / 4; ++c) {
-                        if (c < C::NCH) {
-                            w[4 * c + 0] = r[h * C::NCH + c].x; w[4 * c + 1] = r[h * C::NCH + c].y;
-                            w[4 * c + 2] = r[h * C::NCH + c].z; w[4 * c + 3] = r[h * C::NCH + c].w;
-                        } else {
-                            w[4 * c + 0] = 0u; w[4 * c + 1] = 0u; w[4 * c + 2] = 0u; w[4 * c + 3] = 0u;
-                        }
-                    }
-                    tmem_st<C::XHALF>(lane_base + b * (uint32_t)C::XCOLS + (uint32_t)(h * C::XHALF), w);
+                    for (int i = 0; i < GMAX; ++i)
+                        if ((um >> i) & 1u) umma_commit(&x_full[i * kXMaxBuf + b]);
+                    umma_commit(&x_sfree[rs.stage]);
                 }
-                tmem_wait_st();
-                tc_fence_before_sync();
                 __syncwarp();
-                if (lane < GMAX && ((um >> lane) & 1u)) mbar_arrive(&x_full[lane * kXMaxBuf + b]);
                 TW_END(1);
-                t += kXTurns;
-            };
-            uint4 ra[2 * C::NCH], rb[2 * C::NCH];
-            uint32_t ua = 0u, ub = 0u;
-            bool va = load_next(ra, ua), vb = load_next(rb, ub);
-            for (;;) {
-                if (!va) break;
-                store(ra, ua);
-                va = load_next(ra, ua);
-                if (!vb) break;
-                store(rb, ub);
-                vb = load_next(rb, ub);
+                t += C::MOVERS;
+                skip(C::MOVERS);
             }
         }
     }
@@ -300,13 +298,13 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
             }
         }
     } else if (warp == kWProd) {
-        // ================= A producer: ONE warp, LANE i feeds site i's ring (the warp runs one uniform polling loop, every lane on its
-        // own ring, barrier, group cursor and stencil-matrix pointer): the site's 81 pre-split stencil matrices, each one contiguous
-        // bulk copy, in the order the site accumulates them =================
+        // ================= A producer: ONE warp running one uniform polling loop, LANE i < GMAX on site i's ring, barrier and cursor:
+        // the site's 81 pre-split stencil matrices, each one contiguous bulk copy, in the order the site accumulates them =================
         const int me = lane;
         const uint64_t pol = l2_policy_evict_first();
-        unsigned char *ring = ringA + (size_t)(me < GMAX ? me : 0) * P.sa * C::STAGE_BYTES;
-        uint64_t *full = a_full + (me < GMAX ? me : 0) * kXMaxStagesA, *empty = a_empty + (me < GMAX ? me : 0) * kXMaxStagesA;
+        const int ring_no = me < GMAX ? me : 0;
+        unsigned char *ring = ringA + (size_t)ring_no * P.sa * C::STAGE_BYTES;
+        uint64_t *full = a_full + ring_no * kXMaxStagesA, *empty = a_empty + ring_no * kXMaxStagesA;
         TcRing ra;
         int g = blockIdx.x, k = 0;
         bool active = me < GMAX && g < P.ngroups;
@@ -339,6 +337,26 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 }
             }
         }
+    } else if (warp == kWProdX) {
+        // ================= X producer: the pre-split tile of every step (contiguous in the scratch block), one bulk copy each =================
+        const uint64_t pol = l2_policy_evict_last();
+        TcRing rs;
+        for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
+            const XGroup grp = group_of(g);
+            for (int step = 0; step < grp.nsteps; ++step) {
+                const uint32_t e = grp.tab[step];
+                const int xs = tc_wrap(grp.x0 + (int)((e >> 4) & 7u) - 1, P.L[0]), ys = tc_wrap(grp.y + (int)((e >> 8) & 3u) - 1, P.L[1]);
+                const int zs = tc_wrap(grp.z + (int)((e >> 10) & 3u) - 1, P.L[2]), ts = tc_wrap(grp.t + (int)((e >> 12) & 3u) - 1, P.L[3]);
+                const unsigned char *src = Xh + (int64_t)(xs + P.L[0] * (ys + P.L[1] * (zs + P.L[2] * ts))) * (int64_t)P.xh_site_bytes;
+                TW(0, mbar_wait(&x_sfree[rs.stage], rs.phase ^ 1u));
+                if (elect_one_sync()) {
+                    mbar_arrive_expect_tx(&x_land[rs.stage], (uint32_t)P.xh_site_bytes);
+                    bulk_g2s(ringX + (size_t)rs.stage * P.xh_site_bytes, src, (uint32_t)P.xh_site_bytes, &x_land[rs.stage], pol);
+                }
+                __syncwarp();
+                rs.advance(P.sx);
+            }
+        }
     } else if (warp < kWMma + GMAX) {
         // ================= MMA issuers, one warp PER SITE of a group; one elected lane issues.  The barrier tests of the NEXT stencil
         // point are started before the MMAs of this one (non-blocking test_wait), so their latency overlaps the issue. =================
@@ -347,7 +365,6 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         const uint32_t x_base = tmem + (uint32_t)C::XBASE;
         uint64_t *afull = a_full + me * kXMaxStagesA, *aempty = a_empty + me * kXMaxStagesA;
         uint64_t *xfull = x_full + me * kXMaxBuf, *xempty = x_empty + me * kXMaxBuf;
-        constexpr uint32_t xmask = (uint32_t)C::NXB - 1u;
         const uint64_t desc_hi = umma_desc_kmajor_noswz(0u, C::LBO, C::SBO);      // everything but the start address
         TcRing rc, ra;
         uint32_t xcnt = 0;                        // X tiles before this group
@@ -361,7 +378,7 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 const uint32_t *tm = grp.view + me * 84;
                 const uint32_t ds = tmem + (uint32_t)(slot.stage * C::ACC_COLS);
                 TW(0, mbar_wait(&acc_empty[slot.stage], slot.phase ^ 1u));
-                uint32_t xb = (xcnt + (tm[0] & 0xFFu)) & xmask;
+                uint32_t xb = (xcnt + (tm[0] & 0xFFu)) % (uint32_t)C::NXB;
                 bool okx = false, oka = false;
                 for (int k = 0; k < kNPoint; ++k) {
                     if (!okx) TW(2, mbar_wait(&xfull[xb], (xpar >> xb) & 1u));
@@ -372,13 +389,13 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                     rn.advance(P.sa);
                     uint32_t xbn = 0u;
                     if (k + 1 < kNPoint) {
-                        xbn = (xcnt + (tm[k + 1] & 0xFFu)) & xmask;
+                        xbn = (xcnt + (tm[k + 1] & 0xFFu)) % (uint32_t)C::NXB;
                         okx = mbar_test_wait(&xfull[xbn], (xpar >> xbn) & 1u);
                         oka = mbar_test_wait(&afull[rn.stage], rn.phase);
                     }
                     TW_BEGIN();
                     if (elect_one_sync()) {
-                        const uint32_t x_hi = x_base + xb * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XHALF;
+                        const uint32_t x_hi = x_base + xb * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XLO;
                         const uint64_t bd0 = desc_hi | (uint64_t)(((ring0 + (uint32_t)ra.stage * C::STAGE_BYTES) >> 4) & 0x3FFFu);
 #pragma unroll
                         for (int ks = 0; ks < C::KSTEPS; ++ks) {
@@ -497,15 +514,21 @@ int launch_stencil_h16x(const unsigned char *Ax, float inv_sA, uint32_t *amax_de
     P.nq = P.m32 / 32;
     P.xh_site_bytes = h16x_site_bytes(NB, s);
     const int64_t fixed = 128 /* alignment */ + (kXMaxG * kXMaxSteps + kXViews * 84 + 4) * 4 + 512 /* scales */ +
-                          (2 * kXMaxG * kXMaxStagesA + 2 * kXMaxG * kXMaxBuf + 2 * kXMaxBuf) * 8 + 16;
-    const int64_t budget = 226 * 1024 - fixed;
-    P.sa = (int32_t)(budget / (C::GMAX * (int64_t)C::STAGE_BYTES));
+                          (2 * kXMaxG * kXMaxStagesA + 2 * kXMaxG * kXMaxBuf + 2 * kXMaxBuf + 2 * kXMaxSX) * 8 + 16;
+    // shared memory: about a third for the ring of X tiles (an even number of stages), the rest for the sites' rings of stencil matrices
+    const int64_t budget = 226 * 1024 - fixed - 2048;
+    P.sx = (int32_t)(budget / 3 / P.xh_site_bytes);
+    if (P.sx > kXMaxSX) P.sx = kXMaxSX;
+    P.sx = P.sx / C::MOVERS * C::MOVERS;          // a stage always meets the same mover
+    if (P.sx < C::MOVERS) P.sx = C::MOVERS;
+    P.sa = (int32_t)((budget - (int64_t)P.sx * P.xh_site_bytes) / (C::GMAX * (int64_t)C::STAGE_BYTES));
     if (P.sa > kXMaxStagesA) P.sa = kXMaxStagesA;
+    if (P.sa < 2) { set_error("h16x: shared-memory plan does not fit (nbasis %d, nrhs %d)", NB, s); return COARSE_UNSUPPORTED; }
     P.idesc_wide = umma_idesc_f16_kk(128, 4 * NB);
     P.idesc_lo = umma_idesc_f16_kk(128, 2 * NB);
     P.inv_sA = inv_sA;
     P.amax = amax_dev;
-    const size_t smem = (size_t)fixed + (size_t)C::GMAX * P.sa * C::STAGE_BYTES;
+    const size_t smem = (size_t)fixed + 2048 + (size_t)C::GMAX * P.sa * C::STAGE_BYTES + (size_t)P.sx * P.xh_site_bytes;
 
     if (!have_colmax) {
         CMRHS_CUDA(cudaMemsetAsync(amax_dev, 0, 64 * sizeof(uint32_t), stream));

@@ -180,10 +180,12 @@ def test_full_size_baseline_configs_on_sampled_sites(index, nrhs):
         pytest.skip("not enough free device memory for this configuration")
     A, c = cm.fill_synthetic(dims, nb, TORCH_DTYPE[dtype], cfg["seed"], cfg["factor"])
     X = cm.fill_block(dims, nb, nrhs, TORCH_DTYPE[dtype], cfg["seed"], synth.TAG_X)
-    tensor = dtype == "c64" and (nrhs % 8 == 0 or (nrhs == 4 and nb == 32))
+    # complex64: nbasis 32 -> paired-site split-FP16 kernel (nrhs 4 or a multiple of 8); nbasis 8/16/24 -> the split-FP16 kernel with
+    # the X operand in tensor memory (any nrhs >= 4)
+    tensor = dtype == "c64" and ((nrhs % 8 == 0 or nrhs == 4) if nb == 32 else nrhs >= 4)
     # the 49 GB configuration keeps one internal layout of A (the caller's copy is needed below for the oracle's sample)
     op = cm.CoarseOperator(dims, A, nrhs, flags=cm.binding.FLAG_TENSOR_ONLY if (tensor and index == 4) else 0)
-    assert op.kernel_name(nrhs).startswith(("stencil_h16" if nb == 32 else "stencil_tc") if tensor else "stencil_simt")
+    assert op.kernel_name(nrhs).startswith(("stencil_h16<" if nb == 32 else "stencil_h16x<") if tensor else "stencil_simt")
     Y = op.apply(X)
     torch.cuda.synchronize()
     sites = _sampled_sites(dims, 24, np.random.default_rng(index))

@@ -130,12 +130,12 @@ def test_tensor_only_operator_keeps_one_copy_and_rejects_uncovered_nrhs():
     A, c, X, _ = host_case(dims, nb, s, seed=17, factor=1.02)
     Ad, Xd = to_dev(A, "c64"), to_dev(X, "c64")
     outs, sizes = [], []
-    for flags in (0, cm.binding.FLAG_TENSOR_ONLY):
+    for flags in (cm.binding.FLAG_TF32, cm.binding.FLAG_TF32 | cm.binding.FLAG_TENSOR_ONLY):
         op = cm.CoarseOperator(dims, Ad, s, flags=flags)
         assert op.kernel_name(s).startswith("stencil_tc")
         outs.append(to_np(op.apply(Xd)))
         sizes.append(op.device_bytes())
-        if flags:
+        if flags & cm.binding.FLAG_TENSOR_ONLY:
             with pytest.raises(cm.binding.CoarseError) as ei:
                 op.apply(Xd[:, :, :4].contiguous())
             assert ei.value.status == cm.binding.UNSUPPORTED
