@@ -287,6 +287,15 @@ int coarse_fill_block(void *X_dev, const int32_t dims[4], int32_t nbasis, int32_
  * has launched in this process so far (monotonic; used for bench.py's gpu_launches). */
 const char *coarse_op_kernel_name(const coarse_op_t *op, int32_t nrhs);
 int64_t coarse_op_device_bytes(const coarse_op_t *op);
+/*
+ * coarse_measure_peaks -- bench helper: roofline denominators measured on the current device.
+ *   out_host[0] read-only HBM stream GB/s (the stencil operator is read once and never written: a copy is the wrong roof),
+ *   out_host[1] FFMA, [2] packed FFMA2, [3] DFMA, [4] DMMA (mma.sync m8n8k4) TFLOP/s of register-resident loops.
+ *   nout >= 5; scratch_dev: device block of scratch_bytes >= 256 MiB (larger than L2 for a meaningful stream figure; its
+ *   contents are read, its first 256 bytes may be written).  Synchronises `stream`.  Nothing on the product path calls it.
+ */
+int coarse_measure_peaks(double *out_host, int32_t nout, void *scratch_dev, int64_t scratch_bytes, void *stream);
+
 int64_t coarse_launch_count(void);
 
 /* Per-launch device timing of the stencil kernel (measurement aid for bench.py's roofline object):

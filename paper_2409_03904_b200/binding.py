@@ -26,7 +26,7 @@ EXPORTS = [
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
     "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve", "stacked_cg_solve", "coarse_block_project", "coarse_block_promote",
-    "block_cg_solve_ex", "block_cg_solve_host_ex",
+    "block_cg_solve_ex", "block_cg_solve_host_ex", "coarse_measure_peaks",
 ]
 
 
@@ -94,6 +94,7 @@ def lib():
             "stacked_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(BlockCGResult), vp]),
             "pblock_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(CoarsePrecond), C.POINTER(BlockCGResult), vp]),
             "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
+            "coarse_measure_peaks": (C.c_int, [C.POINTER(dbl), i32, vp, i64, vp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -133,6 +134,15 @@ def _dev(t: torch.Tensor) -> int:
 
 def launch_count() -> int:
     return int(lib().coarse_launch_count())
+
+
+def measure_peaks(scratch_bytes: int = 4 << 30, stream=None) -> dict:
+    """coarse_measure_peaks on the current device: read-only HBM stream GB/s and FFMA / FFMA2 / DFMA / DMMA TFLOP/s."""
+    scratch = torch.randint(0, 2 ** 31 - 1, (int(scratch_bytes) // 4,), dtype=torch.int32, device="cuda")
+    out = (C.c_double * 5)()
+    _check(lib().coarse_measure_peaks(out, 5, _dev(scratch), C.c_int64(scratch.numel() * 4), _stream(stream)))
+    del scratch
+    return dict(hbm_read_gbs=out[0], ffma_tflops=out[1], ffma2_tflops=out[2], dfma_tflops=out[3], dmma_tflops=out[4])
 
 
 class CoarseOperator:

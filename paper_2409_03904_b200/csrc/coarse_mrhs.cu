@@ -20,6 +20,7 @@
 #include "stencil_tc.cuh"
 #include "stencil_h16.cuh"
 #include "stencil_h16x.cuh"
+#include "peaks.cuh"
 
 namespace cmrhs {
 
@@ -1387,6 +1388,66 @@ extern "C" int coarse_block_promote(const void *Basis_dev, const void *C_dev, vo
     CMRHS_STEP(transfer_check(Basis_dev, C_dev, F_dev, Vc, vblock, nbasis, nrhs, dtype));
     return dtype == COARSE_C64 ? transfer_launch<float>(false, Basis_dev, C_dev, F_dev, Vc, vblock, nbasis, nrhs, (cudaStream_t)stream)
                                : transfer_launch<double>(false, Basis_dev, C_dev, F_dev, Vc, vblock, nbasis, nrhs, (cudaStream_t)stream);
+}
+
+// ---- roofline denominators measured on this device (bench helper) -----------------------------------
+template <int KIND>
+static int time_alu_peak(int num_sms, double flops_per_thread_iter, double *sink_dev, cudaStream_t stream, cudaEvent_t e0, cudaEvent_t e1, double *tflops)
+{
+    const int iters = 4096, grid = num_sms * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CMRHS_CUDA(cudaEventRecord(e0, stream));
+        peak_alu_kernel<KIND><<<grid, threads, 0, stream>>>(iters, 1.0f + rep, sink_dev);
+        CMRHS_LAUNCH_CHECK();
+        CMRHS_CUDA(cudaEventRecord(e1, stream));
+        CMRHS_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CMRHS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        const double tf = flops_per_thread_iter * iters * (double)grid * threads / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    *tflops = best;
+    return COARSE_OK;
+}
+
+extern "C" int coarse_measure_peaks(double *out_host, int32_t nout, void *scratch_dev, int64_t scratch_bytes, void *stream_v)
+{
+    if (!out_host || nout < 5 || !scratch_dev || scratch_bytes < (int64_t)1 << 28) {
+        set_error("coarse_measure_peaks: need out[>=5] and a device scratch block of at least 256 MiB");
+        return COARSE_INVALID_ARG;
+    }
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    int dev = 0, num_sms = 0;
+    CMRHS_CUDA(cudaGetDevice(&dev));
+    CMRHS_CUDA(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev));
+    cudaEvent_t e0, e1;
+    CMRHS_CUDA(cudaEventCreate(&e0));
+    CMRHS_CUDA(cudaEventCreate(&e1));
+    uint32_t *sink = static_cast<uint32_t *>(scratch_dev);               // first 256 bytes: sinks of the kernels
+    const uint4 *buf = reinterpret_cast<const uint4 *>(static_cast<unsigned char *>(scratch_dev) + 256);
+    const int64_t n16 = (scratch_bytes - 256) / 16;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {                                   // read-only stream, best of 5 after one warm-up
+        CMRHS_CUDA(cudaEventRecord(e0, stream));
+        peak_read_kernel<<<num_sms * 16, 256, 0, stream>>>(buf, n16, sink);
+        CMRHS_LAUNCH_CHECK();
+        CMRHS_CUDA(cudaEventRecord(e1, stream));
+        CMRHS_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CMRHS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        const double gbs = (double)n16 * 16.0 / (ms * 1e-3) / 1e9;
+        if (rep > 0 && gbs > best) best = gbs;
+    }
+    out_host[0] = best;
+    double *dsink = reinterpret_cast<double *>(sink) + 8;
+    int st = time_alu_peak<0>(num_sms, 16 * 2.0, dsink, stream, e0, e1, &out_host[1]);                      // FFMA
+    if (st == COARSE_OK) st = time_alu_peak<1>(num_sms, 16 * 4.0, dsink, stream, e0, e1, &out_host[2]);     // FFMA2
+    if (st == COARSE_OK) st = time_alu_peak<2>(num_sms, 16 * 2.0, dsink, stream, e0, e1, &out_host[3]);     // DFMA
+    if (st == COARSE_OK) st = time_alu_peak<3>(num_sms, 16 * 512.0 / 32.0, dsink, stream, e0, e1, &out_host[4]);   // DMMA m8n8k4: 512 flops per warp
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return st;
 }
 
 extern "C" int coarse_op_profile(coarse_op_t *op, int32_t enable)
