@@ -72,6 +72,7 @@ enum {
 
 #define COARSE_MAX_NRHS 64
 #define COARSE_MAX_NBASIS 64
+#define COARSE_MAX_NEV 4096 /* eigenvectors of coarse_deflate (the paper: several hundred to 1000) */
 
 /*
  * coarse_op_create -- build the operator object.  "The coarse matrix coefficients are stored entirely
@@ -167,10 +168,11 @@ int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t 
 /*
  * coarse_deflate -- multi-RHS deflation with n_ev eigenpairs of the operator (Eq. 7-10; "applied to
  * multiple right-hand sides"):  C = Vev^H B;  QBpar = Vev (C / lambda) = (sum_i |i><i| / lambda_i) b;
- * Bperp = B - Vev C = (1 - sum_i |i><i|) b.  Two tall-skinny products: a deterministic two-stage reduction (complex128
- * sums) and one pass over Vev and B.
+ * Bperp = B - Vev C = (1 - sum_i |i><i|) b.  Tall-skinny products, eigenvectors taken in chunks of min(64, nrhs_max)
+ * columns (chunk j projects the running Bperp: the columns are orthonormal): per chunk a deterministic two-stage reduction
+ * (complex128 sums) and one pass over the chunk and the block.
  *   Vev_dev     : [V*nbasis][nev] device block of the operator's dtype, eigenvector index fastest, orthonormal columns
- *   lambda_host : [nev] HOST doubles, all > 0;  1 <= nev <= nrhs_max (<= 64) this round
+ *   lambda_host : [nev] HOST doubles, all > 0;  1 <= nev <= COARSE_MAX_NEV (the paper deflates with 192-1000 vectors)
  *   B_dev       : [V][nb][nrhs];  QBpar_dev, Bperp_dev: outputs of the same shape, QBpar != B, QBpar != Bperp (Bperp may alias B)
  * coarse_cheby_defl_solve -- the paper's stationary coarse solve  X = Defl(b_par) + P^Cheby(b_perp)  (Eq. 11-12), P as in
  * coarse_cheby_apply.  Asynchronous on `stream`; both use the handle's block-CG workspace.

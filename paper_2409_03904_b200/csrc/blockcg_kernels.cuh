@@ -518,8 +518,8 @@ struct DeflLambda { double inv[COARSE_MAX_NRHS]; };      // 1 / lambda_i, passed
 
 template <typename T>
 __global__ void __launch_bounds__(kLaThreads)
-rgram_partial_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict__ B, int64_t n, int m, int s, int rows_per_tile,
-                     zdouble *__restrict__ partial)
+rgram_partial_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *__restrict__ B, int64_t n, int m, int s, int rows_per_tile,
+                     zdouble *__restrict__ partial)      // Vev: m columns of a block whose rows are ldv apart
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T> *sV = reinterpret_cast<cplx<T> *>(smem_raw);
@@ -541,7 +541,7 @@ rgram_partial_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict_
     for (int64_t r0 = r_begin; r0 < r_end; r0 += rows_per_tile) {
         const int nrow = (int)((r_end - r0 < rows_per_tile) ? (r_end - r0) : rows_per_tile);
         __syncthreads();
-        for (int e = threadIdx.x; e < nrow * m; e += kLaThreads) sV[e] = Vev[r0 * m + e];
+        for (int e = threadIdx.x; e < nrow * m; e += kLaThreads) sV[e] = Vev[(r0 + e / m) * ldv + e % m];
         for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) sB[e] = B[r0 * s + e];
         __syncthreads();
 #pragma unroll
@@ -564,8 +564,9 @@ rgram_partial_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *__restrict_
 
 template <typename T>
 __global__ void __launch_bounds__(kLaThreads)
-deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *B, const zdouble *__restrict__ Cm, const DeflLambda lam,
-                      cplx<T> *__restrict__ QBpar, cplx<T> *Bperp, int64_t n, int m, int s, int rows_per_tile)      // Bperp may alias B
+deflate_update_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *B, const zdouble *__restrict__ Cm, const DeflLambda lam,
+                      cplx<T> *__restrict__ QBpar, cplx<T> *Bperp, int64_t n, int m, int s, int rows_per_tile, int accumulate)
+// Bperp may alias B.  accumulate != 0 (the second and later chunks of eigenvectors): QBpar += Vev (C / lambda)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T> *sC = reinterpret_cast<cplx<T> *>(smem_raw);          // [m][s]   <i|b>
@@ -581,7 +582,7 @@ deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *B, const z
         const int64_t r0 = t * rows_per_tile;
         const int nrow = (int)((n - r0 < rows_per_tile) ? (n - r0) : rows_per_tile);
         __syncthreads();
-        for (int e = threadIdx.x; e < nrow * m; e += kLaThreads) sV[e] = Vev[r0 * m + e];
+        for (int e = threadIdx.x; e < nrow * m; e += kLaThreads) sV[e] = Vev[(r0 + e / m) * ldv + e % m];
         __syncthreads();
         for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) {
             const int k = e / s, r = e - k * s;
@@ -592,6 +593,11 @@ deflate_update_kernel(const cplx<T> *__restrict__ Vev, const cplx<T> *B, const z
                 cmac(q, v, sCl[i * s + r]);
             }
             const cplx<T> b = B[r0 * s + e];
+            if (accumulate) {
+                const cplx<T> q0 = QBpar[r0 * s + e];
+                q.re += q0.re;
+                q.im += q0.im;
+            }
             QBpar[r0 * s + e] = q;
             Bperp[r0 * s + e] = {b.re - par.re, b.im - par.im};
         }

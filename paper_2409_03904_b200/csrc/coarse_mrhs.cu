@@ -1085,7 +1085,7 @@ extern "C" int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_de
 static int deflate_check(const coarse_op *op, const void *Vev, const double *lambda, int nev, int nrhs)
 {
     if (!Vev || !lambda) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
-    if (nev < 1 || nev > op->nrhs_max || nev > COARSE_MAX_NRHS) { set_error("nev %d outside 1..nrhs_max (%d)", nev, op->nrhs_max); return COARSE_INVALID_ARG; }
+    if (nev < 1 || nev > COARSE_MAX_NEV) { set_error("nev %d outside 1..%d", nev, COARSE_MAX_NEV); return COARSE_INVALID_ARG; }
     if (nrhs < 1 || nrhs > op->nrhs_max) { set_error("nrhs %d outside 1..%d", nrhs, op->nrhs_max); return COARSE_INVALID_ARG; }
     for (int i = 0; i < nev; ++i)
         if (!(lambda[i] > 0.0)) { set_error("lambda[%d] is not positive", i); return COARSE_INVALID_ARG; }
@@ -1093,32 +1093,41 @@ static int deflate_check(const coarse_op *op, const void *Vev, const double *lam
 }
 
 template <typename T>
-static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, int m, const void *B, void *QBpar, void *Bperp, int s,
+static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, int nev, const void *B, void *QBpar, void *Bperp, int s,
                         cudaStream_t stream)
 {
+    // The eigenvectors are taken in chunks of m <= min(64, nrhs_max) columns (the paper deflates with several hundred,
+    // PAPER.md:118, 196): chunk j projects the running b_perp (orthonormal vectors: <i|b_perp> = <i|b> for the vectors still to
+    // come), so one pass over a chunk and the block per stage, and b_perp may alias B.
     const int64_t n = op->dims.V * op->nb;
     zdouble *Cm = small_view(op).G;                     // m x s <= 64 x 64 complex128
-    // stage 1: C = Vev^H B
-    int rows = (int)(32768 / ((size_t)(m + s) * sizeof(cplx<T>)));
-    if (rows < 1) rows = 1;
-    int blocks = op->gram_blocks;
-    if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
-    const size_t smem1 = (size_t)rows * (m + s) * sizeof(cplx<T>);
-    rgram_partial_kernel<T><<<blocks, kLaThreads, smem1, stream>>>((const cplx<T> *)Vev, (const cplx<T> *)B, n, m, s, rows, op->gram_partial);
-    CMRHS_LAUNCH_CHECK();
-    gram_reduce_kernel<<<(m * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, m * s, Cm);
-    CMRHS_LAUNCH_CHECK();
-    // stage 2: Qb_par = Vev (C / lambda), b_perp = B - Vev C
-    DeflLambda lam;
-    for (int i = 0; i < COARSE_MAX_NRHS; ++i) lam.inv[i] = i < m ? 1.0 / lambda[i] : 0.0;
-    const int rows2 = 64;
-    const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);
-    auto kern = deflate_update_kernel<T>;
-    CMRHS_SMEM_ATTR(kern, smem2);
-    const int64_t ntiles = ceil_div(n, rows2);
-    const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
-    kern<<<grid, kLaThreads, smem2, stream>>>((const cplx<T> *)Vev, (const cplx<T> *)B, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, rows2);
-    CMRHS_LAUNCH_CHECK();
+    const int mc = op->nrhs_max < COARSE_MAX_NRHS ? op->nrhs_max : COARSE_MAX_NRHS;
+    for (int j0 = 0; j0 < nev; j0 += mc) {
+        const int m = nev - j0 < mc ? nev - j0 : mc;
+        const cplx<T> *Vj = (const cplx<T> *)Vev + j0;
+        const cplx<T> *Bin = j0 == 0 ? (const cplx<T> *)B : (const cplx<T> *)Bperp;
+        // stage 1: C = V_j^H b_perp
+        int rows = (int)(32768 / ((size_t)(m + s) * sizeof(cplx<T>)));
+        if (rows < 1) rows = 1;
+        int blocks = op->gram_blocks;
+        if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
+        const size_t smem1 = (size_t)rows * (m + s) * sizeof(cplx<T>);
+        rgram_partial_kernel<T><<<blocks, kLaThreads, smem1, stream>>>(Vj, nev, Bin, n, m, s, rows, op->gram_partial);
+        CMRHS_LAUNCH_CHECK();
+        gram_reduce_kernel<<<(m * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, m * s, Cm);
+        CMRHS_LAUNCH_CHECK();
+        // stage 2: Qb_par (+)= V_j (C / lambda), b_perp -= V_j C
+        DeflLambda lam;
+        for (int i = 0; i < COARSE_MAX_NRHS; ++i) lam.inv[i] = i < m ? 1.0 / lambda[j0 + i] : 0.0;
+        const int rows2 = 64;
+        const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);
+        auto kern = deflate_update_kernel<T>;
+        CMRHS_SMEM_ATTR(kern, smem2);
+        const int64_t ntiles = ceil_div(n, rows2);
+        const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
+        kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, rows2, j0 > 0 ? 1 : 0);
+        CMRHS_LAUNCH_CHECK();
+    }
     return COARSE_OK;
 }
 

@@ -137,6 +137,36 @@ def test_deflate_matches_oracle(dims, nb, s, nev, dtype):
     assert rel_err_cols(to_np(perp).reshape(n, 1, s), perp_ref.reshape(n, 1, s)) <= tol
 
 
+@pytest.mark.parametrize("dims,nb,s,nev,nrhs_max,dtype", [((2, 2, 2, 4), 16, 12, 192, 12, "c128"),      # 16 chunks of 12 eigenvectors
+                                                          ((4, 2, 2, 4), 8, 16, 200, 64, "c64"),         # chunks 64, 64, 64, 8
+                                                          ((2, 2, 2, 4), 16, 5, 65, 64, "c128")])        # 64 + 1
+def test_deflate_with_hundreds_of_eigenvectors(dims, nb, s, nev, nrhs_max, dtype):
+    # the paper deflates the coarse solve with "several hundred" eigenvectors (192 in its production runs, up to 1000 computed:
+    # PAPER.md:118, 196, 384-388): more than one chunk of <= min(64, nrhs_max) vectors, in place as well (Bperp aliases B)
+    from inputs import synth
+    A, lam_all, Vev, lam = _eigenpairs(dims, nb, 35, nev)
+    B = synth.make_block(dims, nb, s, 35, synth.TAG_B)
+    n = B.shape[0] * B.shape[1]
+    assert n >= 512 and nev > 64
+    Vq = Vev.astype(np.complex64).astype(np.complex128) if dtype == "c64" else Vev
+    q_ref, perp_ref = cheby_oracle.deflate(Vq, lam, B.reshape(n, s))
+    op = cm.CoarseOperator(dims, to_dev(A, dtype), nrhs_max)
+    Vd, Bd = to_dev(Vev, dtype), to_dev(B, dtype)
+    q, perp = op.deflate(Vd, lam, Bd)
+    tol = 1e-12 if dtype == "c128" else 2e-6
+    assert rel_err_cols(to_np(q).reshape(n, 1, s), q_ref.reshape(n, 1, s)) <= tol
+    assert rel_err_cols(to_np(perp).reshape(n, 1, s), perp_ref.reshape(n, 1, s)) <= tol
+    # projector identities on the device result: V^H b_perp = 0, b_perp + V V^H b = b
+    assert np.abs(Vq.conj().T @ to_np(perp).reshape(n, s)).max() <= (1e-12 if dtype == "c128" else 3e-6)
+    q2 = torch.empty_like(Bd)
+    lam_c = (cm.binding.C.c_double * nev)(*[float(x) for x in lam])
+    st = cm.lib().coarse_deflate(op._h, Vd.data_ptr(), lam_c, nev, Bd.data_ptr(), q2.data_ptr(), Bd.data_ptr(), s, None)
+    torch.cuda.synchronize()
+    op.close()
+    assert st == 0
+    assert torch.equal(q2, q) and torch.equal(Bd, perp)
+
+
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
 def test_deflate_in_place_Bperp_aliases_B(dtype):
     # coarse_mrhs.h: "Bperp may alias B" -- the projection written over its own input
