@@ -21,6 +21,7 @@
 #include "stencil_h16.cuh"
 #include "stencil_h16x.cuh"
 #include "peaks.cuh"
+#include "blockla_tc.cuh"
 
 namespace cmrhs {
 
@@ -459,9 +460,19 @@ extern "C" int coarse_op_apply_host(coarse_op_t *op, const void *X_host, void *Y
 }
 
 // ---- block-CG building blocks --------------------------------------------------------------------------
+static bool use_tla(const coarse_op *op, int s);
+
 template <typename T>
 static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble *G, int64_t n, int s, cudaStream_t stream)
 {
+    if (sizeof(T) == 4 && use_tla(op, s)) {               // wide complex64 blocks: split-FP16 Gram on the tensor cores (blockla_tc.cuh)
+        int blocks = 0;
+        const int st_tg = launch_tgram(U, W, op->gram_partial, op->gram_blocks, n, s, op->num_sms, stream, &blocks);
+        if (st_tg != COARSE_OK) return st_tg;
+        gram_reduce_kernel<<<(s * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, s * s, G);
+        CMRHS_LAUNCH_CHECK();
+        return COARSE_OK;
+    }
     int TT = s > 32 ? 4 : (s >= 8 ? 2 : 1);
     const int nt = (s + TT - 1) / TT;
     const int RG = kLaThreads / (nt * nt);
@@ -532,9 +543,17 @@ static int rotate_impl(const coarse_op *op, const void *U, const zdouble *K, con
     return COARSE_OK;
 }
 
+// complex64 blocks of width >= 32 (or >= 16 with COARSE_FLAG_TENSOR_LINALG): rotations and Gram products on the tensor cores
+static bool use_tla(const coarse_op *op, int s)
+{
+    if (op->dtype != COARSE_C64 || (op->flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) || !tla_supported(s)) return false;
+    return s >= 32 || (op->flags & COARSE_FLAG_TENSOR_LINALG);
+}
+
 static int rotate_dispatch(const coarse_op *op, const void *U, const zdouble *K, const void *Vin, void *out, double beta, int64_t n,
                            int s, cudaStream_t stream)
 {
+    if (use_tla(op, s)) return launch_trot(U, K, beta != 0.0 ? Vin : nullptr, out, beta, n, s, op->num_sms, stream);
     return op->dtype == COARSE_C64 ? rotate_impl<float>(op, U, K, Vin, out, beta, n, s, stream)
                                    : rotate_impl<double>(op, U, K, Vin, out, beta, n, s, stream);
 }
@@ -782,7 +801,7 @@ static int bcg_step(coarse_op *op, cudaStream_t stream)
     op->d_colmax_ready = false;
     CMRHS_STEP(gram_dispatch(op, D, Z, w.G, n, s, stream));                        // D^H Z
     CMRHS_STEP(small_launch(bcg_step1_kernel, op, s, 3, stream));                  // M, K1 = M C, K2 = -M
-    if (op->flags & COARSE_FLAG_UNFUSED_LINALG) {
+    if ((op->flags & COARSE_FLAG_UNFUSED_LINALG) || use_tla(op, s)) {       // (wide complex64 blocks: every product on the tensor cores)
         CMRHS_STEP(rotate_dispatch(op, D, w.K1, X, X, 1.0, n, s, stream));             // X += D M C
         CMRHS_STEP(rotate_dispatch(op, Z, w.K2, Q, T, 1.0, n, s, stream));             // T = Q - Z M
         CMRHS_STEP(gram_dispatch(op, T, T, w.G, n, s, stream));                        // T^H T
