@@ -201,10 +201,10 @@ __global__ void __launch_bounds__(kTlaThreads, 2) trot_kernel(const TrotParams P
 // Both operands are MN-major (the blocks' own memory order), converted tile by tile (64 rows) into the SWIZZLE_128B image the
 // stencil kernel stencil_h16.cuh uses: MMA 1: U_hi^T . [W_hi | W_lo] -> D | C, MMA 2: U_lo^T . W_hi -> C per K = 16 rows.
 // A CTA owns a contiguous range of rows (split-K) and keeps D, C in tensor memory across its tiles; it
-// FLUSHES them into its float64 partial (global, read-modify-write by the owning thread: deterministic) every kTgFlushRows
+// FLUSHES them into its float64 partial (global, read-modify-write by the owning thread: deterministic) every kTgFlushRows = 256
 // rows -- the tensor core truncates when it adds into its FP32 accumulator, so a run of sums is kept short (reading R11) --
 // and whenever a tile's magnitude leaves the range of the CTA's current power-of-two scales (one per operand).
-constexpr int kTgFlushRows = 1024;
+constexpr int kTgFlushRows = 256;
 constexpr uint32_t kTgAtom = kTlaRows * 128;          // one 64-column atom of a 64-row tile
 
 struct TgramParams {
