@@ -68,8 +68,8 @@ enum {
     COARSE_FLAG_H16X = 1u << 5,          /* complex64, nbasis 32: keep the operator in the layout of the split-FP16 kernel that
                                             holds the X operand in tensor memory (stencil_h16x: the default for nbasis 8, 16, 24)
                                             instead of the paired-site kernel's (stencil_h16) */
-    COARSE_FLAG_TENSOR_LINALG = 1u << 6  /* complex64: run the block rotations and Gram products of width 16 and 24 on the tensor
-                                            cores too (split-FP16, as the stencil kernels); widths >= 32 always do, unless
+    COARSE_FLAG_TENSOR_LINALG = 1u << 6  /* complex64: run the block rotations and Gram products of widths 16 to 32 on the tensor
+                                            cores too (split-FP16, as the stencil kernels); widths >= 40 always do, unless
                                             COARSE_FLAG_NO_TENSOR */
 };
 

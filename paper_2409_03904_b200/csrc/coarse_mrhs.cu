@@ -18,6 +18,7 @@
 #include "stencil_generic.cuh"
 #include "stencil_simt.cuh"
 #include "stencil_tc.cuh"
+#include "stencil_dmma.cuh"
 #include "stencil_h16.cuh"
 #include "stencil_h16x.cuh"
 #include "peaks.cuh"
@@ -75,6 +76,14 @@ using V_f24_s16 = SimtConfig<float, 24, 6, 2, 8, 3, 5, 16>;
 using V_d24_s8 = SimtConfig<double, 24, 3, 2, 4, 3, 3, 16>;
 using V_d8_s4 = SimtConfig<double, 8, 1, 1, 4, 1, 8, 16>;
 using V_d32_s16 = SimtConfig<double, 32, 4, 4, 4, 4, 4, 8>;
+// complex128 on the FP64 tensor path (DMMA):   NB  S KSPLIT STAGES WARPS
+using D_d24_s8 = DmmaConfig<24, 8, 1, 2, 8>;       // (whole stencil matrices per stage: 0.614 ms at configs[1]; KSPLIT 3 with 16 warps: 0.71, SIMT: 0.624)
+using D_d32_s16 = DmmaConfig<32, 16, 4, 4, 8>;
+using D_d24_s16 = DmmaConfig<24, 16, 3, 4, 8>;
+using D_d32_s8 = DmmaConfig<32, 8, 4, 3, 12>;
+using D_d16_s16 = DmmaConfig<16, 16, 2, 4, 8>;
+using D_d16_s8 = DmmaConfig<16, 8, 2, 4, 16>;
+using D_d8_s8 = DmmaConfig<8, 8, 1, 6, 16>;
 
 struct SimtVariant {
     int dtype, nb, s;
@@ -82,17 +91,20 @@ struct SimtVariant {
     int (*launch)(const void *, const int32_t *, const void *, void *, int64_t, int, cudaStream_t);
 };
 #define CMRHS_VARIANT(DT, CFG) {DT, CFG::NB, CFG::S, "stencil_simt<" #CFG ">", &launch_stencil_simt<CFG>}
-static const SimtVariant kSimtVariants[] = {
+#define CMRHS_DMMA_VARIANT(CFG) {COARSE_C128, CFG::NB, CFG::S, "stencil_dmma<" #CFG ">", &launch_stencil_dmma<CFG>}
+static const SimtVariant kSimtVariants[] = {         // (first match wins: the DMMA variants come before the SIMT ones of the same shape)
+    CMRHS_DMMA_VARIANT(D_d24_s8), CMRHS_DMMA_VARIANT(D_d32_s16), CMRHS_DMMA_VARIANT(D_d24_s16), CMRHS_DMMA_VARIANT(D_d32_s8),
+    CMRHS_DMMA_VARIANT(D_d16_s16), CMRHS_DMMA_VARIANT(D_d16_s8), CMRHS_DMMA_VARIANT(D_d8_s8),
     CMRHS_VARIANT(COARSE_C64, V_f32_s64), CMRHS_VARIANT(COARSE_C64, V_f32_s32), CMRHS_VARIANT(COARSE_C64, V_f32_s16),
     CMRHS_VARIANT(COARSE_C64, V_f32_s8),  CMRHS_VARIANT(COARSE_C64, V_f32_s4),  CMRHS_VARIANT(COARSE_C64, V_f32_s1),
     CMRHS_VARIANT(COARSE_C64, V_f24_s64), CMRHS_VARIANT(COARSE_C64, V_f24_s16), CMRHS_VARIANT(COARSE_C128, V_d24_s8),
     CMRHS_VARIANT(COARSE_C128, V_d8_s4),  CMRHS_VARIANT(COARSE_C128, V_d32_s16),
 };
 
-static const SimtVariant *find_variant(int dtype, int nb, int s)
+static const SimtVariant *find_variant(int dtype, int nb, int s, bool allow_dmma = true)
 {
     for (const auto &v : kSimtVariants)
-        if (v.dtype == dtype && v.nb == nb && v.s == s) return &v;
+        if (v.dtype == dtype && v.nb == nb && v.s == s && (allow_dmma || v.name[8] != 'd')) return &v;      // "stencil_dmma<..."
     return nullptr;
 }
 
@@ -341,7 +353,7 @@ extern "C" int64_t coarse_op_device_bytes(const coarse_op_t *op) { return op ? o
 static const SimtVariant *select_variant(const coarse_op *op, int nrhs)
 {
     if (op->flags & COARSE_FLAG_FORCE_GENERIC) return nullptr;
-    return find_variant(op->dtype, op->nb, nrhs);
+    return find_variant(op->dtype, op->nb, nrhs, !(op->flags & COARSE_FLAG_NO_TENSOR));
 }
 
 static bool use_tc(const coarse_op *op, int nrhs) { return op->tc_ok && tc_supported(op->nb, nrhs); }
@@ -547,7 +559,7 @@ static int rotate_impl(const coarse_op *op, const void *U, const zdouble *K, con
 static bool use_tla(const coarse_op *op, int s)
 {
     if (op->dtype != COARSE_C64 || (op->flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) || !tla_supported(s)) return false;
-    return s >= 32 || (op->flags & COARSE_FLAG_TENSOR_LINALG);
+    return s >= 40 || (op->flags & COARSE_FLAG_TENSOR_LINALG);      // (measured at configs[3]: at width 32 the fused SIMT passes are still faster: 2.4 vs 2.9 ms)
 }
 
 static int rotate_dispatch(const coarse_op *op, const void *U, const zdouble *K, const void *Vin, void *out, double beta, int64_t n,

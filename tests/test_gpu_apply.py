@@ -185,7 +185,8 @@ def test_full_size_baseline_configs_on_sampled_sites(index, nrhs):
     tensor = dtype == "c64" and ((nrhs % 8 == 0 or nrhs == 4) if nb == 32 else nrhs >= 4)
     # the 49 GB configuration keeps one internal layout of A (the caller's copy is needed below for the oracle's sample)
     op = cm.CoarseOperator(dims, A, nrhs, flags=cm.binding.FLAG_TENSOR_ONLY if (tensor and index == 4) else 0)
-    assert op.kernel_name(nrhs).startswith(("stencil_h16<" if nb == 32 else "stencil_h16x<") if tensor else "stencil_simt")
+    dmma = dtype == "c128" and nb % 8 == 0 and nrhs % 8 == 0          # complex128: the FP64 tensor path (mma.sync, SASS DMMA)
+    assert op.kernel_name(nrhs).startswith(("stencil_h16<" if nb == 32 else "stencil_h16x<") if tensor else ("stencil_dmma" if dmma else "stencil_simt"))
     Y = op.apply(X)
     torch.cuda.synchronize()
     sites = _sampled_sites(dims, 24, np.random.default_rng(index))

@@ -1,7 +1,7 @@
 """-m gpu parity of the block-CG linear algebra on the tensor cores (csrc/blockla_tc.cuh: split-FP16 tcgen05 Gram product
 G = U^H W and rotation out = beta Vin + U K for complex64 blocks; Table 6 "ThinQR") against the CPU oracle.
 
-Widths >= 32 take this path by default; COARSE_FLAG_TENSOR_LINALG selects it for widths 16 and 24 as well.  Bars: the Gram
+Widths >= 40 take this path by default; COARSE_FLAG_TENSOR_LINALG selects it for widths 16 to 32 as well.  Bars: the Gram
 tolerance of test_gpu_blockcg.py (|G_gpu - G_or|_ab <= 2e-6 ||u_a|| ||w_b||, reading R11) and the apply metric (<= 1e-6 per
 column here) for rotations.  What is specific to these kernels:
  * one power-of-two scale per 64-row tile (rotation) / per CTA with re-scaling (Gram): blocks whose magnitude varies by many
@@ -130,7 +130,7 @@ def test_tensor_rotation_identity_and_imaginary_unit():
     op.close()
 
 
-@pytest.mark.parametrize("s,flags", [(16, cm.binding.FLAG_TENSOR_LINALG), (32, 0), (64, 0)])
+@pytest.mark.parametrize("s,flags", [(16, cm.binding.FLAG_TENSOR_LINALG), (32, cm.binding.FLAG_TENSOR_LINALG), (64, 0)])
 def test_block_cg_through_the_tensor_linear_algebra(s, flags):
     # BlockCGrQ with every Gram product and rotation on the tensor cores against the oracle: iteration count, histories, true residual
     dims, nb, tol = (4, 4, 4, 4), 32, 1e-6
