@@ -327,7 +327,9 @@ def run_ours(args, cfg):
     seed = cfg["seed"]
     A, c = cm.fill_synthetic(dims, nb, tdt, seed, cfg["factor"])
     nrhs_max = max(SWEEP) if (args.sweep and rank == 0) else s
-    op = cm.CoarseOperator(dims, A, nrhs_max)
+    # nbasis 32 with wide blocks on the handle: keep both split-FP16 layouts (the kernel with the X operand in tensor memory is the
+    # faster one above nrhs 48, the paired-site kernel below)
+    op = cm.CoarseOperator(dims, A, nrhs_max, flags=cm.binding.FLAG_H16X_WIDE if (nb == 32 and dtype == "c64" and nrhs_max > 48) else 0)
     kernel_name = op.kernel_name(s)
 
     # bounded sample of canonical A for the oracle leg (inputs, read back before A is released)

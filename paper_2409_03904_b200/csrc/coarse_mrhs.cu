@@ -127,6 +127,7 @@ struct coarse_op {
     bool h16_ok = false;
     unsigned char *Ax = nullptr; // pre-split FP16 tiles, K-major core-matrix image [V][81][8 nb^2 bytes] (stencil_h16x.cuh: any nbasis in {8,16,24,32})
     bool h16x_ok = false;
+    bool x_wide_only = false;    // both split-FP16 layouts are kept (COARSE_FLAG_H16X_WIDE): Ax serves nrhs > 48 only
     float inv_sA = 1.0f;         // 1 / (power-of-two operator scale of Ah)
     unsigned char *Xh = nullptr; // [V] split operand tiles of the current X (pre-pass of the FP16-split kernel)
     cudaStream_t copy_stream = nullptr;   // device->host copy of the solution overlapping the true-residual apply (block_cg_solve_host*)
@@ -262,25 +263,27 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
     } while (0)
     const bool want_tc = dtype == COARSE_C64 && !(flags & (COARSE_FLAG_NO_TENSOR | COARSE_FLAG_FORCE_GENERIC)) && tc_supported(nbasis, 8);
     const bool want_split16 = want_tc && !(flags & COARSE_FLAG_TF32);
-    const bool want_h16x = want_split16 && h16x_supported(nbasis, 8) && (nbasis != 32 || (flags & COARSE_FLAG_H16X));
-    const bool want_h16 = want_split16 && !want_h16x && h16_supported(nbasis, 8);
+    // nbasis 32: the paired-site kernel (stencil_h16) by default; COARSE_FLAG_H16X: the X-in-tensor-memory kernel instead;
+    // COARSE_FLAG_H16X_WIDE: BOTH layouts, the latter serving nrhs > 48 where it is the faster one
+    const bool both16 = want_split16 && nbasis == 32 && (flags & COARSE_FLAG_H16X_WIDE) && !(flags & COARSE_FLAG_H16X) && nrhs_max > 48;
+    const bool want_h16x = want_split16 && h16x_supported(nbasis, 8) && (nbasis != 32 || (flags & COARSE_FLAG_H16X) || both16);
+    const bool want_h16 = want_split16 && (!want_h16x || both16) && h16_supported(nbasis, 8);
+    op->x_wide_only = both16;
     const bool want_simt = !(want_tc && (flags & COARSE_FLAG_TENSOR_ONLY));
     if (want_simt) CMRHS_TRY(alloc_dev(op, &op->At, a_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->nbr, (size_t)ntiles * sizeof(int32_t)));
     if (want_tc && !want_h16 && !want_h16x) CMRHS_TRY(alloc_dev(op, (void **)&op->Ak, a_bytes));
-    if (want_h16x) {
-        CMRHS_TRY(alloc_dev(op, (void **)&op->Ax, a_bytes));
+    if (want_h16x) CMRHS_TRY(alloc_dev(op, (void **)&op->Ax, a_bytes));
+    if (want_h16) CMRHS_TRY(alloc_dev(op, (void **)&op->Ah, a_bytes));
+    if (want_h16 || want_h16x) {
         CMRHS_TRY(alloc_dev(op, (void **)&op->amax, 128 * sizeof(uint32_t)));
-        const size_t xh_bytes = (size_t)V * h16x_site_bytes(nbasis, nrhs_max);
+        // scratch block of the split X tiles (padding rows / columns of a tile are never written again: zeroed once).  A handle with
+        // both layouts uses it in either format: the two kernels serve disjoint widths and every apply rewrites the rows it reads
+        size_t xh_bytes = want_h16x ? (size_t)V * h16x_site_bytes(nbasis, nrhs_max) : 0;
+        const size_t xh2 = want_h16 ? (size_t)V * h16_xo_bytes(nrhs_max < 8 ? 8 : nrhs_max) : 0;
+        if (xh2 > xh_bytes) xh_bytes = xh2;
         CMRHS_TRY(alloc_dev(op, (void **)&op->Xh, xh_bytes));
-        CMRHS_CUDA(cudaMemsetAsync(op->Xh, 0, xh_bytes, stream));       // padding rows of the chunks are never written again
-    }
-    if (want_h16) {
-        CMRHS_TRY(alloc_dev(op, (void **)&op->Ah, a_bytes));
-        CMRHS_TRY(alloc_dev(op, (void **)&op->amax, 128 * sizeof(uint32_t)));
-        const size_t xh_bytes = (size_t)V * h16_xo_bytes(nrhs_max < 8 ? 8 : nrhs_max);
-        CMRHS_TRY(alloc_dev(op, (void **)&op->Xh, xh_bytes));
-        CMRHS_CUDA(cudaMemsetAsync(op->Xh, 0, xh_bytes, stream));       // padding columns of the tiles are never written again
+        CMRHS_CUDA(cudaMemsetAsync(op->Xh, 0, xh_bytes, stream));
     }
     for (int b = 0; b < 6; ++b) CMRHS_TRY(alloc_dev(op, &op->blk[b], blk_bytes));
     CMRHS_TRY(alloc_dev(op, (void **)&op->gram_partial, (size_t)op->gram_blocks * nrhs_max * nrhs_max * sizeof(zdouble)));
@@ -331,11 +334,13 @@ extern "C" int coarse_op_create(coarse_op_t **out, const int32_t dims[4], int32_
         if (want_h16) {
             relayout_h16_kernel<<<rgrid, 256, 0, stream>>>((const cplx<float> *)A_dev, op->Ah, ntiles, sA);
             op->h16_ok = true;
-        } else {
+            count_launch();
+        }
+        if (want_h16x) {
             relayout_h16x_kernel<<<rgrid, 256, 0, stream>>>((const cplx<float> *)A_dev, op->Ax, ntiles, nbasis, sA);
             op->h16x_ok = true;
+            count_launch();
         }
-        count_launch();
     }
     ce = cudaGetLastError();
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(stream);
@@ -357,11 +362,12 @@ static const SimtVariant *select_variant(const coarse_op *op, int nrhs)
 }
 
 static bool use_tc(const coarse_op *op, int nrhs) { return op->tc_ok && tc_supported(op->nb, nrhs); }
-static bool use_h16(const coarse_op *op, int nrhs) { return op->h16_ok && h16_supported(op->nb, nrhs); }
+static bool use_h16(const coarse_op *op, int nrhs) { return op->h16_ok && h16_supported(op->nb, nrhs) && !(op->x_wide_only && nrhs > 48); }
 // the X-in-tensor-memory kernel covers every nrhs; a single column (or a pair) is left to a tuned SIMT variant when there is one
 static bool use_h16x(const coarse_op *op, int nrhs)
 {
     if (!op->h16x_ok || !h16x_supported(op->nb, nrhs)) return false;
+    if (op->x_wide_only) return nrhs > 48;
     return nrhs >= 4 || !op->At || !find_variant(op->dtype, op->nb, nrhs);
 }
 // the kernels whose X operand is scaled by per-column powers of two (column maxima in op->amax)

@@ -55,8 +55,8 @@ template <int NB> struct XCfg {
                                                                  //  numbers that meet the zero chunk of the stencil matrix)
     // tensor-memory plan (512 columns): sites per group, accumulator slots (one per site of a group; one spare at nbasis 32),
     // X buffers of XCOLS = nb columns, and one mover warp per X buffer
-    static constexpr int GMAX = NB == 32 ? 2 : 4;
-    static constexpr int NACC = NB == 32 ? 3 : (NB == 8 ? 8 : 4);
+    static constexpr int GMAX = NB == 32 ? 3 : 4;
+    static constexpr int NACC = GMAX;                            // accumulator slot i belongs to site i of every group (its MMA warp is the one waiter)
     static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS) / XCOLS;
     static constexpr int MOVERS = NXB;
     static constexpr int XBASE = NACC * ACC_COLS;
@@ -262,15 +262,16 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         const int n = 32 * q + lane, c = n & 1;
         const bool live = n < P.N2;
         const float sc = live ? inv[n] : 0.0f;
-        TcRing rc;
+        uint32_t fpar = 0u;                               // bit i: parity of slot i's next "full" phase
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const XGroup grp = group_of(g);
             for (int i = 0; i < grp.G; ++i) {
-                TW(0, mbar_wait_long(&acc_full[rc.stage], rc.phase, 256u));
+                TW(0, mbar_wait_long(&acc_full[i], (fpar >> i) & 1u, 256u));
+                fpar ^= 1u << i;
                 tc_fence_after_sync();
                 TW_BEGIN();
                 if (q < P.nq) {
-                    const uint32_t ds = lane_base + (uint32_t)(rc.stage * C::ACC_COLS);
+                    const uint32_t ds = lane_base + (uint32_t)(i * C::ACC_COLS);
                     float *yrow = Y + site_of(grp.x0 + i, grp.y, grp.z, grp.t) * (int64_t)(NB * P.N2) + n;
 #pragma unroll
                     for (int ic = 0; ic < NB / 8; ++ic) {
@@ -292,9 +293,8 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 }
                 tc_fence_before_sync();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&acc_empty[rc.stage]);
+                if (lane == 0) mbar_arrive(&acc_empty[i]);
                 TW_END(1);
-                rc.advance(C::NACC);
             }
         }
     } else if (warp == kWProd) {
@@ -366,18 +366,17 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         uint64_t *afull = a_full + me * kXMaxStagesA, *aempty = a_empty + me * kXMaxStagesA;
         uint64_t *xfull = x_full + me * kXMaxBuf, *xempty = x_empty + me * kXMaxBuf;
         const uint64_t desc_hi = umma_desc_kmajor_noswz(0u, C::LBO, C::SBO);      // everything but the start address
-        TcRing rc, ra;
+        TcRing ra;
+        uint32_t epar = 1u;                       // parity to wait for on this site's "accumulator empty" barrier (first wait passes)
         uint32_t xcnt = 0;                        // X tiles before this group
         uint32_t xpar = 0u;                       // bit b: parity of this site's next "full" phase of X buffer b
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const XGroup grp = group_of(g);
-            TcRing slot = rc;
-            for (int i = 0; i < me; ++i) slot.advance(C::NACC);
-            for (int i = 0; i < grp.G; ++i) rc.advance(C::NACC);
             if (me < grp.G) {
                 const uint32_t *tm = grp.view + me * 84;
-                const uint32_t ds = tmem + (uint32_t)(slot.stage * C::ACC_COLS);
-                TW(0, mbar_wait(&acc_empty[slot.stage], slot.phase ^ 1u));
+                const uint32_t ds = tmem + (uint32_t)(me * C::ACC_COLS);
+                TW(0, mbar_wait(&acc_empty[me], epar));
+                epar ^= 1u;
                 uint32_t xb = (xcnt + (tm[0] & 0xFFu)) % (uint32_t)C::NXB;
                 bool okx = false, oka = false;
                 for (int k = 0; k < kNPoint; ++k) {
@@ -405,7 +404,7 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                         }
                         umma_commit(&aempty[ra.stage]);
                         umma_commit(&xempty[xb]);
-                        if (k == kNPoint - 1) umma_commit(&acc_full[slot.stage]);
+                        if (k == kNPoint - 1) umma_commit(&acc_full[me]);
                     }
                     __syncwarp();
                     TW_END(3);

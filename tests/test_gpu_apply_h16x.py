@@ -8,7 +8,7 @@ dominant operators of BASELINE.json a tighter 1e-6 is asserted as well (block CG
 of stencil_h16.cuh (hi + 2^-11 lo in binary16 after power-of-two scalings), so the same "exact to 2^-21" bars apply.
 
 Lattice shapes exercise every group size: x extent 1..4 = one group of G = 1..4 sites, 5 = 4 + 1, 6 = 4 + 2, 7 = 4 + 3,
-9 = 4 + 4 + 1 (nbasis 32: pairs); extents 1-2 make several stencil points alias one neighbour.
+9 = 4 + 4 + 1 (nbasis 32: groups of up to 3); extents 1-2 make several stencil points alias one neighbour.
 """
 import numpy as np
 import pytest
@@ -185,4 +185,23 @@ def test_h16x_repeated_applies_are_bit_identical():
     Y0 = op.apply(Xd).clone()
     for _ in range(5):
         assert torch.equal(op.apply(Xd), Y0)
+    op.close()
+
+
+def test_h16x_wide_flag_keeps_both_layouts_and_splits_the_widths():
+    # COARSE_FLAG_H16X_WIDE (nbasis 32, nrhs_max > 48): stencil_h16 serves nrhs <= 48, stencil_h16x the wider blocks; the two
+    # kernels share the scratch block of split X tiles in their own formats, so alternate the widths
+    dims, nb = (6, 3, 3, 4), 32
+    A, c = synth.make_operator(dims, nb, 61, 1.05)
+    op = cm.CoarseOperator(dims, to_dev(A, "c64"), 64, flags=cm.binding.FLAG_H16X_WIDE)
+    assert op.kernel_name(64).startswith("stencil_h16x<") and op.kernel_name(56).startswith("stencil_h16x<")
+    assert op.kernel_name(48).startswith("stencil_h16<") and op.kernel_name(16).startswith("stencil_h16<")
+    for s in (64, 16, 24, 56, 8, 64, 48):
+        X = synth.make_block(dims, nb, s, 61 + s, synth.TAG_X)
+        Y = to_np(op.apply(to_dev(X, "c64")))
+        assert rel_err_cols(Y, oracle.apply(dims, A, X)) <= 1e-6, s
+    op.close()
+    # without wide blocks on the handle the flag changes nothing
+    op = cm.CoarseOperator(dims, to_dev(A, "c64"), 32, flags=cm.binding.FLAG_H16X_WIDE)
+    assert op.kernel_name(32).startswith("stencil_h16<")
     op.close()
