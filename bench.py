@@ -329,7 +329,10 @@ def run_ours(args, cfg):
     nrhs_max = max(SWEEP) if (args.sweep and rank == 0) else s
     # nbasis 32 with wide blocks on the handle: keep both split-FP16 layouts (the kernel with the X operand in tensor memory is the
     # faster one above nrhs 48, the paired-site kernel below)
-    op = cm.CoarseOperator(dims, A, nrhs_max, flags=cm.binding.FLAG_H16X_WIDE if (nb == 32 and dtype == "c64" and nrhs_max > 48) else 0)
+    flags = cm.binding.FLAG_H16X_WIDE if (nb == 32 and dtype == "c64" and nrhs_max > 48) else 0
+    if dtype == "c64" and 81 * V * nb * nb * esize > (40 << 30) and nrhs_max >= 4:
+        flags |= cm.binding.FLAG_TENSOR_ONLY                     # the 49 GB operator of configs[4]: one internal layout only
+    op = cm.CoarseOperator(dims, A, nrhs_max, flags=flags)
     kernel_name = op.kernel_name(s)
 
     # bounded sample of canonical A for the oracle leg (inputs, read back before A is released)

@@ -11,10 +11,12 @@
 // Arithmetic: X(y) as the real K x 2S matrix it is in memory; per 8-row tile of A and 8 real columns of X
 //   P0 += Re A . X_re   Q0 += Im A . X_re   P1 += Re A . X_im   Q1 += Im A . X_im      (4 DMMAs per k = 4 slab)
 //   Y_re = P0 - Q1,  Y_im = P1 + Q0   once per site.
-// Fragments: lane l holds A[row l/4][k l%4] -- Re and Im arrive together in ONE 16-byte load (k-major tile: the 8 rows of a
-// k are 128 contiguous bytes, the 4 k of a slab hit the same banks in 4 wavefronts: the minimum) -- and X[k l%4][column
-// l/4]: the 8 "columns" of a tile are the EVEN (re) resp. ODD (im) real columns of 8 consecutive right-hand sides, so one
-// 16-byte load of (re, im) feeds both the X_re and the X_im tile.
+// Fragments: lane l holds A[row l/4][k l%4] -- Re and Im arrive together in ONE 16-byte load -- and X[k l%4][column l/4]: the 8
+// "columns" of a tile are the EVEN (re) resp. ODD (im) real columns of 8 consecutive right-hand sides, so one 16-byte load of
+// (re, im) feeds both the X_re and the X_im tile.  Known cost (ncu, configs[1]: LSU wavefronts 72 % busy): the 8 lanes the LSU
+// serves together hold 2 rows x 4 k, and the k rows of the bulk-copied tile are 384 / 512 bytes apart -- a 4-way bank conflict.
+// Padding the rows (one bulk copy per k row) removes it but costs more than it saves (48 copies of 128-416 bytes per stage:
+// configs[1] 0.61 -> 0.90 ms), so the tile keeps its one-copy layout.
 #pragma once
 
 #include "stencil_simt.cuh"
