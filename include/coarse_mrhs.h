@@ -71,9 +71,11 @@ enum {
     COARSE_FLAG_TENSOR_LINALG = 1u << 6, /* complex64: run the block rotations and Gram products of widths 16 to 32 on the tensor
                                             cores too (split-FP16, as the stencil kernels); widths >= 40 always do, unless
                                             COARSE_FLAG_NO_TENSOR */
-    COARSE_FLAG_H16X_WIDE = 1u << 7      /* complex64, nbasis 32, nrhs_max > 48: keep BOTH split-FP16 layouts of the operator (one more
+    COARSE_FLAG_H16X_WIDE = 1u << 7,     /* complex64, nbasis 32, nrhs_max > 48: keep BOTH split-FP16 layouts of the operator (one more
                                             internal copy): stencil_h16 serves nrhs <= 48, stencil_h16x the wider blocks, where it
                                             is the faster kernel (7.4 vs 7.8 ms at BASELINE configs[3], nrhs 64) */
+    COARSE_FLAG_NO_GRAPH = 1u << 8       /* block_cg_*: never replay an iteration as a CUDA graph (by default small, launch-bound blocks --
+                                            V * nbasis * nrhs <= 2^22 -- do, from the second iteration of a solve on) */
 };
 
 #define COARSE_MAX_NRHS 64

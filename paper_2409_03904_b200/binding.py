@@ -16,7 +16,7 @@ from . import build as _build
 
 C64, C128 = 0, 1
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY, NOT_CONVERGED, BREAKDOWN = 0, -1, -2, -3, -4, -5, -6
-FLAG_FORCE_GENERIC, FLAG_NO_TENSOR, FLAG_TENSOR_ONLY, FLAG_TF32, FLAG_UNFUSED_LINALG, FLAG_H16X, FLAG_TENSOR_LINALG, FLAG_H16X_WIDE = 1, 2, 4, 8, 16, 32, 64, 128
+FLAG_FORCE_GENERIC, FLAG_NO_TENSOR, FLAG_TENSOR_ONLY, FLAG_TF32, FLAG_UNFUSED_LINALG, FLAG_H16X, FLAG_TENSOR_LINALG, FLAG_H16X_WIDE, FLAG_NO_GRAPH = 1, 2, 4, 8, 16, 32, 64, 128, 256
 MAX_NRHS, MAX_HISTORY = 64, 256
 SOLVE_ZERO_GUESS = 1
 

@@ -152,6 +152,15 @@ struct coarse_op {
     int prof_n = 0;
     cudaEvent_t prof_ev[2 * 64] = {};
     int64_t device_bytes = 0;
+    // one BlockCGrQ iteration as a CUDA graph (launch-bound small lattices: 9-14 launches per iteration; the paper loses ~50 % of its
+    // coarse operator to launch synchronisation).  Captured at the second iteration of a solve (the first differs in one
+    // pre-pass) and replayed while the block X, the width and the pre-pass state are the same; any capture error turns it off.
+    cudaGraphExec_t step_graph = nullptr;
+    cudaStream_t graph_stream = nullptr;      // the handle's own (blocking) stream: a capture cannot run on the legacy default stream
+    const void *graph_X = nullptr, *graph_cand_X = nullptr;
+    int graph_cand_s = 0, graph_seen = 0;
+    int graph_s = 0, graph_launches = 0;
+    bool graph_colmax_in = false, graph_colmax_out = false, graph_off = false;
 };
 
 static int alloc_dev(coarse_op *op, void **p, size_t bytes)
@@ -220,6 +229,8 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     cudaFree(op->dinfo);
     if (op->hpin) cudaFreeHost(op->hpin);
     for (cudaEvent_t e : op->prof_ev) if (e) cudaEventDestroy(e);
+    if (op->step_graph) cudaGraphExecDestroy(op->step_graph);
+    if (op->graph_stream) cudaStreamDestroy(op->graph_stream);
     delete op;
     return COARSE_OK;
 }
@@ -839,6 +850,55 @@ static int bcg_step(coarse_op *op, cudaStream_t stream)
     return COARSE_OK;
 }
 
+// bcg_step through a CUDA graph where that pays (the iteration is launch-bound: small lattices) and is possible
+static int bcg_step_fast(coarse_op *op, cudaStream_t stream)
+{
+    const int64_t n_elems = op->dims.V * op->nb * (int64_t)op->bcg_s;
+    if (op->graph_off || op->prof_on || n_elems > (1ll << 22) || (op->flags & COARSE_FLAG_NO_GRAPH)) return bcg_step(op, stream);
+    if (op->step_graph && op->graph_X == op->bcg_X && op->graph_s == op->bcg_s && op->graph_colmax_in == op->d_colmax_ready) {
+        cudaStream_t gs = stream ? stream : op->graph_stream;
+        CMRHS_CUDA(cudaGraphLaunch(op->step_graph, gs));
+        count_launch(op->graph_launches);
+        op->d_colmax_ready = op->graph_colmax_out;
+        op->bcg_its += 1;
+        return COARSE_OK;
+    }
+    if (op->bcg_its < 1) return bcg_step(op, stream);          // (the first iteration of a solve runs the column-maxima pre-pass itself)
+    // capturing and instantiating costs ~0.15 ms: only once the same block and width have run a few iterations without a graph
+    if (op->graph_cand_X != op->bcg_X || op->graph_cand_s != op->bcg_s) { op->graph_cand_X = op->bcg_X; op->graph_cand_s = op->bcg_s; op->graph_seen = 0; }
+    if (++op->graph_seen <= 5) return bcg_step(op, stream);
+    if (!op->graph_stream && cudaStreamCreate(&op->graph_stream) != cudaSuccess) { op->graph_off = true; cudaGetLastError(); return bcg_step(op, stream); }
+    cudaStream_t gs = stream ? stream : op->graph_stream;
+    const bool colmax_in = op->d_colmax_ready;
+    const int its0 = op->bcg_its;
+    const int64_t l0 = g_launches.load();
+    if (cudaStreamBeginCapture(gs, cudaStreamCaptureModeRelaxed) != cudaSuccess) { op->graph_off = true; cudaGetLastError(); return bcg_step(op, stream); }
+    const int st = bcg_step(op, gs);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(gs, &graph);
+    const int launches = (int)(g_launches.load() - l0);
+    g_launches.fetch_sub(launches);                             // (counted when the graph is launched)
+    op->bcg_its = its0;
+    if (st != COARSE_OK || ce != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        op->graph_off = true;
+        op->d_colmax_ready = colmax_in;
+        return bcg_step(op, stream);
+    }
+    if (op->step_graph) { cudaGraphExecDestroy(op->step_graph); op->step_graph = nullptr; }
+    const cudaError_t ie = cudaGraphInstantiate(&op->step_graph, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ie != cudaSuccess) { cudaGetLastError(); op->step_graph = nullptr; op->graph_off = true; op->d_colmax_ready = colmax_in; return bcg_step(op, stream); }
+    op->graph_X = op->bcg_X;
+    op->graph_s = op->bcg_s;
+    op->graph_colmax_in = colmax_in;
+    op->graph_colmax_out = op->d_colmax_ready;
+    op->graph_launches = launches;
+    op->d_colmax_ready = colmax_in;
+    return bcg_step_fast(op, stream);                           // now replays it
+}
+
 // true residual from one extra apply; fills res (iterations, residuals); synchronises
 static int bcg_end(coarse_op *op, block_cg_result *res, cudaStream_t stream)
 {
@@ -876,7 +936,7 @@ static int block_cg_impl(coarse_op *op, const void *B, void *X, int s, double to
     res->history[0] = h_stop[0];
     if (status == COARSE_NOT_CONVERGED) {
         for (int k = 0; k < maxiter; ++k) {
-            CMRHS_STEP(bcg_step(op, stream));
+            CMRHS_STEP(bcg_step_fast(op, stream));
             CMRHS_STEP(fetch_scalars(op, stream));                                         // stop scalar -> host
             if (h_stop[1] != 0.0) {
                 // D^H Z failed (statement 9): the iteration did nothing (the s x s kernels froze X, blockcg_kernels.cuh): it does not count
@@ -1033,7 +1093,7 @@ extern "C" int block_cg_step(coarse_op_t *op, int32_t count, void *stream)
 {
     if (!op || count < 0) { set_error("bad argument"); return COARSE_INVALID_ARG; }
     if (!op->bcg_active) { set_error("block_cg_step without an active block_cg_begin"); return COARSE_INVALID_ARG; }
-    for (int k = 0; k < count; ++k) CMRHS_STEP(bcg_step(op, (cudaStream_t)stream));
+    for (int k = 0; k < count; ++k) CMRHS_STEP(bcg_step_fast(op, (cudaStream_t)stream));
     return COARSE_OK;
 }
 

@@ -300,3 +300,35 @@ def test_first_solve_of_a_fresh_process_at_this_width(s):
         "print('ok', out['iterations'])\n")
     r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "ok" in r.stdout, r.stdout + r.stderr
+
+
+@pytest.mark.parametrize("dims,nb,s,dtype,tol", [((4, 4, 4, 4), 8, 4, "c128", 1e-10), ((4, 4, 2, 2), 32, 16, "c64", 1e-6), ((3, 3, 2, 4), 13, 5, "c128", 1e-10)])
+def test_graph_replay_of_an_iteration_equals_eager_launches(dims, nb, s, dtype, tol):
+    # small blocks replay iterations 2, 3, ... of a solve as a CUDA graph (captured once per handle, block and width): same kernels in
+    # the same order, so solution, iteration count and residual history are bit-identical to COARSE_FLAG_NO_GRAPH; repeated
+    # solves on the handle (the graph is reused), a solve into another block (re-captured) and the begin/step/end form as well
+    A, c, X0, B = host_case(dims, nb, s, seed=123, factor=1.05)
+    outs = {}
+    for name, flags in (("graph", 0), ("eager", cm.binding.FLAG_NO_GRAPH)):
+        op = cm.CoarseOperator(dims, to_dev(A, dtype), s, flags=flags)
+        Bd = to_dev(B, dtype)
+        X1, X2 = torch.zeros_like(Bd), torch.zeros_like(Bd)
+        r1 = op.block_cg(Bd, X1, tol=tol, maxiter=60)
+        l0 = cm.launch_count()
+        r2 = op.block_cg(Bd, X1.zero_(), tol=tol, maxiter=60)             # same block again
+        launches = cm.launch_count() - l0
+        r3 = op.block_cg(Bd, X2, tol=tol, maxiter=60)                     # another block
+        st, _ = op.block_cg_begin(Bd, X2.zero_(), tol=1e-300)
+        op.block_cg_step(r1["iterations"])
+        r4 = op.block_cg_end()
+        outs[name] = (r1, r2, r3, r4, to_np(X1), to_np(X2), launches)
+        op.close()
+    g, e = outs["graph"], outs["eager"]
+    ref = oracle.block_cg(dims, A, B, tol=tol, maxiter=60)
+    for k in range(3):
+        assert g[k]["iterations"] == e[k]["iterations"] == ref["iterations"] >= 3
+        assert g[k]["history"] == e[k]["history"]
+        assert g[k]["rel_res_true"] == e[k]["rel_res_true"]
+    assert np.array_equal(g[4], e[4]) and np.array_equal(g[5], e[5])
+    assert g[3]["rel_res_recursive"] == e[3]["rel_res_recursive"]
+    assert g[6] == e[6]                                                   # the launch counter counts the kernels of a replayed graph too
