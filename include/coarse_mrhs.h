@@ -106,9 +106,13 @@ int coarse_op_destroy(coarse_op_t *op);
  * (Eq. 19 summed over the stencil; the paper issues 81 batched GEMMs).
  *   X_dev, Y_dev : device, [V][nbasis][nrhs], dtype of the operator, 16-byte aligned; Y must not alias X
  *   nrhs         : 1..nrhs_max
- * Asynchronous on `stream`; allocates nothing.  complex64, nbasis 32, nrhs 4 or a multiple of 8 (the split-FP16 tensor
- * kernel): two short pre-pass kernels first write the scaled, split copy of X into a scratch block OWNED BY THE HANDLE, so
- * applies on one handle must be ordered (same stream, or externally synchronised); distinct handles are independent.
+ * Asynchronous on `stream`; allocates nothing.  Kernel selection (coarse_op_kernel_name tells which): complex64 with nbasis 32
+ * and nrhs 4 or a multiple of 8 -> stencil_h16 (tcgen05, split FP16, paired sites); complex64 with nbasis 8, 16, 24 and nrhs >= 4
+ * (nbasis 32 with COARSE_FLAG_H16X, or above nrhs 48 with COARSE_FLAG_H16X_WIDE) -> stencil_h16x (tcgen05, split FP16, X operand
+ * in tensor memory); COARSE_FLAG_TF32 -> stencil_tc; complex128 with nbasis and nrhs multiples of 8 -> stencil_dmma (mma.sync
+ * f64); otherwise a tiled SIMT variant or the generic kernel.  The split-FP16 kernels first run two short pre-pass kernels that
+ * write the scaled, split copy of X into a scratch block OWNED BY THE HANDLE, so applies on one handle must be ordered (same
+ * stream, or externally synchronised) although the handle is passed as const; distinct handles are independent.
  */
 int coarse_op_apply(const coarse_op_t *op, const void *X_dev, void *Y_dev, int32_t nrhs, void *stream);
 
