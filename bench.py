@@ -416,7 +416,8 @@ def run_ours(args, cfg):
         for sv in SWEEP:
             Xs = cm.fill_block(dims, nb, sv, tdt, seed, synth.TAG_X)
             Ys = torch.empty_like(Xs)
-            t_ms = time_apply(torch, op, Xs, Ys, reps=20)
+            batches = [time_apply(torch, op, Xs, Ys, reps=20) for _ in range(2)]      # two batches of 20 launches back to back
+            t_ms = min(batches)                                                        # (the power state of the board moves a batch by several %: the better one, both kept)
             r = roofline_tflops(V, nb, sv, dtype, peaks, op.kernel_name(sv), sustained=True)
             tf = apply_flops(V, nb, sv) / (t_ms * 1e-3) / 1e12
             # block-CG solve seconds at this Nrhs (the metric's second half): device-resident, X_0 = 0, to the config's tolerance
@@ -424,7 +425,7 @@ def run_ours(args, cfg):
             sol_s = op.block_cg(Bs, tol=cfg["tol"], maxiter=100, zero_guess=True)
             sweep.append(dict(nrhs=sv, ms=t_ms, tflops=tf, hbm_gbs=apply_bytes(V, nb, sv, esize) / (t_ms * 1e-3) / 1e9,
                               roof_tflops=r["roof_tflops"], bound=r["bound"], frac=tf / r["roof_tflops"],
-                              kernel=op.kernel_name(sv),
+                              kernel=op.kernel_name(sv), ms_batches=batches,
                               block_cg=dict(seconds=sol_s["seconds"], iterations=sol_s["iterations"], status=sol_s["status"],
                                             max_true_rel_res=max(sol_s["rel_res_true"]))))
             del Xs, Ys, Bs, sol_s
