@@ -6,9 +6,12 @@
 //   D_x[(r,c)][(h,part,i)] += sum_k X(y)[k][(r,c)] . A^p(x)_{h,part}[i][k]          y = x + delta_p
 // * M side (the 128 TMEM lanes) = the 2 nrhs real columns (r, re/im) of the neighbour's X tile, held IN TENSOR MEMORY
 //   (tcgen05.mma with the A operand from TMEM): lane m, 16-bit pairs along k, [X_hi | X_lo] in nb columns.  The pre-split
-//   tile arrives in a shared-memory ring by one bulk copy and goes to tensor memory by tcgen05.cp (no thread touches it);
-//   every MMA then reads only the stencil matrix through the shared-memory pipe.  (stencil_h16.cuh reads both operands of
-//   every MMA from shared memory and is bound by that pipe from nrhs 32 up.)
+//   tile arrives in a shared-memory ring by one bulk copy; loader warps (4 per lane quarter, taking turns) carry it on with
+//   one 16-byte shared-memory load per lane and k chunk and tcgen05.st.  (tcgen05.cp does the same without threads and is
+//   kept as a compile-time alternative, -DCMRHS_XLOAD=0: it runs in the tensor pipe's own queue at 64 B/clk, 192 clk per
+//   tile during which no MMA runs -- at configs[4] 3.6 of 16.1 ms, measured by leaving the copies out.)  Every MMA then
+//   reads only the stencil matrix through the shared-memory pipe.  (stencil_h16.cuh reads both operands of every MMA from
+//   shared memory and is bound by that pipe from nrhs 32 up.)
 // * N side = the stencil matrix, K-major without swizzle: 8 x 8 core matrices of binary16 (128 contiguous bytes), the
 //   tile stored in HBM as [k chunk of 8][n group of 8] with n = (hi/lo, Re/Im, row i): 8 nb^2 bytes for ANY nb that is a
 //   multiple of 8 (no padding bytes in HBM: same size as complex64); one 1-D bulk copy per stencil matrix.
@@ -24,10 +27,11 @@
 //   not the tensor pipe (144-192 clk per point): the sites' accumulators are independent, so their streams need no order.
 //   Barriers are per site too: a parity wait cannot tell phases two apart, so every barrier has exactly one waiter
 //   that sees each of its phases (X buffers: full / empty barriers per site; the mover of a buffer keeps who used it last).
-// * One persistent CTA per SM: one mover warp per X buffer, 4 epilogue warps, one producer warp for the stencil matrices
-//   (lane i feeds site i), one producer warp for the X tiles, GMAX MMA issuers.
-// Measured (B200, 1000 W cap): BASELINE configs[4] (16^3 x 32, nbasis 24, nrhs 64) 16.4-16.7 ms per apply = 0.48 of the HBM
-// roof (the TF32 kernel: 31.5 ms); the board sits at its power cap (SM clock 1.1-1.2 GHz) -- DESIGN.md section 5.5.
+// * One persistent CTA per SM: 16 loader warps, 4 epilogue warps, one producer warp for the stencil matrices (lane i feeds
+//   site i), one producer warp for the X tiles (32 source addresses computed at once), GMAX MMA issuers.
+// Measured (B200, 1000 W cap): BASELINE configs[4] (16^3 x 32, nbasis 24) 16.0-16.3 ms per apply at nrhs 64 = 0.49-0.50 of the
+// HBM roof (the TF32 kernel: 31.5 ms), 13.0 ms at nrhs 32 (0.59), 11.7 ms at nrhs 16 (0.65); at nrhs 64 the board sits at its
+// power cap (SM clock 0.9-1.2 GHz) -- DESIGN.md section 5.5.
 #pragma once
 
 #include "stencil_h16.cuh"
@@ -57,10 +61,19 @@ template <int NB> struct XCfg {
     // X buffers of XCOLS = nb columns, and one mover warp per X buffer
     static constexpr int GMAX = NB == 32 ? 3 : 4;
     static constexpr int NACC = GMAX;                            // accumulator slot i belongs to site i of every group (its MMA warp is the one waiter)
-    static constexpr int NXB = (512 - NACC * ACC_COLS) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS) / XCOLS;
-    static constexpr int MOVERS = NXB;
+#ifndef CMRHS_XLOAD
+#define CMRHS_XLOAD 1       // 1: loader warps carry the X tile from the shared-memory ring to tensor memory (tcgen05.st); 0: tcgen05.cp movers
+#endif
+#ifndef CMRHS_XTURNS
+#define CMRHS_XTURNS 4
+#endif
+    static constexpr bool LOAD = CMRHS_XLOAD != 0;
+    static constexpr int TURNS = CMRHS_XTURNS;                   // loader warps per TMEM lane quarter, taking turns tile by tile
+    static constexpr int NXB_FIT = (512 - NACC * ACC_COLS - (NCH % 2 ? 4 : 0)) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS - (NCH % 2 ? 4 : 0)) / XCOLS;
+    static constexpr int NXB = LOAD ? NXB_FIT / TURNS * TURNS : NXB_FIT;      // (a buffer always meets the same loader turn / mover)
+    static constexpr int MOVERS = LOAD ? TURNS : NXB;            // owners of X buffers and ring stages: tile t belongs to owner t mod MOVERS
     static constexpr int XBASE = NACC * ACC_COLS;
-    static constexpr int MWARPS = (MOVERS + 3) / 4 * 4;          // (the epilogue warps must start at a multiple of 4)
+    static constexpr int MWARPS = LOAD ? 4 * TURNS : (MOVERS + 3) / 4 * 4;      // (the epilogue warps must start at a multiple of 4)
     static constexpr int WARPS = MWARPS + 4 + 2 + GMAX;
     static constexpr int THREADS = 32 * WARPS;
     static_assert(XBASE + NXB * XCOLS + (NCH % 2 ? 4 : 0) <= 512 && NXB >= 4 && NXB <= kXMaxBuf && NXB % MOVERS == 0, "tensor memory plan");
@@ -142,10 +155,10 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     if (threadIdx.x == 0) {
         for (int j = 0; j < GMAX; ++j) {
             for (int i = 0; i < P.sa; ++i) { mbar_init(&a_full[j * kXMaxStagesA + i], 1); mbar_init(&a_empty[j * kXMaxStagesA + i], 1); }
-            for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[j * kXMaxBuf + i], 1); mbar_init(&x_empty[j * kXMaxBuf + i], 1); }
+            for (int i = 0; i < C::NXB; ++i) { mbar_init(&x_full[j * kXMaxBuf + i], C::LOAD ? (uint32_t)P.nq : 1u); mbar_init(&x_empty[j * kXMaxBuf + i], 1); }
         }
         for (int i = 0; i < C::NACC; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 4); }
-        for (int i = 0; i < P.sx; ++i) { mbar_init(&x_land[i], 1); mbar_init(&x_sfree[i], 1); }
+        for (int i = 0; i < P.sx; ++i) { mbar_init(&x_land[i], 1); mbar_init(&x_sfree[i], C::LOAD ? (uint32_t)P.nq : 1u); }
         mbar_fence_init();
     }
     if (warp >= 1 && warp <= GMAX && lane == 0) {
@@ -196,6 +209,75 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
     };
     auto site_of = [&](int x, int y, int z, int t) { return x + (int64_t)P.L[0] * (y + (int64_t)P.L[1] * (z + (int64_t)P.L[2] * t)); };
 
+    if (C::LOAD && warp < kWEpi) {
+        // ================= X loaders: pre-split tile (shared-memory ring, filled by bulk copies) -> registers -> tensor memory (tcgen05.st).
+        // tcgen05.cp would do this without threads, but it runs in the tensor pipe's own queue at 64 B/clk: 12 KB per tile = 192 clk during
+        // which no MMA runs (measured at configs[4]: 3.6 of 16.1 ms); tcgen05.st writes 256 B/clk beside the MMAs. =================
+        const int q = warp & 3, turn = warp >> 2;
+        if (q < P.nq) {
+            const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)C::XBASE;
+            const uint32_t row_off = (uint32_t)(32 * q + lane) * 16u, chunk_stride = (uint32_t)P.m32 * 16u;
+            int cg = blockIdx.x, cstep = 0;       // cursor in the sequence of X tiles this CTA walks
+            bool more = cg < P.ngroups;
+            XGroup grp;
+            if (more) grp = group_of(cg);
+            TcRing rs;                            // stage of the X ring that holds the cursor's tile
+            auto skip = [&](int n) {
+                for (int k = 0; k < n && more; ++k) {
+                    rs.advance(P.sx);
+                    if (++cstep == grp.nsteps) {
+                        cstep = 0;
+                        cg += gridDim.x;
+                        more = cg < P.ngroups;
+                        if (more) grp = group_of(cg);
+                    }
+                }
+            };
+            skip(turn);
+            uint32_t t = (uint32_t)turn, pend = 0u, par = 0u;      // per buffer and site: who used the last tile stored there, parity of that site's next release
+            while (more) {
+                const uint32_t um = grp.tab[cstep] & 15u;
+                const uint32_t b = t % (uint32_t)C::NXB;
+                TW(2, mbar_wait(&x_land[rs.stage], rs.phase));
+                const unsigned char *src = ringX + (size_t)rs.stage * P.xh_site_bytes + row_off;
+                uint32_t w[8 * C::NCH];
+#pragma unroll
+                for (int c = 0; c < 2 * C::NCH; ++c) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(src + (size_t)c * chunk_stride);
+                    w[4 * c + 0] = v.x; w[4 * c + 1] = v.y; w[4 * c + 2] = v.z; w[4 * c + 3] = v.w;
+                }
+                fence_proxy_async_smem();         // this warp's reads of the stage are done before a bulk copy may overwrite it
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&x_sfree[rs.stage]);
+#pragma unroll
+                for (int i = 0; i < GMAX; ++i) {
+                    const uint32_t bit = 1u << (4u * b + i);
+                    if (pend & bit) {
+                        TW(0, mbar_wait(&x_empty[i * kXMaxBuf + b], (par & bit) ? 1u : 0u));
+                        par ^= bit;
+                    }
+                }
+                pend = (pend & ~(15u << (4u * b))) | (um << (4u * b));
+                tc_fence_after_sync();
+                TW_BEGIN();
+                const uint32_t dst = lane_base + b * (uint32_t)C::XCOLS;
+                if constexpr (C::NCH == 1) {
+                    tmem_st_x8(dst, reinterpret_cast<const uint32_t (&)[8]>(w[0]));
+                } else {
+                    tmem_st_x16(dst, reinterpret_cast<const uint32_t (&)[16]>(w[0]));
+                    if constexpr (C::NCH == 3) tmem_st_x8(dst + 16u, reinterpret_cast<const uint32_t (&)[8]>(w[16]));
+                    if constexpr (C::NCH == 4) tmem_st_x16(dst + 16u, reinterpret_cast<const uint32_t (&)[16]>(w[16]));
+                }
+                tmem_wait_st();
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane < GMAX && ((um >> lane) & 1u)) mbar_arrive(&x_full[lane * kXMaxBuf + b]);
+                TW_END(1);
+                t += C::TURNS;
+                skip(C::TURNS);
+            }
+        }
+    } else
     if (warp < kWEpi) {
         // ================= X movers: tile (shared-memory ring, filled by bulk copies) -> tensor memory by tcgen05.cp; warp m takes the
         // tiles t = m (mod MOVERS) and with them always the same X buffers and ring stages; one elected lane issues =================
@@ -338,23 +420,31 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
             }
         }
     } else if (warp == kWProdX) {
-        // ================= X producer: the pre-split tile of every step (contiguous in the scratch block), one bulk copy each =================
+        // ================= X producer: the pre-split tile of every step (contiguous in the scratch block), one bulk copy each.  The source
+        // addresses of 32 steps are computed at once, one per lane (the wrap arithmetic is most of this warp's work: one lane at a time
+        // it was busy 78 % of the kernel); then the copies are issued step by step =================
         const uint64_t pol = l2_policy_evict_last();
         TcRing rs;
         for (int g = blockIdx.x; g < P.ngroups; g += gridDim.x) {
             const XGroup grp = group_of(g);
-            for (int step = 0; step < grp.nsteps; ++step) {
-                const uint32_t e = grp.tab[step];
-                const int xs = tc_wrap(grp.x0 + (int)((e >> 4) & 7u) - 1, P.L[0]), ys = tc_wrap(grp.y + (int)((e >> 8) & 3u) - 1, P.L[1]);
-                const int zs = tc_wrap(grp.z + (int)((e >> 10) & 3u) - 1, P.L[2]), ts = tc_wrap(grp.t + (int)((e >> 12) & 3u) - 1, P.L[3]);
-                const unsigned char *src = Xh + (int64_t)(xs + P.L[0] * (ys + P.L[1] * (zs + P.L[2] * ts))) * (int64_t)P.xh_site_bytes;
-                TW(0, mbar_wait(&x_sfree[rs.stage], rs.phase ^ 1u));
-                if (elect_one_sync()) {
-                    mbar_arrive_expect_tx(&x_land[rs.stage], (uint32_t)P.xh_site_bytes);
-                    bulk_g2s(ringX + (size_t)rs.stage * P.xh_site_bytes, src, (uint32_t)P.xh_site_bytes, &x_land[rs.stage], pol);
+            for (int s0 = 0; s0 < grp.nsteps; s0 += 32) {
+                const int nb_ = min(32, grp.nsteps - s0);
+                unsigned long long mine_src = 0ull;
+                if (lane < nb_) {
+                    const uint32_t e = grp.tab[s0 + lane];
+                    const int xs = tc_wrap(grp.x0 + (int)((e >> 4) & 7u) - 1, P.L[0]), ys = tc_wrap(grp.y + (int)((e >> 8) & 3u) - 1, P.L[1]);
+                    const int zs = tc_wrap(grp.z + (int)((e >> 10) & 3u) - 1, P.L[2]), ts = tc_wrap(grp.t + (int)((e >> 12) & 3u) - 1, P.L[3]);
+                    mine_src = (unsigned long long)(uintptr_t)(Xh + (int64_t)(xs + P.L[0] * (ys + P.L[1] * (zs + P.L[2] * ts))) * (int64_t)P.xh_site_bytes);
                 }
-                __syncwarp();
-                rs.advance(P.sx);
+                for (int j = 0; j < nb_; ++j) {
+                    const unsigned char *src = reinterpret_cast<const unsigned char *>((uintptr_t)__shfl_sync(0xffffffffu, mine_src, j));
+                    TW(0, mbar_wait(&x_sfree[rs.stage], rs.phase ^ 1u));
+                    if (lane == 0) {
+                        mbar_arrive_expect_tx(&x_land[rs.stage], (uint32_t)P.xh_site_bytes);
+                        bulk_g2s(ringX + (size_t)rs.stage * P.xh_site_bytes, src, (uint32_t)P.xh_site_bytes, &x_land[rs.stage], pol);
+                    }
+                    rs.advance(P.sx);
+                }
             }
         }
     } else if (warp < kWMma + GMAX) {
