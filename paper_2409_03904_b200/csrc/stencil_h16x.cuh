@@ -26,7 +26,7 @@
 //   (barrier tests, descriptor arithmetic, 4 MMAs + 2 commits per stencil point: 600-1000 clk) is what bounds an issuer,
 //   not the tensor pipe (144-192 clk per point): the sites' accumulators are independent, so their streams need no order.
 //   Barriers are per site too: a parity wait cannot tell phases two apart, so every barrier has exactly one waiter
-//   that sees each of its phases (X buffers: full / empty barriers per site; the mover of a buffer keeps who used it last).
+//   that sees each of its phases (X buffers: full / empty barriers per site; the loader warps of a buffer keep who used it last).
 // * One persistent CTA per SM: 16 loader warps, 4 epilogue warps, one producer warp for the stencil matrices (lane i feeds
 //   site i), one producer warp for the X tiles (32 source addresses computed at once), GMAX MMA issuers.
 // Measured (B200, 1000 W cap): BASELINE configs[4] (16^3 x 32, nbasis 24) 16.0-16.3 ms per apply at nrhs 64 = 0.49-0.50 of the
@@ -58,7 +58,7 @@ template <int NB> struct XCfg {
     static constexpr int XCOLS = 8 * NCH;                        // (a half-empty last K slab reads on into the next columns: finite
                                                                  //  numbers that meet the zero chunk of the stencil matrix)
     // tensor-memory plan (512 columns): sites per group, accumulator slots (one per site of a group; one spare at nbasis 32),
-    // X buffers of XCOLS = nb columns, and one mover warp per X buffer
+    // X buffers of XCOLS = nb columns
     static constexpr int GMAX = NB == 32 ? 3 : 4;
     static constexpr int NACC = GMAX;                            // accumulator slot i belongs to site i of every group (its MMA warp is the one waiter)
 #ifndef CMRHS_XLOAD
@@ -608,7 +608,7 @@ int launch_stencil_h16x(const unsigned char *Ax, float inv_sA, uint32_t *amax_de
     const int64_t budget = 226 * 1024 - fixed - 2048;
     P.sx = (int32_t)(budget / 3 / P.xh_site_bytes);
     if (P.sx > kXMaxSX) P.sx = kXMaxSX;
-    P.sx = P.sx / C::MOVERS * C::MOVERS;          // a stage always meets the same mover
+    P.sx = P.sx / C::MOVERS * C::MOVERS;          // a stage always meets the same loader turn (or tcgen05.cp mover)
     if (P.sx < C::MOVERS) P.sx = C::MOVERS;
     P.sa = (int32_t)((budget - (int64_t)P.sx * P.xh_site_bytes) / (C::GMAX * (int64_t)C::STAGE_BYTES));
     if (P.sa > kXMaxStagesA) P.sa = kXMaxStagesA;

@@ -1,7 +1,7 @@
 """-m gpu parity of the split-FP16 tensor-core stencil kernel that holds the X operand in tensor memory
-(csrc/stencil_h16x.cuh: tcgen05 kind::f16 with the M-side operand from TMEM, tcgen05.cp, groups of up to 4 x-adjacent
+(csrc/stencil_h16x.cuh: tcgen05 kind::f16 with the M-side operand from TMEM, loader warps + tcgen05.st, groups of up to 4 x-adjacent
 sites, one MMA-issuing warp per site) against the CPU oracle.  Default kernel for complex64 with nbasis 8, 16, 24 (any nrhs
->= 4); nbasis 32 with COARSE_FLAG_H16X.
+>= 4); nbasis 32 with COARSE_FLAG_H16X, or above nrhs 48 with COARSE_FLAG_H16X_WIDE.
 
 Metric and tolerance as in test_gpu_apply.py (complex64: <= 1e-5 relative per column, north_star); on the diagonally
 dominant operators of BASELINE.json a tighter 1e-6 is asserted as well (block CG to 1e-6 needs it).  The numbers are those
