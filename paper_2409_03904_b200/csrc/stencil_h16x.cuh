@@ -15,10 +15,13 @@
 // * N side = the stencil matrix, K-major without swizzle: 8 x 8 core matrices of binary16 (128 contiguous bytes), the
 //   tile stored in HBM as [k chunk of 8][n group of 8] with n = (hi/lo, Re/Im, row i): 8 nb^2 bytes for ANY nb that is a
 //   multiple of 8 (no padding bytes in HBM: same size as complex64); one 1-D bulk copy per stencil matrix.
-//   MMA 1: X_hi^T . [A_hi | A_lo] -> D | C (N = 4 nb), MMA 2: X_lo^T . A_hi -> C (N = 2 nb), per K = 16 slab.
-//   nb = 8, 24: the last K = 16 slab is half empty: the ring stage holds a zero chunk there (never overwritten), and the X
-//   operand simply reads on into the next columns of tensor memory (always finite binary16 numbers).
-// * A GROUP of up to GMAX x-adjacent sites (4; 2 at nbasis 32, where tensor memory holds no more accumulators) shares
+//   MMA 1: X_hi^T . [A_hi | A_lo] -> D | C (N = 4 nb), MMA 2: X_lo^T . A_hi -> C (N = 2 nb), per K = 16 slab of two k chunks.
+//   nb = 8, 24 (an odd number of k chunks): the last chunk c pairs its own halves instead of a zero chunk,
+//     (X_lo c, X_hi c)^T . (A_hi c ; A_lo c) -> C   and   (X_hi c, 0)^T . (A_hi c ; A_lo c) -> D      (N = 2 nb each)
+//   -- A_lo c follows A_hi c in the tile, so a descriptor with half the chunk stride reads them as the two k chunks of a slab; the
+//   zero sits in 4 tensor-memory columns per X buffer, written once.  nb 24: 240 N x K units per stencil point instead of 288
+//   with a zero chunk in the stage, and ring stages of 4608 instead of 6144 bytes.
+// * A GROUP of up to GMAX x-adjacent sites (4; 3 at nbasis 32, where tensor memory holds no more accumulators) shares
 //   every X tile it needs: (G + 2) x 27 tile loads per group instead of 81 G -- the gather of X through L2 is the
 //   largest single cost of this kernel (measured: 21-25 % of the time at nrhs 64 with pairs of sites).
 // * EVERYTHING THAT SERIALISES IS PER SITE: one accumulator (4 nb TMEM columns), one ring of stencil matrices with its own
@@ -52,14 +55,20 @@ template <int NB> struct XCfg {
     static constexpr uint32_t LBO = 64u * NB;                    // bytes between k chunks: 4 nb / 8 core matrices of 128 B
     static constexpr uint32_t SBO = 128u;                        // bytes between n groups
     static constexpr uint32_t TILE_BYTES = 8u * NB * NB;         // one stencil matrix, [A_hi | A_lo]
-    static constexpr uint32_t STAGE_BYTES = 2u * KSTEPS * LBO;   // ring stage (>= TILE_BYTES; the rest stays zero)
+    static constexpr uint32_t STAGE_BYTES = TILE_BYTES;          // ring stage
     static constexpr int ACC_COLS = 4 * NB;                      // D (2 nb) | C (2 nb) per site
-    static constexpr int XLO = 4 * NCH;                          // TMEM column of X_lo within a tile: [X_hi: 4 per k chunk | X_lo]
-    static constexpr int XCOLS = 8 * NCH;                        // (a half-empty last K slab reads on into the next columns: finite
-                                                                 //  numbers that meet the zero chunk of the stencil matrix)
+    // TMEM columns of one X tile, 4 per k chunk ("slot").  Even NCH: [X_hi 0 .. NCH-1 | X_lo 0 .. NCH-1].  Odd NCH (nb = 8, 24), whose
+    // last chunk c has no partner for a K = 16 slab: [X_hi 0 .. c-1 | X_lo 0 .. c-1 | X_lo c | X_hi c | zero] -- the slab (X_lo c, X_hi c)
+    // meets (A_hi c, A_lo c) and gives both C products of the chunk at once, the slab (X_hi c, zero) meets (A_hi c, anything) for D.
+    static constexpr int ODD = NCH % 2;
+    static constexpr int KFULL = NCH / 2;                        // K = 16 slabs made of two data chunks
+    static constexpr int XLO = 4 * (NCH - ODD);                  // X_lo of the full slabs
+    static constexpr int XC = 8 * (NCH - ODD);                   // odd NCH: (X_lo c, X_hi c)
+    static constexpr int XD = XC + 4;                            //          (X_hi c, zero): the zero slot is written once, at kernel start
+    static constexpr int XCOLS = 8 * NCH + 4 * ODD;
     // tensor-memory plan (512 columns): sites per group, accumulator slots (one per site of a group; one spare at nbasis 32),
     // X buffers of XCOLS = nb columns
-    static constexpr int GMAX = NB == 32 ? 3 : 4;
+    static constexpr int GMAX = NB == 32 ? 3 : 4;                // (nb 24 with 3, nb 32 with 2 sites and twice the X buffers: 15 % / 7 % slower -- the issuers bound it)
     static constexpr int NACC = GMAX;                            // accumulator slot i belongs to site i of every group (its MMA warp is the one waiter)
 #ifndef CMRHS_XLOAD
 #define CMRHS_XLOAD 1       // 1: loader warps carry the X tile from the shared-memory ring to tensor memory (tcgen05.st); 0: tcgen05.cp movers
@@ -69,14 +78,14 @@ template <int NB> struct XCfg {
 #endif
     static constexpr bool LOAD = CMRHS_XLOAD != 0;
     static constexpr int TURNS = CMRHS_XTURNS;                   // loader warps per TMEM lane quarter, taking turns tile by tile
-    static constexpr int NXB_FIT = (512 - NACC * ACC_COLS - (NCH % 2 ? 4 : 0)) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS - (NCH % 2 ? 4 : 0)) / XCOLS;
+    static constexpr int NXB_FIT = (512 - NACC * ACC_COLS) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS) / XCOLS;
     static constexpr int NXB = LOAD ? NXB_FIT / TURNS * TURNS : NXB_FIT;      // (a buffer always meets the same loader turn / mover)
     static constexpr int MOVERS = LOAD ? TURNS : NXB;            // owners of X buffers and ring stages: tile t belongs to owner t mod MOVERS
     static constexpr int XBASE = NACC * ACC_COLS;
     static constexpr int MWARPS = LOAD ? 4 * TURNS : (MOVERS + 3) / 4 * 4;      // (the epilogue warps must start at a multiple of 4)
     static constexpr int WARPS = MWARPS + 4 + 2 + GMAX;
     static constexpr int THREADS = 32 * WARPS;
-    static_assert(XBASE + NXB * XCOLS + (NCH % 2 ? 4 : 0) <= 512 && NXB >= 4 && NXB <= kXMaxBuf && NXB % MOVERS == 0, "tensor memory plan");
+    static_assert(XBASE + NXB * XCOLS <= 512 && NXB >= 4 && NXB <= kXMaxBuf && NXB % MOVERS == 0, "tensor memory plan");
     static_assert(NACC >= GMAX, "one accumulator per site of a group");
 };
 
@@ -170,23 +179,18 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         const float sc = col < P.N2 ? h_scale_from_bits(P.amax[col >> 1]) : 1.0f;
         inv[col] = P.inv_sA / sc;
     }
-    if constexpr (C::STAGE_BYTES != C::TILE_BYTES) {
-        // the half-empty last K slab: the chunk after the data stays zero for the whole kernel (bulk copies never reach it)
-        for (int e = threadIdx.x; e < (int)((size_t)GMAX * P.sa * C::STAGE_BYTES / 16); e += C::THREADS)
-            reinterpret_cast<uint4 *>(ringA)[e] = make_uint4(0u, 0u, 0u, 0u);
-        fence_proxy_async_smem();
-    }
     if (warp == kWProd) tmem_alloc_cols(tmem_slot, 512u);
     tc_fence_before_sync();
     __syncthreads();
     tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
     if (warp >= kWEpi && warp < kWEpi + 4) {
-        // the X buffers start as zeros: the copies never touch the columns of a half-empty K slab (nb = 8, 24)
+        // the X buffers start as zeros: the zero slot of an odd NCH (never written again), and the lanes of quarters no loader writes
+        // (the MMAs read all 128 lanes: finite numbers, rows nobody reads)
         uint32_t zz[16];
 #pragma unroll
         for (int k = 0; k < 16; ++k) zz[k] = 0u;
-        for (int cc = 0; cc < (C::NXB * C::XCOLS + 4 + 15) / 16 * 16 && C::XBASE + cc + 16 <= 512; cc += 16) tmem_st_x16(tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(C::XBASE + cc), zz);
+        for (int cc = 0; cc < (C::NXB * C::XCOLS + 15) / 16 * 16 && C::XBASE + cc + 16 <= 512; cc += 16) tmem_st_x16(tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(C::XBASE + cc), zz);
         tmem_wait_st();
     }
     tc_fence_before_sync();
@@ -322,7 +326,7 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                     const uint32_t src = ringx0 + (uint32_t)rs.stage * (uint32_t)P.xh_site_bytes;
                     const uint32_t dst = tmem + (uint32_t)C::XBASE + b * (uint32_t)C::XCOLS;
 #pragma unroll
-                    for (int c = 0; c < 2 * C::NCH; c += 2)            // chunks [hi 0 .. NCH-1 | lo 0 .. NCH-1], two per copy
+                    for (int c = 0; c < 2 * C::NCH; c += 2)            // the tile's 2 NCH slots of 4 columns, two per copy
                         tmem_cp_128x256b(dst + (uint32_t)(4 * c), desc_hi | (uint64_t)(((src + (uint32_t)c * chunk_stride) >> 4) & 0x3FFFu));
 #pragma unroll
                     for (int i = 0; i < GMAX; ++i)
@@ -456,6 +460,7 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         uint64_t *afull = a_full + me * kXMaxStagesA, *aempty = a_empty + me * kXMaxStagesA;
         uint64_t *xfull = x_full + me * kXMaxBuf, *xempty = x_empty + me * kXMaxBuf;
         const uint64_t desc_hi = umma_desc_kmajor_noswz(0u, C::LBO, C::SBO);      // everything but the start address
+        const uint64_t desc_odd = umma_desc_kmajor_noswz(0u, C::LBO / 2, C::SBO); // k chunk 0 = A_hi, k chunk 1 = A_lo of ONE chunk (2 nb n rows each)
         TcRing ra;
         uint32_t epar = 1u;                       // parity to wait for on this site's "accumulator empty" barrier (first wait passes)
         uint32_t xcnt = 0;                        // X tiles before this group
@@ -487,10 +492,15 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                         const uint32_t x_hi = x_base + xb * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XLO;
                         const uint64_t bd0 = desc_hi | (uint64_t)(((ring0 + (uint32_t)ra.stage * C::STAGE_BYTES) >> 4) & 0x3FFFu);
 #pragma unroll
-                        for (int ks = 0; ks < C::KSTEPS; ++ks) {
+                        for (int ks = 0; ks < C::KFULL; ++ks) {
                             const uint64_t bd = bd0 + (uint64_t)((uint32_t)ks * 2u * C::LBO >> 4);
                             umma_f16_ts(ds, x_hi + 8u * ks, bd, P.idesc_wide, (k | ks) ? 1u : 0u);      // X_hi^T . [A_hi | A_lo] -> D | C
                             umma_f16_ts(ds + 2u * NB, x_lo + 8u * ks, bd, P.idesc_lo, 1u);              // X_lo^T . A_hi -> C
+                        }
+                        if constexpr (C::ODD) {   // the last chunk c: two full-rate N = 2 nb slabs instead of two half-empty N = 4 nb, 2 nb ones
+                            const uint64_t bo = desc_odd | (uint64_t)(((ring0 + (uint32_t)ra.stage * C::STAGE_BYTES + (uint32_t)(C::NCH - 1) * C::LBO) >> 4) & 0x3FFFu);
+                            umma_f16_ts(ds + 2u * NB, x_hi + (uint32_t)C::XC, bo, P.idesc_lo, (k | C::KFULL) ? 1u : 0u);      // (X_lo c, X_hi c)^T . (A_hi c ; A_lo c) -> C
+                            umma_f16_ts(ds, x_hi + (uint32_t)C::XD, bo, P.idesc_lo, (k | C::KFULL) ? 1u : 0u);                // (X_hi c, 0)^T . (A_hi c ; A_lo c) -> D
                         }
                         umma_commit(&aempty[ra.stage]);
                         umma_commit(&xempty[xb]);
@@ -556,8 +566,9 @@ __global__ void __launch_bounds__(256) relayout_h16x_kernel(const cplx<float> *_
     }
 }
 
-// per-apply pre-pass: X (fp32, [site][k][2 s real columns]) -> Xh[site][h][k chunk][m32 rows] of 16 bytes: the 8 binary16 values
-// k = 8 c .. 8 c + 7 of real column n, scaled by the column's power of two and split (hi = fp16(x), lo = fp16(2^11 (x - hi))).
+// per-apply pre-pass: X (fp32, [site][k][2 s real columns]) -> Xh[site][slot][m32 rows] of 16 bytes: the 8 binary16 values
+// k = 8 c .. 8 c + 7 of real column n, scaled by the column's power of two and split (hi = fp16(x), lo = fp16(2^11 (x - hi)));
+// slot = the group of 4 TMEM columns the chunk goes to (XCfg).
 // Rows n >= 2 s of a chunk are never written (zeroed once at create).
 __global__ void __launch_bounds__(256) xsplit_x_kernel(const float *__restrict__ X, unsigned char *__restrict__ Xh, const uint32_t *__restrict__ amax,
                                                        int64_t nsites, int nb, int s, int m32, int site_bytes)
@@ -582,8 +593,10 @@ __global__ void __launch_bounds__(256) xsplit_x_kernel(const float *__restrict__
                 hw[u] = *reinterpret_cast<const uint32_t *>(&h);
                 lw[u] = *reinterpret_cast<const uint32_t *>(&l);
             }
-            *reinterpret_cast<uint4 *>(dst + ((int64_t)c * m32 + n) * 16) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
-            *reinterpret_cast<uint4 *>(dst + ((int64_t)(nch + c) * m32 + n) * 16) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+            const bool last_odd = (nch & 1) && c == nch - 1;       // slots as the TMEM columns of XCfg: odd nch ends with (lo c, hi c)
+            const int hi_slot = last_odd ? 2 * c + 1 : c, lo_slot = last_odd ? 2 * c : (nch - (nch & 1)) + c;
+            *reinterpret_cast<uint4 *>(dst + ((int64_t)hi_slot * m32 + n) * 16) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+            *reinterpret_cast<uint4 *>(dst + ((int64_t)lo_slot * m32 + n) * 16) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
         }
     }
 }
