@@ -19,8 +19,9 @@
 //   nb = 8, 24 (an odd number of k chunks): the last chunk c pairs its own halves instead of a zero chunk,
 //     (X_lo c, X_hi c)^T . (A_hi c ; A_lo c) -> C   and   (X_hi c, 0)^T . (A_hi c ; A_lo c) -> D      (N = 2 nb each)
 //   -- A_lo c follows A_hi c in the tile, so a descriptor with half the chunk stride reads them as the two k chunks of a slab; the
-//   zero sits in 4 tensor-memory columns per X buffer, written once.  nb 24: 240 N x K units per stencil point instead of 288
-//   with a zero chunk in the stage, and ring stages of 4608 instead of 6144 bytes.
+//   zero is ONE block of 32 nb bytes in shared memory, which the D slab's descriptor names as its second k chunk (the X side of
+//   that half reads the 4 columns after the tile: finite numbers).  nb 24: 240 N x K units per stencil point instead of 288 with
+//   a zero chunk in every ring stage, stages of 4608 instead of 6144 bytes, and an X tile of 24 columns: 5 X buffers.
 // * A GROUP of up to GMAX x-adjacent sites (4; 3 at nbasis 32, where tensor memory holds no more accumulators) shares
 //   every X tile it needs: (G + 2) x 27 tile loads per group instead of 81 G -- the gather of X through L2 is the
 //   largest single cost of this kernel (measured: 21-25 % of the time at nrhs 64 with pairs of sites).
@@ -36,6 +37,9 @@
 // HBM roof (the TF32 kernel: 31.5 ms), 13.0 ms at nrhs 32 (0.59), 11.7 ms at nrhs 16 (0.65); at nrhs 64 the board sits at its
 // power cap (SM clock 0.9-1.2 GHz) -- DESIGN.md section 5.5.
 #pragma once
+#ifndef CMRHS_ABL
+#define CMRHS_ABL 0
+#endif
 
 #include "stencil_h16.cuh"
 
@@ -58,14 +62,16 @@ template <int NB> struct XCfg {
     static constexpr uint32_t STAGE_BYTES = TILE_BYTES;          // ring stage
     static constexpr int ACC_COLS = 4 * NB;                      // D (2 nb) | C (2 nb) per site
     // TMEM columns of one X tile, 4 per k chunk ("slot").  Even NCH: [X_hi 0 .. NCH-1 | X_lo 0 .. NCH-1].  Odd NCH (nb = 8, 24), whose
-    // last chunk c has no partner for a K = 16 slab: [X_hi 0 .. c-1 | X_lo 0 .. c-1 | X_lo c | X_hi c | zero] -- the slab (X_lo c, X_hi c)
-    // meets (A_hi c, A_lo c) and gives both C products of the chunk at once, the slab (X_hi c, zero) meets (A_hi c, anything) for D.
+    // last chunk c has no partner for a K = 16 slab: [X_hi 0 .. c-1 | X_lo 0 .. c-1 | X_lo c | X_hi c] -- the slab (X_lo c, X_hi c)
+    // meets (A_hi c ; A_lo c) and gives both C products of the chunk at once; the slab (X_hi c, whatever follows: the next buffer's
+    // first slot, always finite binary16 numbers) meets (A_hi c ; a block of zeros in shared memory) for D.
     static constexpr int ODD = NCH % 2;
     static constexpr int KFULL = NCH / 2;                        // K = 16 slabs made of two data chunks
     static constexpr int XLO = 4 * (NCH - ODD);                  // X_lo of the full slabs
     static constexpr int XC = 8 * (NCH - ODD);                   // odd NCH: (X_lo c, X_hi c)
-    static constexpr int XD = XC + 4;                            //          (X_hi c, zero): the zero slot is written once, at kernel start
-    static constexpr int XCOLS = 8 * NCH + 4 * ODD;
+    static constexpr int XD = XC + 4;                            //          (X_hi c, the 4 columns after the tile)
+    static constexpr int XCOLS = 8 * NCH;
+    static constexpr uint32_t ZERO_BYTES = 32u * NB;             // one k chunk of 2 nb n rows
     // tensor-memory plan (512 columns): sites per group, accumulator slots (one per site of a group; one spare at nbasis 32),
     // X buffers of XCOLS = nb columns
     static constexpr int GMAX = NB == 32 ? 3 : 4;                // (nb 24 with 3, nb 32 with 2 sites and twice the X buffers: 15 % / 7 % slower -- the issuers bound it)
@@ -76,8 +82,11 @@ template <int NB> struct XCfg {
 #ifndef CMRHS_XTURNS
 #define CMRHS_XTURNS 4
 #endif
+#ifndef CMRHS_XTURNS24
+#define CMRHS_XTURNS24 5    // nbasis 24: tensor memory has room for 5 X buffers beside 4 accumulators, and a buffer keeps its loader turn
+#endif
     static constexpr bool LOAD = CMRHS_XLOAD != 0;
-    static constexpr int TURNS = CMRHS_XTURNS;                   // loader warps per TMEM lane quarter, taking turns tile by tile
+    static constexpr int TURNS = NB == 24 ? CMRHS_XTURNS24 : CMRHS_XTURNS;                   // loader warps per TMEM lane quarter, taking turns tile by tile
     static constexpr int NXB_FIT = (512 - NACC * ACC_COLS) / XCOLS > kXMaxBuf ? kXMaxBuf : (512 - NACC * ACC_COLS) / XCOLS;
     static constexpr int NXB = LOAD ? NXB_FIT / TURNS * TURNS : NXB_FIT;      // (a buffer always meets the same loader turn / mover)
     static constexpr int MOVERS = LOAD ? TURNS : NXB;            // owners of X buffers and ring stages: tile t belongs to owner t mod MOVERS
@@ -85,7 +94,7 @@ template <int NB> struct XCfg {
     static constexpr int MWARPS = LOAD ? 4 * TURNS : (MOVERS + 3) / 4 * 4;      // (the epilogue warps must start at a multiple of 4)
     static constexpr int WARPS = MWARPS + 4 + 2 + GMAX;
     static constexpr int THREADS = 32 * WARPS;
-    static_assert(XBASE + NXB * XCOLS <= 512 && NXB >= 4 && NXB <= kXMaxBuf && NXB % MOVERS == 0, "tensor memory plan");
+    static_assert(XBASE + NXB * XCOLS + 4 * ODD <= 512 && NXB >= 4 && NXB <= kXMaxBuf && NXB % MOVERS == 0, "tensor memory plan");
     static_assert(NACC >= GMAX, "one accumulator per site of a group");
 };
 
@@ -179,18 +188,22 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         const float sc = col < P.N2 ? h_scale_from_bits(P.amax[col >> 1]) : 1.0f;
         inv[col] = P.inv_sA / sc;
     }
+    if constexpr (C::ODD) {      // the block of zeros the odd D slab reads as its second k chunk: the first bytes of the slack after the X ring
+        if (threadIdx.x < C::ZERO_BYTES / 16) reinterpret_cast<uint4 *>(ringX + (size_t)P.sx * P.xh_site_bytes)[threadIdx.x] = make_uint4(0u, 0u, 0u, 0u);
+        fence_proxy_async_smem();
+    }
     if (warp == kWProd) tmem_alloc_cols(tmem_slot, 512u);
     tc_fence_before_sync();
     __syncthreads();
     tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
     if (warp >= kWEpi && warp < kWEpi + 4) {
-        // the X buffers start as zeros: the zero slot of an odd NCH (never written again), and the lanes of quarters no loader writes
-        // (the MMAs read all 128 lanes: finite numbers, rows nobody reads)
+        // the X buffers (and the 4 columns after the last one, which the odd slab of that buffer reads) start as zeros; so do the lanes
+        // of quarters no loader writes (the MMAs read all 128 lanes: finite numbers, rows nobody reads)
         uint32_t zz[16];
 #pragma unroll
         for (int k = 0; k < 16; ++k) zz[k] = 0u;
-        for (int cc = 0; cc < (C::NXB * C::XCOLS + 15) / 16 * 16 && C::XBASE + cc + 16 <= 512; cc += 16) tmem_st_x16(tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(C::XBASE + cc), zz);
+        for (int cc = 0; cc < (C::NXB * C::XCOLS + 4 * C::ODD + 15) / 16 * 16 && C::XBASE + cc + 16 <= 512; cc += 16) tmem_st_x16(tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(C::XBASE + cc), zz);
         tmem_wait_st();
     }
     tc_fence_before_sync();
@@ -246,7 +259,7 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 const unsigned char *src = ringX + (size_t)rs.stage * P.xh_site_bytes + row_off;
                 uint32_t w[8 * C::NCH];
 #pragma unroll
-                for (int c = 0; c < 2 * C::NCH; ++c) {
+                for (int c = 0; c < (CMRHS_ABL == 2 ? 0 : 2 * C::NCH); ++c) {
                     const uint4 v = *reinterpret_cast<const uint4 *>(src + (size_t)c * chunk_stride);
                     w[4 * c + 0] = v.x; w[4 * c + 1] = v.y; w[4 * c + 2] = v.z; w[4 * c + 3] = v.w;
                 }
@@ -265,7 +278,8 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                 tc_fence_after_sync();
                 TW_BEGIN();
                 const uint32_t dst = lane_base + b * (uint32_t)C::XCOLS;
-                if constexpr (C::NCH == 1) {
+                if constexpr (CMRHS_ABL == 2) {
+                } else if constexpr (C::NCH == 1) {
                     tmem_st_x8(dst, reinterpret_cast<const uint32_t (&)[8]>(w[0]));
                 } else {
                     tmem_st_x16(dst, reinterpret_cast<const uint32_t (&)[16]>(w[0]));
@@ -412,8 +426,9 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         while (__any_sync(0xffffffffu, active)) {
             if (active && mbar_test_wait(&empty[ra.stage], ra.phase ^ 1u)) {
                 const uint32_t p = (tm[k] >> 16) & 0x7Fu;
-                mbar_arrive_expect_tx(&full[ra.stage], C::TILE_BYTES);
-                bulk_g2s(ring + (size_t)ra.stage * C::STAGE_BYTES, src0 + (size_t)p * C::TILE_BYTES, C::TILE_BYTES, &full[ra.stage], pol);
+                constexpr uint32_t kCopy = CMRHS_ABL == 3 ? 16u : C::TILE_BYTES;
+                mbar_arrive_expect_tx(&full[ra.stage], kCopy);
+                bulk_g2s(ring + (size_t)ra.stage * C::STAGE_BYTES, src0 + (size_t)p * C::TILE_BYTES, kCopy, &full[ra.stage], pol);
                 ra.advance(P.sa);
                 if (++k == kNPoint) {
                     k = 0;
@@ -444,8 +459,9 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                     const unsigned char *src = reinterpret_cast<const unsigned char *>((uintptr_t)__shfl_sync(0xffffffffu, mine_src, j));
                     TW(0, mbar_wait(&x_sfree[rs.stage], rs.phase ^ 1u));
                     if (lane == 0) {
-                        mbar_arrive_expect_tx(&x_land[rs.stage], (uint32_t)P.xh_site_bytes);
-                        bulk_g2s(ringX + (size_t)rs.stage * P.xh_site_bytes, src, (uint32_t)P.xh_site_bytes, &x_land[rs.stage], pol);
+                        const uint32_t xcopy = CMRHS_ABL == 4 ? 16u : (uint32_t)P.xh_site_bytes;
+                        mbar_arrive_expect_tx(&x_land[rs.stage], xcopy);
+                        bulk_g2s(ringX + (size_t)rs.stage * P.xh_site_bytes, src, xcopy, &x_land[rs.stage], pol);
                     }
                     rs.advance(P.sx);
                 }
@@ -461,6 +477,8 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
         uint64_t *xfull = x_full + me * kXMaxBuf, *xempty = x_empty + me * kXMaxBuf;
         const uint64_t desc_hi = umma_desc_kmajor_noswz(0u, C::LBO, C::SBO);      // everything but the start address
         const uint64_t desc_odd = umma_desc_kmajor_noswz(0u, C::LBO / 2, C::SBO); // k chunk 0 = A_hi, k chunk 1 = A_lo of ONE chunk (2 nb n rows each)
+        const uint64_t desc_zero = umma_desc_kmajor_noswz(0u, 0u, C::SBO);        // k chunk 0 = A_hi of that chunk, k chunk 1 = the block of zeros (LBO per stage)
+        const uint32_t zero_addr = smem_u32(ringX + (size_t)P.sx * P.xh_site_bytes);
         TcRing ra;
         uint32_t epar = 1u;                       // parity to wait for on this site's "accumulator empty" barrier (first wait passes)
         uint32_t xcnt = 0;                        // X tiles before this group
@@ -491,6 +509,7 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                     if (elect_one_sync()) {
                         const uint32_t x_hi = x_base + xb * (uint32_t)C::XCOLS, x_lo = x_hi + (uint32_t)C::XLO;
                         const uint64_t bd0 = desc_hi | (uint64_t)(((ring0 + (uint32_t)ra.stage * C::STAGE_BYTES) >> 4) & 0x3FFFu);
+#if CMRHS_ABL != 1
 #pragma unroll
                         for (int ks = 0; ks < C::KFULL; ++ks) {
                             const uint64_t bd = bd0 + (uint64_t)((uint32_t)ks * 2u * C::LBO >> 4);
@@ -498,10 +517,13 @@ stencil_h16x_kernel(const unsigned char *__restrict__ Ax, const unsigned char *_
                             umma_f16_ts(ds + 2u * NB, x_lo + 8u * ks, bd, P.idesc_lo, 1u);              // X_lo^T . A_hi -> C
                         }
                         if constexpr (C::ODD) {   // the last chunk c: two full-rate N = 2 nb slabs instead of two half-empty N = 4 nb, 2 nb ones
-                            const uint64_t bo = desc_odd | (uint64_t)(((ring0 + (uint32_t)ra.stage * C::STAGE_BYTES + (uint32_t)(C::NCH - 1) * C::LBO) >> 4) & 0x3FFFu);
+                            const uint32_t ac = ring0 + (uint32_t)ra.stage * C::STAGE_BYTES + (uint32_t)(C::NCH - 1) * C::LBO;
+                            const uint64_t bo = desc_odd | (uint64_t)((ac >> 4) & 0x3FFFu);
+                            const uint64_t bz = desc_zero | (uint64_t)((ac >> 4) & 0x3FFFu) | ((uint64_t)(((zero_addr - ac) >> 4) & 0x3FFFu) << 16);
                             umma_f16_ts(ds + 2u * NB, x_hi + (uint32_t)C::XC, bo, P.idesc_lo, (k | C::KFULL) ? 1u : 0u);      // (X_lo c, X_hi c)^T . (A_hi c ; A_lo c) -> C
-                            umma_f16_ts(ds, x_hi + (uint32_t)C::XD, bo, P.idesc_lo, (k | C::KFULL) ? 1u : 0u);                // (X_hi c, 0)^T . (A_hi c ; A_lo c) -> D
+                            umma_f16_ts(ds, x_hi + (uint32_t)C::XD, bz, P.idesc_lo, (k | C::KFULL) ? 1u : 0u);                // (X_hi c, any)^T . (A_hi c ; 0) -> D
                         }
+#endif
                         umma_commit(&aempty[ra.stage]);
                         umma_commit(&xempty[xb]);
                         if (k == kNPoint - 1) umma_commit(&acc_full[me]);
