@@ -33,12 +33,14 @@
 //   that sees each of its phases (X buffers: full / empty barriers per site; the loader warps of a buffer keep who used it last).
 // * One persistent CTA per SM: 16 loader warps, 4 epilogue warps, one producer warp for the stencil matrices (lane i feeds
 //   site i), one producer warp for the X tiles (32 source addresses computed at once), GMAX MMA issuers.
-// Measured (B200, 1000 W cap): BASELINE configs[4] (16^3 x 32, nbasis 24) 16.0-16.3 ms per apply at nrhs 64 = 0.49-0.50 of the
-// HBM roof (the TF32 kernel: 31.5 ms), 13.0 ms at nrhs 32 (0.59), 11.7 ms at nrhs 16 (0.65); at nrhs 64 the board sits at its
-// power cap (SM clock 0.9-1.2 GHz) -- DESIGN.md section 5.5.
+// Measured (B200, 1000 W cap): BASELINE configs[4] (16^3 x 32, nbasis 24) 15.3-15.9 ms per apply at nrhs 64 = 0.50-0.52 of the
+// HBM roof (the TF32 kernel: 31.5 ms), 12.6 ms at nrhs 32 (0.61), 11.5 ms at nrhs 16 (0.66).  The board sits at its power cap
+// at every width (SM clock 1.1 GHz at nrhs 64, 1.45 at 16): with the MMAs, the loaders' moves, the stencil-matrix bytes or the
+// X-tile bytes left out (-DCMRHS_ABL=1..4: wrong results, timing only) the kernel takes 10.5 / 12.7 / 10.9 / 13.2 ms at nrhs 64
+// but the SAME 17-18 M cycles per CTA -- less work buys clock, not cycles: energy per apply is the bound.
 #pragma once
 #ifndef CMRHS_ABL
-#define CMRHS_ABL 0
+#define CMRHS_ABL 0        // 1 no MMAs, 2 loaders move nothing, 3 / 4 the bulk copies of stencil matrices / X tiles carry 16 bytes: TIMING ONLY
 #endif
 
 #include "stencil_h16.cuh"
