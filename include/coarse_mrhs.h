@@ -277,6 +277,27 @@ int block_cg_solve_host_ex(coarse_op_t *op, const void *B_host, void *X_host, in
  */
 int coarse_block_gram(coarse_op_t *op, const void *U_dev, const void *W_dev, void *G_dev, int64_t n,
                       int32_t s, void *stream);
+/*
+ * coarse_block_gram_noalloc -- the same G = U^H W for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it) and so cannot hold a handle (coarse_op_create allocates).
+ * It takes no handle and allocates nothing: no cudaMalloc / cudaFree / allocating library routine on any call, the first
+ * included.  The per-CTA partial sums of the two-stage reduction live in a file-scope device array of
+ * COARSE_NOALLOC_SCRATCH_BYTES (4 MiB) that every GPU holds from the moment it loads the library until the process exits.
+ *   dtype        : COARSE_C64 or COARSE_C128 (U, W: [n][s] in dtype, device, 16-byte aligned; caller-owned, read only)
+ *   G_dev        : [s][s] complex128, row-major, device, 16-byte aligned; caller-owned, overwritten
+ *   n >= 1, 1 <= s <= COARSE_NOALLOC_MAX_NRHS (32).  A larger s returns COARSE_UNSUPPORTED with a message naming the limit
+ *                  and leaves G untouched; use coarse_block_gram for it.
+ *   stream       : the two kernels are launched on it; nothing synchronises.
+ * EVERY call on a device shares the one array: calls that overlap on the GPU (different streams, different host threads)
+ * race -- order them on one stream or with events.  The array keeps the last call's contents; nothing in it has to be
+ * zero (each launch overwrites every partial it later reads).  Deterministic; SIMT kernels only (widths <= 32 never take
+ * the tensor path of coarse_block_gram either), same arithmetic as coarse_block_gram up to the order of the partial sums.
+ * Errors: COARSE_INVALID_ARG (NULL, dtype, n, s < 1, alignment), COARSE_UNSUPPORTED (s beyond the limit), CUDA errors.
+ */
+#define COARSE_NOALLOC_MAX_NRHS 32
+#define COARSE_NOALLOC_SCRATCH_BYTES (256 * 32 * 32 * 16)
+int coarse_block_gram_noalloc(int32_t dtype, const void *U_dev, const void *W_dev, void *G_dev, int64_t n, int32_t s,
+                              void *stream);
 int coarse_small_cholesky(const void *G_dev, void *S_dev, void *Sinv_dev /* may be NULL */, int32_t s,
                           int32_t *info_dev, void *stream);
 int coarse_small_hpd_inverse(const void *G_dev, void *M_dev, int32_t s, int32_t *info_dev, void *stream);

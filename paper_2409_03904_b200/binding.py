@@ -26,7 +26,7 @@ EXPORTS = [
     "coarse_block_rotate", "coarse_op_fill_synthetic", "coarse_fill_block", "coarse_op_kernel_name",
     "coarse_op_device_bytes", "coarse_launch_count", "coarse_last_error", "coarse_op_profile", "coarse_op_profile_read",
     "coarse_cheby_apply", "coarse_deflate", "coarse_cheby_defl_solve", "pblock_cg_solve", "stacked_cg_solve", "coarse_block_project", "coarse_block_promote",
-    "block_cg_solve_ex", "block_cg_solve_host_ex", "coarse_measure_peaks",
+    "block_cg_solve_ex", "block_cg_solve_host_ex", "coarse_measure_peaks", "coarse_block_gram_noalloc",
 ]
 
 
@@ -95,6 +95,7 @@ def lib():
             "pblock_cg_solve": (C.c_int, [vp, vp, vp, i32, dbl, i32, C.POINTER(CoarsePrecond), C.POINTER(BlockCGResult), vp]),
             "coarse_cheby_defl_solve": (C.c_int, [vp, vp, C.POINTER(dbl), i32, vp, vp, i32, dbl, dbl, i32, vp]),
             "coarse_measure_peaks": (C.c_int, [C.POINTER(dbl), i32, vp, i64, vp]),
+            "coarse_block_gram_noalloc": (C.c_int, [i32, vp, vp, vp, i64, i32, vp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -143,6 +144,23 @@ def measure_peaks(scratch_bytes: int = 4 << 30, stream=None) -> dict:
     _check(lib().coarse_measure_peaks(out, 5, _dev(scratch), C.c_int64(scratch.numel() * 4), _stream(stream)))
     del scratch
     return dict(hbm_read_gbs=out[0], ffma_tflops=out[1], ffma2_tflops=out[2], dfma_tflops=out[3], dmma_tflops=out[4])
+
+
+NOALLOC_MAX_NRHS, NOALLOC_SCRATCH_BYTES = 32, 256 * 32 * 32 * 16
+
+
+def block_gram_noalloc(U: torch.Tensor, W: torch.Tensor, G: torch.Tensor, stream=None) -> torch.Tensor:
+    """coarse_block_gram_noalloc: G = U^H W into the caller's [s][s] complex128 CUDA tensor, without a handle and without any
+    allocation (the reduction scratch is a static device array of NOALLOC_SCRATCH_BYTES; s <= NOALLOC_MAX_NRHS; calls that
+    overlap on the GPU race on it).  This wrapper allocates nothing either."""
+    s = int(U.shape[-1])
+    if U.dtype not in (torch.complex64, torch.complex128) or W.dtype != U.dtype or W.shape != U.shape:
+        raise ValueError("U and W: complex64 or complex128 blocks of one shape")
+    if G.dtype != torch.complex128 or tuple(G.shape) != (s, s):
+        raise ValueError("G: [s][s] complex128")
+    _check(lib().coarse_block_gram_noalloc(C64 if U.dtype == torch.complex64 else C128, _dev(U), _dev(W), _dev(G), U.numel() // s, s,
+                                           _stream(stream)))
+    return G
 
 
 class CoarseOperator:

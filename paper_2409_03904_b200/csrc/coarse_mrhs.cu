@@ -1581,6 +1581,82 @@ extern "C" int coarse_op_profile_read(coarse_op_t *op, double *ms, int32_t capac
     return COARSE_OK;
 }
 
+// ---- Gram product without any allocation (coarse_mrhs.h: coarse_block_gram_noalloc) -----------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it) and
+// therefore cannot hold a coarse_op handle, whose create allocates the scratch of coarse_block_gram.  The per-CTA partial
+// sums of stage 1 live in a file-scope device array instead: every GPU that loads the library holds these 4 MiB until exit.
+// In HOST code the array's name is a host-side stand-in, not a device address: the address a kernel may be given comes from
+// cudaGetSymbolAddress, asked once per device with that device current (below).  Every call shares the array: calls that
+// overlap on the GPU (two streams, two host threads) race.  Every CTA of stage 1 writes its whole partial and stage 2 reads
+// only the partials of this launch, so nothing has to start at zero and the last call's contents do not matter.
+constexpr int kNoallocMaxS = COARSE_NOALLOC_MAX_NRHS;        // 32
+constexpr int kNoallocBlocks = 256;                          // CTAs of stage 1 (>= 1 per SM on B200)
+static __device__ __align__(256) unsigned char g_noalloc_gram_scratch[(size_t)kNoallocBlocks * kNoallocMaxS * kNoallocMaxS * sizeof(zdouble)];
+static_assert(sizeof(g_noalloc_gram_scratch) == COARSE_NOALLOC_SCRATCH_BYTES, "coarse_mrhs.h states the size of the static scratch");
+
+constexpr int kNoallocMaxDev = 64;
+static std::mutex g_noalloc_mu;
+static zdouble *g_noalloc_ptr[kNoallocMaxDev];               // device address of the array on device d (nullptr: not asked yet)
+
+static int noalloc_scratch(zdouble **out)
+{
+    int dev = 0;
+    CMRHS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoallocMaxDev) { set_error("coarse_block_gram_noalloc: device index %d beyond %d", dev, kNoallocMaxDev - 1); return COARSE_UNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void *ptr = nullptr;
+        CMRHS_CUDA(cudaGetSymbolAddress(&ptr, g_noalloc_gram_scratch));       // of the CURRENT device's copy of the array
+        if (!ptr) { set_error("cudaGetSymbolAddress returned a null address"); return COARSE_CUDA_ERROR; }
+        g_noalloc_ptr[dev] = static_cast<zdouble *>(ptr);
+    }
+    *out = g_noalloc_ptr[dev];
+    return COARSE_OK;
+}
+
+template <typename T>
+static int gram_noalloc_impl(const void *U, const void *W, zdouble *G, int64_t n, int s, zdouble *partial, cudaStream_t stream)
+{
+    // stage 1 as gram_impl's SIMT path, with the run-time-width kernels and a row tile of 32 KB: static + dynamic shared memory stay
+    // below the 48 KB every kernel may use without an attribute call
+    const int TT = s >= 8 ? 2 : 1;
+    const int nt = (s + TT - 1) / TT;
+    const int RG = kLaThreads / (nt * nt);
+    int rows = (int)(32768 / (2 * (size_t)s * sizeof(cplx<T>)));
+    rows = rows / RG * RG;
+    if (rows < RG) rows = RG;
+    size_t smem = (size_t)rows * s * 2 * sizeof(cplx<T>);
+    if (RG > 1 && smem < (size_t)s * s * sizeof(zdouble)) smem = (size_t)s * s * sizeof(zdouble);
+    int blocks = kNoallocBlocks;
+    if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
+    if (blocks < 1) blocks = 1;
+    const cplx<T> *u = static_cast<const cplx<T> *>(U), *w = static_cast<const cplx<T> *>(W);
+    if (TT == 2) gram_partial_kernel<T, 2><<<blocks, kLaThreads, smem, stream>>>(u, w, n, s, rows, partial);
+    else gram_partial_kernel<T, 1><<<blocks, kLaThreads, smem, stream>>>(u, w, n, s, rows, partial);
+    CMRHS_LAUNCH_CHECK();
+    gram_reduce_kernel<<<(s * s * 32 + 127) / 128, 128, 0, stream>>>(partial, blocks, s * s, G);
+    CMRHS_LAUNCH_CHECK();
+    return COARSE_OK;
+}
+
+extern "C" int coarse_block_gram_noalloc(int32_t dtype, const void *U_dev, const void *W_dev, void *G_dev, int64_t n, int32_t s, void *stream)
+{
+    if (!U_dev || !W_dev || !G_dev) { set_error("NULL argument"); return COARSE_INVALID_ARG; }
+    if (dtype != COARSE_C64 && dtype != COARSE_C128) { set_error("dtype must be COARSE_C64 or COARSE_C128"); return COARSE_INVALID_ARG; }
+    if (n < 1 || s < 1) { set_error("bad n/s"); return COARSE_INVALID_ARG; }
+    if (s > kNoallocMaxS) {
+        set_error("coarse_block_gram_noalloc: nrhs %d beyond COARSE_NOALLOC_MAX_NRHS = %d (the static scratch holds %d partials of %d x %d); use coarse_block_gram",
+                  (int)s, kNoallocMaxS, kNoallocBlocks, kNoallocMaxS, kNoallocMaxS);
+        return COARSE_UNSUPPORTED;
+    }
+    if (misaligned16(U_dev) || misaligned16(W_dev) || misaligned16(G_dev)) { set_error("U, W and G must be 16-byte aligned"); return COARSE_INVALID_ARG; }
+    zdouble *partial = nullptr;
+    const int st = noalloc_scratch(&partial);
+    if (st != COARSE_OK) return st;
+    return dtype == COARSE_C64 ? gram_noalloc_impl<float>(U_dev, W_dev, static_cast<zdouble *>(G_dev), n, s, partial, (cudaStream_t)stream)
+                               : gram_noalloc_impl<double>(U_dev, W_dev, static_cast<zdouble *>(G_dev), n, s, partial, (cudaStream_t)stream);
+}
+
 #ifdef CMRHS_TC_TRACE
 // developer diagnostic (not part of the ABI): per-CTA, per-warp cycle counters of the last tensor-kernel launch
 extern "C" int coarse_debug_trace_read(long long *out)
