@@ -110,6 +110,126 @@ gram_partial_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W
     for (int e = threadIdx.x; e < s * s; e += kLaThreads) { out[e].re = red[2 * e]; out[e].im = red[2 * e + 1]; }
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Gram product, stage 1, PIPELINED form for the widths block CG runs at in complex64 (S = 16, 32 at compile time).
+// gram_partial_kernel above stages a tile with per-thread loads and then works on it: with 5 CTAs per SM that keeps ~20 KB
+// per SM in flight and measured 129 us at the headline shape (1.33 M rows x 16: 340 MB, 51 us at the HBM roof).  Here a tile of
+// consecutive rows -- ONE contiguous range of the [n][S] block -- arrives by a bulk copy per operand into a ring of
+// kGramPipeStages stages (one elected thread issues, an mbarrier per stage counts the bytes), 2 CTAs per SM, 4 x 4 sub-blocks
+// per thread (two 16-byte shared-memory loads per operand and row for 16 complex multiply-adds).  Same arithmetic contract as
+// above: products and runs of <= 36 rows in T, flushed to double; fixed partition and order (deterministic).
+// ------------------------------------------------------------------------------------------------------
+constexpr int kGramPipeStages = 3;
+
+template <typename T, int TT>
+__device__ __forceinline__ void gram_pipe_load(cplx<T> (&v)[TT], const cplx<T> *p)
+{
+    if constexpr (sizeof(T) == 4 && TT % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < TT / 2; ++i) {
+            const float4 q = reinterpret_cast<const float4 *>(p)[i];
+            v[2 * i] = {q.x, q.y};
+            v[2 * i + 1] = {q.z, q.w};
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < TT; ++i) v[i] = p[i];
+    }
+}
+
+template <typename T, int TT, int S>
+__global__ void __launch_bounds__(kLaThreads, 2)
+gram_pipe_kernel(const cplx<T> *__restrict__ U, const cplx<T> *__restrict__ W, int64_t n, int rows, int flush_tiles, zdouble *__restrict__ partial)
+{
+    constexpr int NT = S / TT, NTILE = NT * NT, RG = kLaThreads / NTILE;
+    static_assert(S % TT == 0 && kLaThreads % NTILE == 0 && (S * sizeof(cplx<T>)) % 16 == 0, "gram_pipe tiling");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const size_t tile_bytes = (size_t)rows * S * sizeof(cplx<T>);            // one operand's tile; a stage = [U tile | W tile]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)kGramPipeStages * 2 * tile_bytes);
+    const int tile = threadIdx.x % NTILE, rg = threadIdx.x / NTILE;
+    const int a0 = (tile / NT) * TT, b0 = (tile % NT) * TT;
+
+    const int64_t chunk = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t r_begin = blockIdx.x * chunk;
+    const int64_t r_end = (r_begin + chunk < n) ? r_begin + chunk : n;
+    const int64_t ntiles = r_end > r_begin ? (r_end - r_begin + rows - 1) / rows : 0;
+    if (threadIdx.x == 0) {
+        for (int st = 0; st < kGramPipeStages; ++st) mbar_init(&full[st], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint64_t pol = 0;
+    if (threadIdx.x == 0) pol = l2_policy_evict_first();
+    auto issue = [&](int64_t t) {                 // thread 0 only
+        const int st = (int)(t % kGramPipeStages);
+        const int64_t r0 = r_begin + t * rows;
+        const uint32_t bytes = (uint32_t)(((r_end - r0 < rows) ? (r_end - r0) : rows) * S * sizeof(cplx<T>));
+        unsigned char *dst = smem_raw + (size_t)st * 2 * tile_bytes;
+        mbar_arrive_expect_tx(&full[st], 2u * bytes);
+        bulk_g2s(dst, U + r0 * S, bytes, &full[st], pol);
+        bulk_g2s(dst + tile_bytes, W + r0 * S, bytes, &full[st], pol);
+    };
+    if (threadIdx.x == 0)
+        for (int64_t t = 0; t < kGramPipeStages - 1 && t < ntiles; ++t) issue(t);
+
+    double accr[TT][TT], acci[TT][TT];
+    cplx<T> run[TT][TT];
+#pragma unroll
+    for (int a = 0; a < TT; ++a)
+#pragma unroll
+        for (int b = 0; b < TT; ++b) { accr[a][b] = 0.0; acci[a][b] = 0.0; run[a][b].re = 0; run[a][b].im = 0; }
+
+    int st = 0, since_flush = 0;
+    uint32_t parity = 0;
+    for (int64_t t = 0; t < ntiles; ++t) {
+        // the stage tile t + STAGES - 1 goes to was read last for tile t - 1: every thread is past the __syncthreads that ended it
+        if (threadIdx.x == 0 && t + kGramPipeStages - 1 < ntiles) { fence_proxy_async_smem(); issue(t + kGramPipeStages - 1); }
+        const int64_t r0 = r_begin + t * rows;
+        const int nrow = (int)((r_end - r0 < rows) ? (r_end - r0) : rows);
+        mbar_wait(&full[st], parity);
+        const cplx<T> *sU = reinterpret_cast<const cplx<T> *>(smem_raw + (size_t)st * 2 * tile_bytes);
+        const cplx<T> *sW = reinterpret_cast<const cplx<T> *>(smem_raw + (size_t)st * 2 * tile_bytes + tile_bytes);
+        for (int k = rg; k < nrow; k += RG) {
+            cplx<T> u[TT], w[TT];
+            gram_pipe_load<T, TT>(u, sU + k * S + a0);
+            gram_pipe_load<T, TT>(w, sW + k * S + b0);
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) cmac_conj(run[a][b], u[a], w[b]);
+        }
+        if (++since_flush == flush_tiles || t + 1 == ntiles) {
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) {
+                    accr[a][b] += (double)run[a][b].re; acci[a][b] += (double)run[a][b].im;
+                    run[a][b].re = 0; run[a][b].im = 0;
+                }
+            since_flush = 0;
+        }
+        if (++st == kGramPipeStages) { st = 0; parity ^= 1u; }
+        __syncthreads();
+    }
+    // row groups in a fixed order (0, 1, 2, ...) through shared memory: every copy has landed and been read, the ring is free
+    double *red = reinterpret_cast<double *>(smem_raw);
+    for (int g = 0; g < RG; ++g) {
+        if (rg == g) {
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) {
+                    const int e = (a0 + a) * S + b0 + b;
+                    if (g == 0) { red[2 * e] = accr[a][b]; red[2 * e + 1] = acci[a][b]; }
+                    else { red[2 * e] += accr[a][b]; red[2 * e + 1] += acci[a][b]; }
+                }
+        }
+        __syncthreads();
+    }
+    zdouble *out = partial + (size_t)blockIdx.x * S * S;
+    for (int e = threadIdx.x; e < S * S; e += kLaThreads) { out[e].re = red[2 * e]; out[e].im = red[2 * e + 1]; }
+}
+
 // stage 2: G[e] = sum_b partial[b][e], b in increasing order
 // One warp per entry: lane l sums blocks l, l + 32, ... in increasing order, then a fixed shuffle tree.
 __global__ void gram_reduce_kernel(const zdouble *__restrict__ partial, int nblocks, int ss, zdouble *__restrict__ G)

@@ -502,6 +502,32 @@ static int gram_impl(const coarse_op *op, const void *U, const void *W, zdouble 
         CMRHS_LAUNCH_CHECK();
         return COARSE_OK;
     }
+#ifndef CMRHS_NO_GRAM_PIPE      // (A/B builds: the staged kernel below for every width)
+    if constexpr (sizeof(T) == 4) if ((s == 16 || s == 32) && n >= 4096) {       // complex64 at the widths block CG runs at: bulk-copy pipeline (gram_pipe_kernel)
+        constexpr int kTT = 4;
+        const int RGp = kLaThreads / ((s / kTT) * (s / kTT));          // 16 / 4 row groups
+        const int rows = 12288 / (s * (int)sizeof(cplx<T>));           // 12 KB per operand and stage: 96 / 48 rows
+        const int flush = 36 / (rows / RGp);                           // runs of 36 rows in T between flushes to double
+        const size_t smem = (size_t)kGramPipeStages * 2 * rows * s * sizeof(cplx<T>) + kGramPipeStages * sizeof(uint64_t);
+        int blocks = 2 * op->num_sms;
+        if (blocks > op->gram_blocks) blocks = op->gram_blocks;
+        if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
+        const cplx<T> *u = (const cplx<T> *)U, *w = (const cplx<T> *)W;
+        if (s == 16) {
+            auto kern = gram_pipe_kernel<T, kTT, 16>;
+            CMRHS_SMEM_ATTR(kern, smem);
+            kern<<<blocks, kLaThreads, smem, stream>>>(u, w, n, rows, flush, op->gram_partial);
+        } else {
+            auto kern = gram_pipe_kernel<T, kTT, 32>;
+            CMRHS_SMEM_ATTR(kern, smem);
+            kern<<<blocks, kLaThreads, smem, stream>>>(u, w, n, rows, flush, op->gram_partial);
+        }
+        CMRHS_LAUNCH_CHECK();
+        gram_reduce_kernel<<<(s * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, s * s, G);
+        CMRHS_LAUNCH_CHECK();
+        return COARSE_OK;
+    }
+#endif
     int TT = s > 32 ? 4 : (s >= 8 ? 2 : 1);
     const int nt = (s + TT - 1) / TT;
     const int RG = kLaThreads / (nt * nt);
