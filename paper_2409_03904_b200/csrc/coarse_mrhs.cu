@@ -1169,13 +1169,16 @@ static int cheby_impl(coarse_op *op, const void *B_dev, void *X_dev, int nrhs, d
     void *Z = op->blk[2], *Ta = op->blk[0], *Tb = op->blk[1];
     const int64_t cvec = ceil_div(total, (int64_t)(32 / op->esize) * 256);
     const int grid = (int)(cvec < (int64_t)op->num_sms * 8 ? (cvec < 1 ? 1 : cvec) : (int64_t)op->num_sms * 8);
+    // the split-FP16 apply scales every column of its input by a power of two: the step that writes T_{j+1} also finds its column maxima
+    uint32_t *colmax = (op->dtype == COARSE_C64 && use_split16(op, nrhs)) ? op->amax : nullptr;
     auto step = [&](const void *z, const void *tc, void *tp, double ca, double cb, double cp, double cx, double cn) -> int {
+        if (colmax) CMRHS_CUDA(cudaMemsetAsync(colmax, 0, 64 * sizeof(uint32_t), stream));
         if (op->dtype == COARSE_C64)
             cheby_step_kernel<float><<<grid, 256, 0, stream>>>((const cplx<float> *)z, (const cplx<float> *)tc, (cplx<float> *)tp,
-                                                               (cplx<float> *)X_dev, (float)ca, (float)cb, (float)cp, (float)cx, (float)cn, total);
+                                                               (cplx<float> *)X_dev, (float)ca, (float)cb, (float)cp, (float)cx, (float)cn, total, nrhs, colmax);
         else
             cheby_step_kernel<double><<<grid, 256, 0, stream>>>((const cplx<double> *)z, (const cplx<double> *)tc, (cplx<double> *)tp,
-                                                                (cplx<double> *)X_dev, ca, cb, cp, cx, cn, total);
+                                                                (cplx<double> *)X_dev, ca, cb, cp, cx, cn, total, nrhs, nullptr);
         CMRHS_LAUNCH_CHECK();
         return COARSE_OK;
     };
@@ -1190,7 +1193,7 @@ static int cheby_impl(coarse_op *op, const void *B_dev, void *X_dev, int nrhs, d
     CMRHS_CUDA(cudaMemcpyAsync(Tb, B_dev, blk_bytes, cudaMemcpyDeviceToDevice, stream));               // T_prev = T_0
     void *tc = Ta, *tp = Tb;
     for (int j = 1; j < n - 1; ++j) {
-        CMRHS_STEP(apply_impl(op, tc, Z, nrhs, stream));                                               // Z = H T_j
+        CMRHS_STEP(apply_impl(op, tc, Z, nrhs, stream, colmax != nullptr));                            // Z = H T_j (column maxima of T_j: from the step that wrote it)
         CMRHS_STEP(step(Z, tc, tp, 2.0 * alpha, 2.0 * beta, 1.0, 1.0, c[(size_t)j + 1]));              // T_{j+1} -> tp ; X += c_{j+1} T_{j+1}
         void *t = tc; tc = tp; tp = t;
     }
