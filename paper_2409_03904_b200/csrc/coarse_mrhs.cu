@@ -632,7 +632,10 @@ static FusedPlan fused_plan(const coarse_op *op, int64_t n, int s)
     p.W = s >= LA_W4_FROM ? 4 : (s >= 8 ? 2 : 1);
     if ((s + p.W - 1) / p.W > 16) p.W = 4;
     const int ncg = (s + p.W - 1) / p.W, RL = kLaThreads / ncg, su = s + LaPad<T>::v;
-    int tr0 = 4;
+#ifndef LA_TR0
+#define LA_TR0 2      // complex64, width 16: 64-row tiles, 4 CTAs per SM (other_ms 0.693 -> 0.675 against TR 4 with 2 CTAs; TR 8: 0.765; W 4: 0.97)
+#endif
+    int tr0 = (s == 16 && sizeof(T) == 4) ? LA_TR0 : 4;
     for (p.TR = tr0; ; p.TR /= 2) {
         p.rows = RL * p.TR;
         size_t tiles = (size_t)4 * p.rows * su * sizeof(cplx<T>);      // two operands x two stages
@@ -685,6 +688,9 @@ static int fused2_launch(const coarse_op *op, const FusedPlan &p, const void *Ti
         if (p.TR == 4) return CALL(4, 4, 64); if (p.TR == 2) return CALL(2, 4, 64); return CALL(1, 4, 64); \
     }                                                                    \
     if (p.W == 4 && p.TR == 4 && s == 32) return CALL(4, 4, 32);         \
+    if (p.W == 4 && p.TR == 4 && s == 16) return CALL(4, 4, 16);         \
+    if (p.W == 2 && p.TR == 2 && s == 16) return CALL(2, 2, 16);         \
+    if (p.W == 2 && p.TR == 8 && s == 16) return CALL(8, 2, 16);         \
     if (p.TR == 4) {                                                     \
         if (p.W == 4) return CALL(4, 4); if (p.W == 2) return CALL(4, 2); return CALL(4, 1); \
     }                                                                    \
