@@ -77,7 +77,7 @@ using V_d24_s8 = SimtConfig<double, 24, 3, 2, 4, 3, 3, 16>;
 using V_d8_s4 = SimtConfig<double, 8, 1, 1, 4, 1, 8, 16>;
 using V_d32_s16 = SimtConfig<double, 32, 4, 4, 4, 4, 4, 8>;
 // complex128 on the FP64 tensor path (DMMA):   NB  S KSPLIT STAGES WARPS
-using D_d24_s8 = DmmaConfig<24, 8, 1, 2, 8>;       // (whole stencil matrices per stage: 0.614 ms at configs[1]; KSPLIT 3 with 16 warps: 0.71, SIMT: 0.624)
+using D_d24_s8 = DmmaConfig<24, 8, 1, 2, 8>;       // (whole stencil matrices per stage: 0.614 ms at configs[1], 0.538 with the balanced partition; KSPLIT 3 with 16 warps: 0.71, SIMT: 0.624)
 using D_d32_s16 = DmmaConfig<32, 16, 4, 4, 8>;
 using D_d24_s16 = DmmaConfig<24, 16, 3, 4, 8>;
 using D_d32_s8 = DmmaConfig<32, 8, 4, 3, 12>;

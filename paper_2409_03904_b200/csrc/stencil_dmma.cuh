@@ -17,6 +17,14 @@
 // serves together hold 2 rows x 4 k, and the k rows of the bulk-copied tile are 384 / 512 bytes apart -- a 4-way bank conflict.
 // Padding the rows (one bulk copy per k row) removes it but costs more than it saves (48 copies of 128-416 bytes per stage:
 // configs[1] 0.61 -> 0.90 ms), so the tile keeps its one-copy layout.
+//
+// BALANCED mode (template flag BAL; chosen by the launcher for small lattices).  With whole sites per warp the kernel's time is
+// quantised: configs[1] has 4096 sites for 148 x 8 = 1184 warps, 3.46 on average but 4 for the slowest -- measured: V = 4096 and
+// V = 4736 (exactly 4 each) both take 0.614 ms (5.0 against 5.8 TB/s).  In balanced mode every warp takes one contiguous range of
+// the V x 81 (site, stencil point) sequence, cut at equal counts wherever that falls; a site that two warps share is added into a
+// zeroed Y with atomicAdd (double) by both -- two terms onto zero: the sum does not depend on their order, so the result stays
+// bit-reproducible.  The launcher takes this mode only when every warp gets at least 81 points (no site is shared by three).
+// configs[1]: 0.614 -> 0.538 ms (5.73 TB/s, 0.85 of the HBM roof).
 #pragma once
 
 #include "stencil_simt.cuh"
@@ -42,7 +50,7 @@ __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b)
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-template <class C>
+template <class C, bool BAL>
 __global__ void __launch_bounds__(C::THREADS, 1)
 stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restrict__ nbr, const cplx<double> *__restrict__ X,
                     cplx<double> *__restrict__ Y, int64_t V)
@@ -55,11 +63,16 @@ stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restri
     constexpr int NN = C::NB * C::NB, NS = C::NB * C::S;
     constexpr unsigned FULL = 0xffffffffu;
 
-    const int64_t stride = (int64_t)gridDim.x * C::WARPS;
-    const int64_t first = (int64_t)blockIdx.x * C::WARPS + warp;
-    if (first >= V) return;
-    const int64_t nsites = (V - first + stride - 1) / stride;
-    const int64_t nchunks = nsites * C::CPS;
+    // whole sites, interleaved over the warps (site = first + j stride) -- or, balanced, the points [pt_begin, pt_end) of the sequence
+    // g = site * 81 + q (q = position in the site's accumulation order)
+    const int64_t stride = BAL ? 1 : (int64_t)gridDim.x * C::WARPS;
+    const int64_t nwarps = (int64_t)gridDim.x * C::WARPS, wid = (int64_t)blockIdx.x * C::WARPS + warp;
+    const int64_t pt_begin = BAL ? V * kNPoint * wid / nwarps : 0, pt_end = BAL ? V * kNPoint * (wid + 1) / nwarps : 0;
+    const int64_t first = BAL ? pt_begin / kNPoint : wid;
+    if (BAL ? pt_begin >= pt_end : first >= V) return;
+    const int64_t nsites = BAL ? 0 : (V - first + stride - 1) / stride;
+    const int64_t nchunks = BAL ? (pt_end - pt_begin) * C::KSPLIT : nsites * C::CPS;
+    const int w0 = BAL ? (int)(pt_begin - first * kNPoint) * C::KSPLIT : 0;        // chunk of the first site this warp starts at
     if (lane == 0) {
         for (int st = 0; st < C::STAGES; ++st) mbar_init(&full_bar[st], 1);
         mbar_fence_init();
@@ -70,7 +83,7 @@ stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restri
 
     // ---- issue side (as stencil_simt.cuh) ----
     int64_t ix = first;
-    int iw = 0;
+    int iw = w0;
     int32_t n0, n1, n2;
     auto load_nbr_row = [&](int64_t x) {
         const int32_t *row = nbr + x * kNPoint;
@@ -111,7 +124,8 @@ stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restri
             for (int e = 0; e < 2; ++e) { p0[m][n][e] = 0.0; q0[m][n][e] = 0.0; p1[m][n][e] = 0.0; q1[m][n][e] = 0.0; }
 
     int64_t cx = first;
-    int cw = 0, st = 0;
+    int cw = w0, st = 0;
+    bool whole = w0 == 0;                     // (balanced) this warp accumulates every point of site cx
     uint32_t parity = 0;
     for (int64_t c = 0; c < nchunks; ++c) {
         mbar_wait(&full_bar[st], parity);
@@ -139,8 +153,9 @@ stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restri
         if (issued < nchunks) { issue(st); ++issued; }
         if (++st == C::STAGES) { st = 0; parity ^= 1u; }
 
-        if (++cw == C::CPS) {                 // site finished: C fragment of lane l = rows 8 m + l/4, right-hand sides 8 n + 2 (l%4), + 1
+        if (++cw == C::CPS || (BAL && c + 1 == nchunks)) {       // site (or this warp's part of it) finished: C fragment of lane l = rows 8 m + l/4, right-hand sides 8 n + 2 (l%4), + 1
             Z *yout = Y + cx * (int64_t)NS;
+            const bool shared_site = BAL && !(whole && cw == C::CPS);      // another warp holds the rest of this site: both add into the zeroed Y
 #pragma unroll
             for (int m = 0; m < C::MT; ++m)
 #pragma unroll
@@ -149,13 +164,19 @@ stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restri
                     o.x = p0[m][n][0] - q1[m][n][0]; o.y = p1[m][n][0] + q0[m][n][0];
                     o.z = p0[m][n][1] - q1[m][n][1]; o.w = p1[m][n][1] + q0[m][n][1];
                     double2 *dst = reinterpret_cast<double2 *>(yout + (8 * m + fr) * C::S + 8 * n + 2 * fk);
-                    dst[0] = make_double2(o.x, o.y);
-                    dst[1] = make_double2(o.z, o.w);
+                    if (shared_site) {
+                        double *d = reinterpret_cast<double *>(dst);
+                        atomicAdd(d, o.x); atomicAdd(d + 1, o.y); atomicAdd(d + 2, o.z); atomicAdd(d + 3, o.w);
+                    } else {
+                        dst[0] = make_double2(o.x, o.y);
+                        dst[1] = make_double2(o.z, o.w);
+                    }
 #pragma unroll
                     for (int e = 0; e < 2; ++e) { p0[m][n][e] = 0.0; q0[m][n][e] = 0.0; p1[m][n][e] = 0.0; q1[m][n][e] = 0.0; }
                 }
             cw = 0;
             cx += stride;
+            whole = true;
         }
     }
 }
@@ -164,11 +185,20 @@ template <class C>
 int launch_stencil_dmma(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
 {
     using Z = cplx<double>;
-    auto kern = stencil_dmma_kernel<C>;
-    CMRHS_SMEM_ATTR(kern, C::SMEM_BYTES);
     const int64_t nctas = (V + C::WARPS - 1) / C::WARPS;
     const int grid = (int)(nctas < num_sms ? nctas : num_sms);
-    kern<<<grid, C::THREADS, C::SMEM_BYTES, stream>>>(static_cast<const Z *>(At), nbr, static_cast<const Z *>(X), static_cast<Z *>(Y), V);
+    // balanced mode: between 1 and 16 sites per warp, where the whole-site partition loses up to a site's time per warp
+    const int64_t nwarps = (int64_t)grid * C::WARPS;
+    if (V >= nwarps && V < 16 * nwarps && V % nwarps != 0) {
+        auto kern = stencil_dmma_kernel<C, true>;
+        CMRHS_SMEM_ATTR(kern, C::SMEM_BYTES);
+        CMRHS_CUDA(cudaMemsetAsync(Y, 0, (size_t)V * C::NB * C::S * sizeof(Z), stream));
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, stream>>>(static_cast<const Z *>(At), nbr, static_cast<const Z *>(X), static_cast<Z *>(Y), V);
+    } else {
+        auto kern = stencil_dmma_kernel<C, false>;
+        CMRHS_SMEM_ATTR(kern, C::SMEM_BYTES);
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, stream>>>(static_cast<const Z *>(At), nbr, static_cast<const Z *>(X), static_cast<Z *>(Y), V);
+    }
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
 }

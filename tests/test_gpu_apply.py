@@ -156,6 +156,26 @@ def test_errors_are_reported_not_swallowed():
     op.close()
 
 
+# complex128 on the FP64 tensor path, lattices of 1 to 16 sites per warp: the kernel's BALANCED partition (stencil_dmma.cuh) cuts the
+# (site, stencil point) sequence at equal counts, so two warps share most sites and add their parts into a zeroed Y.
+# (6,6,6,6) with 8 warps per CTA: 1296 sites for 1184 warps (88.7 points each: almost every site is shared); (7,7,7,7) with 16.
+@pytest.mark.parametrize("dims,nb,s", [((6, 6, 6, 6), 24, 8), ((6, 6, 6, 6), 16, 16), ((7, 7, 7, 7), 8, 8), ((6, 6, 6, 7), 24, 8)])
+def test_dmma_balanced_partition_matches_oracle_and_is_reproducible(dims, nb, s):
+    A, c, X, _ = host_case(dims, nb, s, seed=300 + nb + s, factor=1.05)
+    op = cm.CoarseOperator(dims, to_dev(A, "c128"), s)
+    assert op.kernel_name(s).startswith("stencil_dmma"), op.kernel_name(s)
+    Xd = to_dev(X, "c128")
+    Yd = torch.full_like(Xd, complex(np.nan, np.nan))        # the kernel's own zeroing, not the caller's
+    op.apply(Xd, Yd)
+    Y1 = to_np(Yd).copy()
+    Yd.fill_(7.0)
+    op.apply(Xd, Yd)
+    Y2 = to_np(Yd)
+    op.close()
+    assert rel_err_cols(Y1, oracle.apply(dims, A, X)) <= TOL["c128"]
+    assert np.array_equal(Y1, Y2)                            # two terms onto zero: the order of the atomic adds cannot show
+
+
 def _sampled_sites(dims, n_random, rng):
     """corners / faces of the periodic lattice plus random interior sites"""
     L = dims
