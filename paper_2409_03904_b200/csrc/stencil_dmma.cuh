@@ -182,7 +182,7 @@ stencil_dmma_kernel(const cplx<double> *__restrict__ At, const int32_t *__restri
 }
 
 template <class C>
-int launch_stencil_dmma(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
+int launch_stencil_dmma_as(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
 {
     using Z = cplx<double>;
     const int64_t nctas = (V + C::WARPS - 1) / C::WARPS;
@@ -201,6 +201,17 @@ int launch_stencil_dmma(const void *At, const int32_t *nbr, const void *X, void 
     }
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
+}
+
+// small lattices: CTAs of 2 or 4 warps when every site still gets its own warp in one round (stencil_simt.cuh: launch_stencil_simt)
+template <class C>
+int launch_stencil_dmma(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
+{
+    using C4 = DmmaConfig<C::NB, C::S, C::KSPLIT, C::STAGES, 4>;
+    using C2 = DmmaConfig<C::NB, C::S, C::KSPLIT, C::STAGES, 2>;
+    if (C::WARPS > 2 && (V + 1) / 2 <= num_sms) return launch_stencil_dmma_as<C2>(At, nbr, X, Y, V, num_sms, stream);
+    if (C::WARPS > 4 && (V + 3) / 4 <= num_sms) return launch_stencil_dmma_as<C4>(At, nbr, X, Y, V, num_sms, stream);
+    return launch_stencil_dmma_as<C>(At, nbr, X, Y, V, num_sms, stream);
 }
 
 }  // namespace cmrhs

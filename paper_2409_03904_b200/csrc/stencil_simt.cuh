@@ -201,7 +201,7 @@ stencil_simt_kernel(const cplx<typename C::real> *__restrict__ At, const int32_t
 }
 
 template <class C>
-int launch_stencil_simt(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
+int launch_stencil_simt_as(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
 {
     using Z = cplx<typename C::real>;
     auto kern = stencil_simt_kernel<C>;
@@ -212,6 +212,20 @@ int launch_stencil_simt(const void *At, const int32_t *nbr, const void *X, void 
                                                        static_cast<Z *>(Y), V);
     CMRHS_LAUNCH_CHECK();
     return COARSE_OK;
+}
+
+// Small lattices: with WARPS sites per CTA a lattice of a few hundred sites keeps only a few SMs busy (configs[0]: 256 sites = 16 CTAs of
+// 16 warps) and its warps share what ONE SM can pull from L2.  When every site still gets its own warp in a single round, the same
+// kernel with 2 or 4 warps per CTA spreads them over more SMs (configs[0]: 53.8 -> 32.8 us).  More rounds are never worth it: a site
+// costs its 81 dependent ring turns whatever else runs (6^4 sites on 296 warps: 149 against 58 us for 81 CTAs of 16 warps).
+template <class C>
+int launch_stencil_simt(const void *At, const int32_t *nbr, const void *X, void *Y, int64_t V, int num_sms, cudaStream_t stream)
+{
+    using C4 = SimtConfig<typename C::real, C::NB, C::TM, C::TN, C::GC, C::KSPLIT, C::STAGES, 4>;
+    using C2 = SimtConfig<typename C::real, C::NB, C::TM, C::TN, C::GC, C::KSPLIT, C::STAGES, 2>;
+    if (C::WARPS > 2 && (V + 1) / 2 <= num_sms) return launch_stencil_simt_as<C2>(At, nbr, X, Y, V, num_sms, stream);
+    if (C::WARPS > 4 && (V + 3) / 4 <= num_sms) return launch_stencil_simt_as<C4>(At, nbr, X, Y, V, num_sms, stream);
+    return launch_stencil_simt_as<C>(At, nbr, X, Y, V, num_sms, stream);
 }
 
 }  // namespace cmrhs
