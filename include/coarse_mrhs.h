@@ -240,7 +240,12 @@ int stacked_cg_solve(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t nr
  * Layouts (device, row-major, interleaved complex of `dtype`): Basis [Vc][vblock][nbasis], fine vectors [Vc][vblock][nrhs]
  * (the fine field block by block -- the paper's "BLAS ready layout"), coarse vectors [Vc][nbasis][nrhs] (the layout of
  * coarse_op_apply).  Stateless (no handle), asynchronous on `stream`, allocate nothing.  nbasis, nrhs <= 64.
- * Errors: COARSE_INVALID_ARG, launch errors.  (SIMT kernels, one CTA per coarse site; not tuned this round.)
+ * Errors: COARSE_INVALID_ARG, launch errors.
+ * Kernels: SIMT.  nbasis and nrhs multiples of 4 (Table 6's 64 x 12 and the coarse operator's shapes) take register-tiled,
+ * pipelined kernels (project: bulk-copied row tiles, several sites per CTA; promote: padded cp.async tiles) at 2.2-3.0 TB/s
+ * = 22-32 TFLOP/s on B200 -- both shapes are bound by the FP32 pipe, not by HBM; other shapes take a plain kernel (1.3-1.5 TB/s).
+ * Sums: project adds runs of <= 32 rows in `dtype` into the site's accumulator (double for complex128, float for complex64:
+ * error <= (32 + vblock/32) eps); promote sums its nbasis terms in `dtype`.
  */
 int coarse_block_project(const void *Basis_dev, const void *F_dev, void *C_dev, int64_t Vc, int32_t vblock, int32_t nbasis,
                          int32_t nrhs, int32_t dtype, void *stream);

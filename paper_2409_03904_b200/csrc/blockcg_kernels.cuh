@@ -5,8 +5,11 @@
 // Reductions are deterministic: fixed partition of rows over CTAs, fixed summation order, no float atomics.
 #pragma once
 
+#include <type_traits>
+
 #include "common.cuh"
 #include "ptx_async.cuh"
+#include "tcgen05_ptx.cuh"
 
 namespace cmrhs {
 
@@ -911,6 +914,212 @@ block_promote_kernel(const cplx<T> *__restrict__ Bas, const cplx<T> *__restrict_
             }
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Tuned forms of the two transfer kernels for nbasis and nrhs multiples of 4 (Table 6's shapes: nbasis 64 x nrhs 12 x V_block 256,
+// PAPER.md:570-571).  The kernels above do one output element per thread and two shared-memory loads per multiply-add
+// (measured: 1.3-1.5 TB/s = 0.2 of the HBM roof); these keep 4 x 4 (project) / TR x 4 (promote) complex results per thread.
+//
+// project: C[x] = Basis[x]^dagger F[x] is a rectangular Gram product per coarse site.  Thread tile 4 x 4; the (nb/4)(s/4) tiles of
+// a site are one GROUP of threads, and the G groups of a CTA work on G DIFFERENT sites at once (no reduction between groups, every
+// group runs all rows of its own tile).  A stage of the 3-stage ring holds `rows` rows of Basis[x] and F[x] for each of the G sites --
+// 2 G bulk copies of contiguous ranges, issued by a producer warp; full / empty mbarriers per stage, no CTA-wide barrier in the loop --
+// and the ring runs on across the CTA's sites.
+// Sums: products and runs of <= 32 rows in T, the runs added into the site's accumulator -- in double for complex128; for
+// complex64 in float (two-level summation: error <= (32 + V_block/32) eps, 1e-6 at V_block 3072 against the 1e-5 bar).
+// ------------------------------------------------------------------------------------------------------
+constexpr int kXferConsumers = kLaThreads - 32;   // 7 consumer warps + one producer warp = kLaThreads (two CTAs per SM keep 128 registers per thread)
+
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads, 2)
+block_project_pipe_kernel(const cplx<T> *__restrict__ Bas, const cplx<T> *__restrict__ F, cplx<T> *__restrict__ Cc, int64_t Vc, int vb, int nb, int s,
+                          int rows, int G, int flush_tiles)
+{
+    constexpr int TT = 4;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int ntb = s / TT, ntile = (nb / TT) * ntb;
+    const size_t bytesB = (size_t)rows * nb * sizeof(cplx<T>), bytesF = (size_t)rows * s * sizeof(cplx<T>);
+    const size_t site_stage = bytesB + bytesF, stage_bytes = (size_t)G * site_stage;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + kGramPipeStages * stage_bytes), *empty = full + kGramPipeStages;
+    const int tile = threadIdx.x % ntile, g = threadIdx.x / ntile;
+    const int a0 = (tile / ntb) * TT, b0 = (tile % ntb) * TT;
+
+    const int tps = (vb + rows - 1) / rows;                                   // tiles per site
+    // round j of this CTA: the G consecutive sites from (j gridDim + blockIdx) G
+    const int64_t nchunk = (Vc + G - 1) / G;                                  // chunks of G sites
+    const int64_t my_rounds = (int64_t)blockIdx.x < nchunk ? (nchunk - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const int64_t total = my_rounds * tps;
+    if (threadIdx.x == 0) {
+        for (int st = 0; st < kGramPipeStages; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], kXferConsumers / 32); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int64_t i, uint64_t pol) {   // one thread
+        const int st = (int)(i % kGramPipeStages);
+        const int64_t base = ((i / tps) * gridDim.x + blockIdx.x) * G;
+        const int nv = (int)((Vc - base < G) ? (Vc - base) : G);
+        const int v0 = (int)(i % tps) * rows, nrow = (vb - v0 < rows) ? (vb - v0) : rows;
+        const uint32_t nB = (uint32_t)((size_t)nrow * nb * sizeof(cplx<T>)), nF = (uint32_t)((size_t)nrow * s * sizeof(cplx<T>));
+        mbar_arrive_expect_tx(&full[st], (uint32_t)nv * (nB + nF));
+        for (int q = 0; q < nv; ++q) {
+            unsigned char *dst = smem_raw + (size_t)st * stage_bytes + (size_t)q * site_stage;
+            bulk_g2s(dst, Bas + ((base + q) * vb + v0) * (int64_t)nb, nB, &full[st], pol);
+            bulk_g2s(dst + bytesB, F + ((base + q) * vb + v0) * (int64_t)s, nF, &full[st], pol);
+        }
+    };
+    if (threadIdx.x >= kXferConsumers) {
+        // ---- producer warp: refills a stage as soon as the 7 consumer warps have released it ----
+        if (threadIdx.x == kXferConsumers) {
+            const uint64_t pol = l2_policy_evict_first();
+            for (int64_t i = 0; i < total; ++i) {
+                const int st = (int)(i % kGramPipeStages);
+                if (i >= kGramPipeStages) mbar_wait(&empty[st], (uint32_t)((i / kGramPipeStages - 1) & 1));
+                issue(i, pol);
+            }
+        }
+        return;
+    }
+
+    using Acc = typename std::conditional<sizeof(T) == 8, double, T>::type;
+    Acc accr[TT][TT], acci[TT][TT];
+    cplx<T> run[TT][TT];
+#pragma unroll
+    for (int a = 0; a < TT; ++a)
+#pragma unroll
+        for (int b = 0; b < TT; ++b) { accr[a][b] = 0; acci[a][b] = 0; run[a][b].re = 0; run[a][b].im = 0; }
+
+    int st = 0, since_flush = 0;
+    uint32_t parity = 0;
+    for (int64_t i = 0; i < total; ++i) {
+        const int t = (int)(i % tps), v0 = t * rows, nrow = (vb - v0 < rows) ? (vb - v0) : rows;
+        const int64_t x = ((i / tps) * gridDim.x + blockIdx.x) * G + g;
+        const bool mine = g < G && x < Vc;
+        mbar_wait(&full[st], parity);
+        if (mine) {
+            const cplx<T> *sB = reinterpret_cast<const cplx<T> *>(smem_raw + (size_t)st * stage_bytes + (size_t)g * site_stage);
+            const cplx<T> *sF = reinterpret_cast<const cplx<T> *>(smem_raw + (size_t)st * stage_bytes + (size_t)g * site_stage + bytesB);
+            for (int k = 0; k < nrow; ++k) {
+                cplx<T> u[TT], w[TT];
+                gram_pipe_load<T, TT>(u, sB + k * nb + a0);
+                gram_pipe_load<T, TT>(w, sF + k * s + b0);
+#pragma unroll
+                for (int a = 0; a < TT; ++a)
+#pragma unroll
+                    for (int b = 0; b < TT; ++b) {
+                        if constexpr (sizeof(T) == 8) {       // complex128: the sums are double already, no runs
+                            accr[a][b] = fma(u[a].re, w[b].re, accr[a][b]); accr[a][b] = fma(u[a].im, w[b].im, accr[a][b]);
+                            acci[a][b] = fma(u[a].re, w[b].im, acci[a][b]); acci[a][b] = fma(-u[a].im, w[b].re, acci[a][b]);
+                        } else {
+                            cmac_conj(run[a][b], u[a], w[b]);
+                        }
+                    }
+            }
+        }
+        const bool last = t == tps - 1;
+        if (sizeof(T) == 4 && (++since_flush == flush_tiles || last)) {
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) {
+                    accr[a][b] += (Acc)run[a][b].re; acci[a][b] += (Acc)run[a][b].im;
+                    run[a][b].re = 0; run[a][b].im = 0;
+                }
+            since_flush = 0;
+        }
+        if (last) {                               // the site is complete: every thread writes its own 4 x 4 block
+            if (mine) {
+                cplx<T> *cx = Cc + x * (int64_t)nb * s;
+#pragma unroll
+                for (int a = 0; a < TT; ++a)
+#pragma unroll
+                    for (int b = 0; b < TT; ++b) cx[(a0 + a) * s + b0 + b] = {(T)accr[a][b], (T)acci[a][b]};
+            }
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int b = 0; b < TT; ++b) { accr[a][b] = 0; acci[a][b] = 0; }
+        }
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);          // this warp has read the stage
+        if (++st == kGramPipeStages) { st = 0; parity ^= 1u; }
+    }
+}
+
+// promote: F[x] = Basis[x] C[x], rows of the fine block times a small matrix.  Thread tile TR rows x 4 columns, lanes along the rows;
+// row tiles of Basis[x] go through cp.async into rows padded by LaPad (a warp's 16-byte loads of consecutive rows then meet
+// different banks), double buffered across the CTA's sites, C[x] rides along with a site's first tile; two contraction indices per
+// shared-memory load for complex64.  Sums over nbasis <= 64 terms in T.
+template <typename T, int TR>
+__global__ void __launch_bounds__(kLaThreads)
+block_promote_tiled_kernel(const cplx<T> *__restrict__ Bas, const cplx<T> *__restrict__ Cc, cplx<T> *__restrict__ F, int64_t Vc, int vb, int nb, int s,
+                           int RL)
+{
+    constexpr int W = 4, AV = 16 / (int)sizeof(cplx<T>);            // contraction indices per 16-byte load: 2 (complex64) or 1
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ld = nb + LaPad<T>::v, rows = RL * TR, ncg = s / W;
+    cplx<T> *sC0 = reinterpret_cast<cplx<T> *>(smem_raw);            // [2][nb * s]
+    cplx<T> *sB0 = sC0 + (size_t)2 * nb * s;                         // [2][rows * ld]
+    const int cg = threadIdx.x / RL, rl = threadIdx.x - cg * RL, c0 = cg * W;
+    const bool active = cg < ncg;
+    const int tps = (vb + rows - 1) / rows;
+    const int64_t my_sites = (int64_t)blockIdx.x < Vc ? (Vc - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const int64_t total = my_sites * tps;
+    auto stage = [&](int64_t i, int buf) {
+        const int64_t n = i / tps, x = blockIdx.x + n * gridDim.x;
+        const int t = (int)(i - n * tps), v0 = t * rows, nrow = (vb - v0 < rows) ? (vb - v0) : rows;
+        la_stage_rows_async(sB0 + (size_t)buf * rows * ld, Bas + x * (int64_t)vb * nb, v0, nrow, rows, nb, ld);
+        if (t == 0) {                             // the site's coarse block, 16-byte chunks (nb * s is a multiple of 16 elements)
+            cplx<T> *dst = sC0 + (size_t)(n & 1) * nb * s;
+            const cplx<T> *src = Cc + x * (int64_t)nb * s;
+            for (int e = threadIdx.x * AV; e < nb * s; e += kLaThreads * AV) cp_async_16(dst + e, src + e);
+        }
+    };
+    if (total > 0) stage(0, 0);
+    cp_async_commit();
+    int buf = 0;
+    for (int64_t i = 0; i < total; ++i, buf ^= 1) {
+        if (i + 1 < total) stage(i + 1, buf ^ 1);
+        cp_async_commit();
+        cp_async_wait<1>();
+        __syncthreads();
+        const int64_t n = i / tps, x = blockIdx.x + n * gridDim.x;
+        const int t = (int)(i - n * tps), v0 = t * rows, nrow = (vb - v0 < rows) ? (vb - v0) : rows;
+        if (active) {
+            const cplx<T> *sB = sB0 + (size_t)buf * rows * ld, *sC = sC0 + (size_t)(n & 1) * nb * s;
+            cplx<T> acc[TR][W];
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt)
+#pragma unroll
+                for (int c = 0; c < W; ++c) { acc[tt][c].re = 0; acc[tt][c].im = 0; }
+#pragma unroll 2
+            for (int a = 0; a < nb; a += AV) {
+                cplx<T> u[TR][AV], k[AV][W];
+#pragma unroll
+                for (int tt = 0; tt < TR; ++tt) gram_pipe_load<T, AV>(u[tt], sB + (rl + tt * RL) * ld + a);
+#pragma unroll
+                for (int j = 0; j < AV; ++j) gram_pipe_load<T, W>(k[j], sC + (a + j) * s + c0);
+#pragma unroll
+                for (int j = 0; j < AV; ++j)
+#pragma unroll
+                    for (int tt = 0; tt < TR; ++tt)
+#pragma unroll
+                        for (int c = 0; c < W; ++c) cmac(acc[tt][c], u[tt][j], k[j][c]);
+            }
+            cplx<T> *fx = F + (x * vb + v0) * (int64_t)s + c0;
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt) {
+                const int row = rl + tt * RL;
+                if (row < nrow) {
+#pragma unroll
+                    for (int c = 0; c < W; c += AV)
+                        *reinterpret_cast<float4 *>(fx + (int64_t)row * s + c) = *reinterpret_cast<const float4 *>(&acc[tt][c]);
+                }
+            }
+        }
+        __syncthreads();                          // the buffer may be restaged
+    }
+    cp_async_wait<0>();
 }
 
 // out = a*U + b*W elementwise (used for R = B - H X and copies)

@@ -1497,12 +1497,46 @@ static int transfer_launch(bool project, const void *Bas, const void *in, void *
     CMRHS_CUDA(cudaGetDevice(&dev));
     CMRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int grid = (int)(Vc < (int64_t)sms * 4 ? Vc : (int64_t)sms * 4);
-    if (project) {
+    const bool tuned = nb % 4 == 0 && s % 4 == 0 && (nb / 4) * (s / 4) <= kXferConsumers;       // 4 x 4 register tiles, 7 consumer warps
+    if (project && tuned) {
+        // G sites at a time (one group of (nb/4)(s/4) threads each, at most 8), stages of about 24 KB, a site's rows cut into equal tiles
+        const int ntile = (nb / 4) * (s / 4);
+        int G = kXferConsumers / ntile;
+        if (G > 8) G = 8;
+        if ((int64_t)G > Vc) G = (int)Vc;
+        int rows = (int)(24576 / ((size_t)G * (nb + s) * sizeof(cplx<T>)));
+        if (rows < 1) rows = 1;
+        if (rows > 32) rows = 32;
+        const int tps = (vb + rows - 1) / rows;
+        rows = (vb + tps - 1) / tps;
+        const int flush = rows >= 32 ? 1 : 32 / rows;                  // runs of <= 32 rows between flushes
+        const size_t smem = (size_t)kGramPipeStages * G * rows * (nb + s) * sizeof(cplx<T>) + 2 * kGramPipeStages * sizeof(uint64_t);
+        const int64_t nchunk = (Vc + G - 1) / G;
+        const int pgrid = (int)(nchunk < (int64_t)sms * 2 ? nchunk : (int64_t)sms * 2);
+        auto kern = block_project_pipe_kernel<T>;
+        CMRHS_SMEM_ATTR(kern, smem);
+        kern<<<pgrid, kLaThreads, smem, stream>>>((const cplx<T> *)Bas, (const cplx<T> *)in, (cplx<T> *)out, Vc, vb, nb, s, rows, G, flush);
+    } else if (project) {
         int rows = (int)(32768 / ((size_t)(nb + s) * sizeof(cplx<T>)));
         if (rows > vb) rows = vb;
         if (rows < 1) rows = 1;
         const size_t smem = (size_t)rows * (nb + s) * sizeof(cplx<T>);
         block_project_kernel<T><<<grid, kLaThreads, smem, stream>>>((const cplx<T> *)Bas, (const cplx<T> *)in, (cplx<T> *)out, Vc, vb, nb, s, rows);
+    } else if (tuned && s / 4 <= 16) {
+        // lanes along the rows: RL row lanes x s/4 column groups; TR = 2 rows per thread; two row tiles and two coarse blocks in shared memory
+        constexpr int TR = 2;
+        const int ncg = s / 4;
+        int RL = kLaThreads / ncg;
+        if (RL > 64) RL = 64;
+        const int ld = nb + LaPad<T>::v;
+        auto smem_of = [&](int rl) { return ((size_t)2 * nb * s + (size_t)2 * rl * TR * ld) * sizeof(cplx<T>); };
+        while (smem_of(RL) > 200 * 1024 && RL > 8) RL /= 2;          // (complex128 at nbasis 64: 64-row tiles)
+        const size_t smem = smem_of(RL);
+        const int per_sm = smem <= 110 * 1024 ? 2 : 1;
+        const int pgrid = (int)(Vc < (int64_t)sms * per_sm ? Vc : (int64_t)sms * per_sm);
+        auto kern = block_promote_tiled_kernel<T, TR>;
+        CMRHS_SMEM_ATTR(kern, smem);
+        kern<<<pgrid, kLaThreads, smem, stream>>>((const cplx<T> *)Bas, (const cplx<T> *)in, (cplx<T> *)out, Vc, vb, nb, s, RL);
     } else {
         int rows = 32;
         if (rows > vb) rows = vb;

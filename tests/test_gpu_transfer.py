@@ -25,6 +25,12 @@ def _rand(rng, dtype, *shape):
     (33, 37, 13, 5, "c64"),          # odd everything
     (3, 3072, 32, 16, "c64"),        # 4^4 x 12 fine degrees of freedom per block
     (1, 1, 1, 1, "c128"),
+    # the tuned kernels (nbasis and nrhs multiples of 4): 8 sites per CTA with a ragged last chunk and ragged row tiles; the widest
+    # promote tiling (16 column groups) with the generic project beside it; complex128 with 5 column groups
+    (37, 70, 8, 4, "c64"),
+    (5, 33, 64, 64, "c64"),
+    (11, 129, 48, 20, "c128"),
+    (300, 64, 32, 16, "c64"),
 ])
 def test_project_and_promote_match_oracle(Vc, vb, nb, s, dtype):
     rng = np.random.default_rng(Vc + vb + nb + s)
