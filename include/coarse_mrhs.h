@@ -180,15 +180,16 @@ int coarse_cheby_apply(coarse_op_t *op, const void *B_dev, void *X_dev, int32_t 
 /*
  * coarse_deflate -- multi-RHS deflation with n_ev eigenpairs of the operator (Eq. 7-10; "applied to
  * multiple right-hand sides"):  C = Vev^H B;  QBpar = Vev (C / lambda) = (sum_i |i><i| / lambda_i) b;
- * Bperp = B - Vev C = (1 - sum_i |i><i|) b.  Tall-skinny products, eigenvectors taken in chunks of min(64, nrhs_max)
+ * Bperp = B - Vev C = (1 - sum_i |i><i|) b.  Tall-skinny products, eigenvectors taken in chunks of 64
  * columns (chunk j projects the running Bperp: the columns are orthonormal): per chunk a deterministic two-stage reduction
- * (complex128 sums) and one pass over the chunk and the block.
+ * (complex128 sums) and one pass over the chunk and the block.  The FIRST call on a handle allocates the scratch for the
+ * 64 x nrhs_max coefficients and their per-CTA partials (about 1 MiB per right-hand side; freed by coarse_op_destroy).
  *   Vev_dev     : [V*nbasis][nev] device block of the operator's dtype, eigenvector index fastest, orthonormal columns
  *   lambda_host : [nev] HOST doubles, all > 0;  1 <= nev <= COARSE_MAX_NEV (the paper deflates with 192-1000 vectors)
  *   B_dev       : [V][nb][nrhs];  QBpar_dev, Bperp_dev: outputs of the same shape, QBpar != B, QBpar != Bperp (Bperp may alias B)
  * coarse_cheby_defl_solve -- the paper's stationary coarse solve  X = Defl(b_par) + P^Cheby(b_perp)  (Eq. 11-12), P as in
  * coarse_cheby_apply.  Asynchronous on `stream`; both use the handle's block-CG workspace.
- * Errors: COARSE_INVALID_ARG (NULL, aliasing, nev / nrhs / lambda / lo / hi / order out of range), launch errors.
+ * Errors: COARSE_INVALID_ARG (NULL, aliasing, nev / nrhs / lambda / lo / hi / order out of range), COARSE_OUT_OF_MEMORY (first call), launch errors.
  */
 int coarse_deflate(coarse_op_t *op, const void *Vev_dev, const double *lambda_host, int32_t nev, const void *B_dev,
                    void *QBpar_dev, void *Bperp_dev, int32_t nrhs, void *stream);

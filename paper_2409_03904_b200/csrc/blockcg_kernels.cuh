@@ -761,6 +761,172 @@ deflate_update_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *B
 }
 
 // ------------------------------------------------------------------------------------------------------
+// Register-tiled forms of the two deflation kernels for m and s multiples of 4 (the kernels above do one output element per
+// thread and convert every operand of every multiply-add: 6.8 TFLOP/s at nev 192, nrhs 16).  Same arithmetic contract.
+// stage 1: 4 x 4 sub-blocks of C = Vev^H B per thread, the threads left over split the rows (fixed-order reduction at the end);
+// products and sums in double as above, but 16 conversions per 16 complex multiply-adds instead of 64.
+// ------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(kLaThreads)
+rgram_tiled_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *__restrict__ B, int64_t n, int m, int s, int rows_per_tile,
+                   zdouble *__restrict__ partial)
+{
+    constexpr int TT = 4;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *sV = reinterpret_cast<cplx<T> *>(smem_raw);
+    cplx<T> *sB = sV + (size_t)rows_per_tile * m;
+    const int ntb = s / TT, ntile = (m / TT) * ntb, RG = kLaThreads / ntile;
+    const int tile = threadIdx.x % ntile, rg = threadIdx.x / ntile;
+    const bool active = rg < RG;
+    const int a0 = (tile / ntb) * TT, b0 = (tile % ntb) * TT;
+    double accr[TT][TT], acci[TT][TT];
+#pragma unroll
+    for (int a = 0; a < TT; ++a)
+#pragma unroll
+        for (int b = 0; b < TT; ++b) { accr[a][b] = 0.0; acci[a][b] = 0.0; }
+    const int64_t chunk = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t r_begin = blockIdx.x * chunk;
+    const int64_t r_end = (r_begin + chunk < n) ? r_begin + chunk : n;
+    const int cpr = m / TT;                       // 4-element pieces per row of the eigenvector chunk
+    for (int64_t r0 = r_begin; r0 < r_end; r0 += rows_per_tile) {
+        const int nrow = (int)((r_end - r0 < rows_per_tile) ? (r_end - r0) : rows_per_tile);
+        __syncthreads();
+        for (int e = threadIdx.x; e < nrow * cpr; e += kLaThreads) {
+            const int k = e / cpr, j = (e - k * cpr) * TT;
+            cplx<T> v[TT];
+            gram_pipe_load<T, TT>(v, Vev + (r0 + k) * ldv + j);
+#pragma unroll
+            for (int u = 0; u < TT; ++u) sV[k * m + j + u] = v[u];
+        }
+        for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) sB[e] = B[r0 * s + e];
+        __syncthreads();
+        if (active) {
+            for (int k = rg; k < nrow; k += RG) {
+                cplx<T> v[TT], b[TT];
+                gram_pipe_load<T, TT>(v, sV + k * m + a0);
+                gram_pipe_load<T, TT>(b, sB + k * s + b0);
+                double vr[TT], vi[TT], br[TT], bi[TT];
+#pragma unroll
+                for (int u = 0; u < TT; ++u) { vr[u] = (double)v[u].re; vi[u] = (double)v[u].im; br[u] = (double)b[u].re; bi[u] = (double)b[u].im; }
+#pragma unroll
+                for (int a = 0; a < TT; ++a)
+#pragma unroll
+                    for (int c = 0; c < TT; ++c) {            // conj(v) * b
+                        accr[a][c] += vr[a] * br[c] + vi[a] * bi[c];
+                        acci[a][c] += vr[a] * bi[c] - vi[a] * br[c];
+                    }
+            }
+        }
+    }
+    zdouble *out = partial + (size_t)blockIdx.x * m * s;
+    if (RG == 1) {                                // one thread per sub-block: no reduction
+#pragma unroll
+        for (int a = 0; a < TT; ++a)
+#pragma unroll
+            for (int c = 0; c < TT; ++c) out[(a0 + a) * s + b0 + c] = {accr[a][c], acci[a][c]};
+        return;
+    }
+    // row groups in a fixed order (0, 1, 2, ...) through shared memory (the launcher sizes it for m * s complex doubles)
+    __syncthreads();
+    double *red = reinterpret_cast<double *>(smem_raw);
+    for (int g = 0; g < RG; ++g) {
+        if (active && rg == g) {
+#pragma unroll
+            for (int a = 0; a < TT; ++a)
+#pragma unroll
+                for (int c = 0; c < TT; ++c) {
+                    const int e = (a0 + a) * s + b0 + c;
+                    if (g == 0) { red[2 * e] = accr[a][c]; red[2 * e + 1] = acci[a][c]; }
+                    else { red[2 * e] += accr[a][c]; red[2 * e + 1] += acci[a][c]; }
+                }
+        }
+        __syncthreads();
+    }
+    for (int e = threadIdx.x; e < m * s; e += kLaThreads) out[e] = {red[2 * e], red[2 * e + 1]};
+}
+
+// stage 2: TR rows x 4 columns of both products per thread, lanes along the rows (rows of the chunk padded by LaPad in shared
+// memory), two contraction indices per 16-byte load for complex64.
+template <typename T, int TR>
+__global__ void __launch_bounds__(kLaThreads)
+deflate_update_tiled_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *B, const zdouble *__restrict__ Cm, const DeflLambda lam,
+                            cplx<T> *__restrict__ QBpar, cplx<T> *Bperp, int64_t n, int m, int s, int RL, int accumulate)
+{
+    constexpr int W = 4, AV = 16 / (int)sizeof(cplx<T>);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ld = m + LaPad<T>::v, rows = RL * TR, ncg = s / W;
+    cplx<T> *sC = reinterpret_cast<cplx<T> *>(smem_raw);          // [m][s]   <i|b>
+    cplx<T> *sCl = sC + m * s;                                     // [m][s]   <i|b> / lambda_i
+    cplx<T> *sV = sCl + m * s;                                     // [rows][ld]
+    for (int e = threadIdx.x; e < m * s; e += kLaThreads) {
+        const double il = lam.inv[e / s];
+        sC[e].re = (T)Cm[e].re; sC[e].im = (T)Cm[e].im;
+        sCl[e].re = (T)(Cm[e].re * il); sCl[e].im = (T)(Cm[e].im * il);
+    }
+    const int cg = threadIdx.x / RL, rl = threadIdx.x - cg * RL, c0 = cg * W;
+    const bool active = cg < ncg;
+    const int cpr = m / W;
+    const int64_t ntiles = (n + rows - 1) / rows;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t r0 = t * rows;
+        const int nrow = (int)((n - r0 < rows) ? (n - r0) : rows);
+        __syncthreads();
+        for (int e = threadIdx.x; e < rows * cpr; e += kLaThreads) {
+            const int k = e / cpr, j = (e - k * cpr) * W;
+            cplx<T> v[W];
+            if (k < nrow) gram_pipe_load<T, W>(v, Vev + (r0 + k) * ldv + j);
+            else {
+#pragma unroll
+                for (int u = 0; u < W; ++u) v[u] = {0, 0};
+            }
+#pragma unroll
+            for (int u = 0; u < W; ++u) sV[k * ld + j + u] = v[u];
+        }
+        __syncthreads();
+        if (active) {
+            cplx<T> par[TR][W], q[TR][W];
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt)
+#pragma unroll
+                for (int c = 0; c < W; ++c) { par[tt][c].re = 0; par[tt][c].im = 0; q[tt][c].re = 0; q[tt][c].im = 0; }
+            for (int i = 0; i < m; i += AV) {
+                cplx<T> v[TR][AV], kc[AV][W], kl[AV][W];
+#pragma unroll
+                for (int tt = 0; tt < TR; ++tt) gram_pipe_load<T, AV>(v[tt], sV + (rl + tt * RL) * ld + i);
+#pragma unroll
+                for (int j = 0; j < AV; ++j) { gram_pipe_load<T, W>(kc[j], sC + (i + j) * s + c0); gram_pipe_load<T, W>(kl[j], sCl + (i + j) * s + c0); }
+#pragma unroll
+                for (int j = 0; j < AV; ++j)
+#pragma unroll
+                    for (int tt = 0; tt < TR; ++tt)
+#pragma unroll
+                        for (int c = 0; c < W; ++c) { cmac(par[tt][c], v[tt][j], kc[j][c]); cmac(q[tt][c], v[tt][j], kl[j][c]); }
+            }
+#pragma unroll
+            for (int tt = 0; tt < TR; ++tt) {
+                const int row = rl + tt * RL;
+                if (row < nrow) {
+                    const int64_t e0 = (r0 + row) * s + c0;
+                    cplx<T> b[W], q0[W];
+                    gram_pipe_load<T, W>(b, B + e0);
+                    if (accumulate) gram_pipe_load<T, W>(q0, QBpar + e0);
+#pragma unroll
+                    for (int c = 0; c < W; ++c) {
+                        if (accumulate) { q[tt][c].re += q0[c].re; q[tt][c].im += q0[c].im; }
+                        b[c].re -= par[tt][c].re; b[c].im -= par[tt][c].im;
+                    }
+#pragma unroll
+                    for (int c = 0; c < W; c += AV) {
+                        *reinterpret_cast<float4 *>(QBpar + e0 + c) = *reinterpret_cast<const float4 *>(&q[tt][c]);
+                        *reinterpret_cast<float4 *>(Bperp + e0 + c) = *reinterpret_cast<const float4 *>(&b[c]);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
 // Stacked single-Krylov CG: one alpha / beta per iteration from Frobenius inner products over the
 // whole block.  Scalars live on the device (sc: 0 rho, 1 alpha, 2 beta, 3 ||B||_F^2, 4 stop = sqrt(rho / ||B||^2)).
 // Reductions: fixed partition over CTAs, fixed order inside (shuffle tree, then warp 0), partials summed by one warp.

@@ -138,6 +138,7 @@ struct coarse_op {
     void *pblk[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};           // q, Q, D, z, Z of pblock_cg_solve (allocated on first use)
     void *blk[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // Q, D, Z, T, and two staging blocks for the *_host entry points
     zdouble *gram_partial = nullptr;
+    zdouble *defl_partial = nullptr, *defl_C = nullptr;      // deflation: 64 x nrhs_max coefficients and their per-CTA partials (allocated by the first coarse_deflate)
     int gram_blocks = 0;
     zdouble *small = nullptr;    // 6 s x s matrices
     double *dscal = nullptr;     // bnorm[64] relres[64] stop[2] truerel[64]
@@ -224,6 +225,8 @@ extern "C" int coarse_op_destroy(coarse_op_t *op)
     cudaFree(op->nbr);
     for (void *b : op->blk) cudaFree(b);
     cudaFree(op->gram_partial);
+    cudaFree(op->defl_partial);
+    cudaFree(op->defl_C);
     cudaFree(op->small);
     cudaFree(op->dscal);
     cudaFree(op->dinfo);
@@ -1228,12 +1231,17 @@ template <typename T>
 static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, int nev, const void *B, void *QBpar, void *Bperp, int s,
                         cudaStream_t stream)
 {
-    // The eigenvectors are taken in chunks of m <= min(64, nrhs_max) columns (the paper deflates with several hundred,
-    // PAPER.md:118, 196): chunk j projects the running b_perp (orthonormal vectors: <i|b_perp> = <i|b> for the vectors still to
-    // come), so one pass over a chunk and the block per stage, and b_perp may alias B.
+    // The eigenvectors are taken in chunks of m <= 64 columns (the paper deflates with several hundred): chunk j
+    // projects the running b_perp (orthonormal vectors: <i|b_perp> = <i|b> for the vectors still to come), so one pass over a chunk
+    // and the block per stage, and b_perp may alias B.  Every chunk costs five passes over the block: wide chunks whatever nrhs_max is
+    // (chunks of nrhs_max = 16 vectors: 9.5 ms at nev 192; the scratch for 64 x nrhs_max coefficients comes with the first call).
     const int64_t n = op->dims.V * op->nb;
-    zdouble *Cm = small_view(op).G;                     // m x s <= 64 x 64 complex128
-    const int mc = op->nrhs_max < COARSE_MAX_NRHS ? op->nrhs_max : COARSE_MAX_NRHS;
+    const int mc = COARSE_MAX_NRHS;
+    if (!op->defl_partial) {
+        CMRHS_STEP(alloc_dev(op, (void **)&op->defl_partial, (size_t)op->gram_blocks * mc * op->nrhs_max * sizeof(zdouble)));
+        CMRHS_STEP(alloc_dev(op, (void **)&op->defl_C, (size_t)mc * op->nrhs_max * sizeof(zdouble)));
+    }
+    zdouble *Cm = op->defl_C;                           // m x s <= 64 x nrhs_max complex128
     for (int j0 = 0; j0 < nev; j0 += mc) {
         const int m = nev - j0 < mc ? nev - j0 : mc;
         const cplx<T> *Vj = (const cplx<T> *)Vev + j0;
@@ -1243,21 +1251,40 @@ static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, in
         if (rows < 1) rows = 1;
         int blocks = op->gram_blocks;
         if ((int64_t)blocks > ceil_div(n, rows)) blocks = (int)ceil_div(n, rows);
-        const size_t smem1 = (size_t)rows * (m + s) * sizeof(cplx<T>);
-        rgram_partial_kernel<T><<<blocks, kLaThreads, smem1, stream>>>(Vj, nev, Bin, n, m, s, rows, op->gram_partial);
+        size_t smem1 = (size_t)rows * (m + s) * sizeof(cplx<T>);
+        // register-tiled kernels: m and s multiples of 4, rows of the eigenvector block 16-byte aligned
+        const bool tiled = m % 4 == 0 && s % 4 == 0 && (m / 4) * (s / 4) <= kLaThreads && (sizeof(T) == 8 || nev % 2 == 0);
+        if (tiled) {
+            if ((m / 4) * (s / 4) * 2 <= kLaThreads && smem1 < (size_t)m * s * sizeof(zdouble)) smem1 = (size_t)m * s * sizeof(zdouble);   // (several row groups: <= 32 KB)
+            rgram_tiled_kernel<T><<<blocks, kLaThreads, smem1, stream>>>(Vj, nev, Bin, n, m, s, rows, op->defl_partial);
+        } else {
+            rgram_partial_kernel<T><<<blocks, kLaThreads, smem1, stream>>>(Vj, nev, Bin, n, m, s, rows, op->defl_partial);
+        }
         CMRHS_LAUNCH_CHECK();
-        gram_reduce_kernel<<<(m * s * 32 + 127) / 128, 128, 0, stream>>>(op->gram_partial, blocks, m * s, Cm);
+        gram_reduce_kernel<<<(m * s * 32 + 127) / 128, 128, 0, stream>>>(op->defl_partial, blocks, m * s, Cm);
         CMRHS_LAUNCH_CHECK();
         // stage 2: Qb_par (+)= V_j (C / lambda), b_perp -= V_j C
         DeflLambda lam;
         for (int i = 0; i < COARSE_MAX_NRHS; ++i) lam.inv[i] = i < m ? 1.0 / lambda[j0 + i] : 0.0;
-        const int rows2 = 64;
-        const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);
-        auto kern = deflate_update_kernel<T>;
-        CMRHS_SMEM_ATTR(kern, smem2);
-        const int64_t ntiles = ceil_div(n, rows2);
-        const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
-        kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, rows2, j0 > 0 ? 1 : 0);
+        if (tiled && s / 4 <= 16) {
+            constexpr int TR = 2;
+            int RL = kLaThreads / (s / 4);
+            if (RL > 64) RL = 64;
+            const size_t smem2 = ((size_t)2 * m * s + (size_t)RL * TR * (m + LaPad<T>::v)) * sizeof(cplx<T>);
+            auto kern = deflate_update_tiled_kernel<T, TR>;
+            CMRHS_SMEM_ATTR(kern, smem2);
+            const int64_t ntiles = ceil_div(n, (int64_t)RL * TR);
+            const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
+            kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, RL, j0 > 0 ? 1 : 0);
+        } else {
+            const int rows2 = 64;
+            const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);
+            auto kern = deflate_update_kernel<T>;
+            CMRHS_SMEM_ATTR(kern, smem2);
+            const int64_t ntiles = ceil_div(n, rows2);
+            const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
+            kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, rows2, j0 > 0 ? 1 : 0);
+        }
         CMRHS_LAUNCH_CHECK();
     }
     return COARSE_OK;
