@@ -256,6 +256,51 @@ def time_apply(torch, op, X, Y, reps=20, warm=3):
     return ev[0].elapsed_time(ev[1]) / reps
 
 
+def next_rows_point(torch, cm, op, dims, nb, s, c, B, peaks):
+    """SURVEY.md section 8(f) NEXT rows, measured (each is parity-tested in tests/): block project / promote at Table 6's shape
+    (PAPER.md:570-571), multi-RHS deflation with 192 eigenvectors, the stacked and the preconditioned block solve on
+    the bench operator.  Synthetic operands (random basis / eigenvector blocks: timing does not depend on their values)."""
+    def timed(f, reps=10, warm=2):
+        for _ in range(warm):
+            f()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(reps):
+            f()
+        ev[1].record()
+        torch.cuda.synchronize()
+        return ev[0].elapsed_time(ev[1]) / reps
+    rows = {}
+    g = torch.Generator(device="cuda")
+    g.manual_seed(20240903)
+    Vc, vb, pnb, ps = 4096, 256, 64, 12
+    Bas = torch.view_as_complex(torch.randn((Vc, vb, pnb, 2), device="cuda", generator=g))
+    F = torch.view_as_complex(torch.randn((Vc, vb, ps, 2), device="cuda", generator=g))
+    Cc = cm.block_project(Bas, F)
+    by, fl = 8.0 * (Vc * vb * pnb + Vc * vb * ps + Vc * pnb * ps), 8.0 * Vc * vb * pnb * ps
+    roof = min(peaks["hbm_gbs"] * 1e9 * fl / by, alu_peak_tflops("c64", peaks) * 1e12)
+    for name, f in (("project", lambda: cm.block_project(Bas, F)), ("promote", lambda: cm.block_promote(Bas, Cc))):
+        ms = timed(f)
+        rows[name] = dict(shape="Vc 4096 x V_block 256 x nbasis 64 x nrhs 12, complex64 (Table 6)", ms=ms, gbs=by / ms / 1e6, tflops=fl / ms / 1e9,
+                          frac_of_min_ffma_hbm=fl / (ms * 1e-3) / roof)
+    del Bas, F, Cc
+    n, nev = int(B.numel() // s), 192
+    Vev = torch.view_as_complex(torch.randn((n, nev, 2), device="cuda", generator=g)) / float(np.sqrt(n))
+    lam = [1.0 + i for i in range(nev)]
+    ms = timed(lambda: op.deflate(Vev, lam, B), reps=5)
+    rows["deflate"] = dict(shape=f"n {n} x nev {nev} x nrhs {s}, complex64", ms=ms, tflops=2 * 8.0 * n * nev * s / ms / 1e9,
+                           gbs=8.0 * (2.0 * n * nev + 15.0 * n * s) / ms / 1e6)
+    del Vev
+    op.stacked_cg(B, tol=1e-6, maxiter=100)
+    r = op.stacked_cg(B, tol=1e-6, maxiter=100)
+    rows["stacked_cg"] = dict(seconds=r["seconds"], iterations=r["iterations"], status=r["status"], max_true_rel_res=max(r["rel_res_true"]))
+    op.pblock_cg(B, lo=c - 12.0, hi=c + 12.0, order=8, tol=1e-6, maxiter=50)
+    r = op.pblock_cg(B, lo=c - 12.0, hi=c + 12.0, order=8, tol=1e-6, maxiter=50)
+    rows["pblock_cg_cheby8"] = dict(seconds=r["seconds"], iterations=r["iterations"], status=r["status"], max_true_rel_res=max(r["rel_res_true"]))
+    return rows
+
+
 def per_config_point(torch, cm, index, peaks):
     """One time-boxed apply + BlockCGrQ solve of another BASELINE.json configuration (parity-tested in tests/; reported here so
     that every figure quoted in DESIGN.md section 5 comes out of a tracked command)."""
@@ -499,6 +544,15 @@ def run_ours(args, cfg):
         cpu = dict(value=len(dts) * step_flops(len(sites), nb, s) / dt / 1e12, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
                    sample=f"{len(dts)} steps on {len(sites)} of {V} sites (operator bits read back from the device), {dt:.1f} s in total")
 
+    # ---- SURVEY.md 8(f) NEXT rows on the same operator (never fatal: a failure is recorded in the line) ----------------------
+    next_rows = None
+    if args.next_rows and dtype == "c64":
+        try:
+            next_rows = next_rows_point(torch, cm, op, dims, nb, s, c, B, peaks)
+        except Exception as e:                                               # noqa: BLE001
+            next_rows = dict(error=f"{type(e).__name__}: {e}")
+            print(f"bench.py: WARNING next_rows failed: {next_rows['error']}", file=sys.stderr)
+
     # ---- the other BASELINE.json configurations (parity cases; one time-boxed apply + solve each) --------------------------
     op.close()
     del B, X, Xs
@@ -524,7 +578,7 @@ def run_ours(args, cfg):
                             operator_bytes=81 * V * nb * nb * esize, parallelism="replicas only" if world > 1 else "1 GPU",
                             l2="inputs (27.5 GB operator) larger than L2; no flush", diagonal_shift_c=c),
                 clocks=clk, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,
-                sweep=sweep, block_cg_solve=bcg, cheby_solve=cheb, per_config=per_config,
+                sweep=sweep, block_cg_solve=bcg, cheby_solve=cheb, per_config=per_config, next_rows=next_rows,
                 peaks={k: v for k, v in peaks.items() if k != "source"}, peaks_source=peaks["source"],
                 step_breakdown=dict(apply_ms=a_ms, other_ms=ms / K - a_ms, final_recursive_rel_res=max(out["rel_res_recursive"])))
     print(json.dumps(line))
@@ -544,6 +598,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3: the Nrhs-sweep workload)")
     ap.add_argument("--no-sweep", dest="sweep", action="store_false")
     ap.add_argument("--no-per-config", dest="per_config", action="store_false", help="skip the apply + solve of the other BASELINE configurations")
+    ap.add_argument("--no-next-rows", dest="next_rows", action="store_false", help="skip the measurements of the SURVEY 8(f) NEXT rows")
     ap.add_argument("--peaks", action="store_true", help="only measure the roofline denominators of this device and print them as JSON")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cheby-order", type=int, default=120, help="order of the Chebyshev coarse solve timed beside block CG (0: skip)")
