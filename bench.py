@@ -124,7 +124,10 @@ def roofline_tflops(V, nb, s, dtype, peaks, kernel="", sustained=True):
 
 # ---- clocks during the timed region (B200_PROFILING.md "clocks line") ----------------------------------------
 class ClockSampler:
-    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi in a loop beside the run.  It is started well BEFORE the timed region (its first line takes a few hundred ms, the
+    timed region of the default run is under 200 ms) and every line carries a timestamp: stop(t0, t1) keeps the samples taken inside
+    the timed region (host clock of the same box)."""
+    FIELDS = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, gpu_index: int):
@@ -135,37 +138,46 @@ class ClockSampler:
             fd, self.path = tempfile.mkstemp(suffix=".csv")
             os.close(fd)
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """t0, t1: datetime.now() at the two ends of the timed region (None: every sample counts)"""
+        from datetime import datetime, timedelta
         out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
         if self.proc is None:
             return out
+        time.sleep(0.05)                                                   # let the sample of the last instants be written
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
-        sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = []
         for line in open(self.path):
             f = [x.strip() for x in line.split(",")]
             if len(f) < 9:
                 continue
             try:
-                sm.append(float(f[1]))
-                mx.append(float(f[2]))
+                ts = datetime.strptime(f[0], "%Y/%m/%d %H:%M:%S.%f")
+                rows.append((ts, float(f[1]), float(f[2]), {n for n, v in zip(names, f[5:9]) if v.lower().startswith("active")}))
             except ValueError:
                 continue
-            for name, val in zip(names, f[5:9]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
         os.unlink(self.path)
-        if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), reasons=sorted(reasons), samples=len(sm))
+        window = "timed region"
+        pick = rows
+        if t0 is not None and t1 is not None:
+            pick = [r for r in rows if t0 <= r[0] <= t1]
+            if not pick:                                                   # (a query takes 10-20 ms: the nearest samples around a very short region)
+                pick = [r for r in rows if t0 - timedelta(seconds=0.1) <= r[0] <= t1 + timedelta(seconds=0.1)]
+                window = "timed region +- 0.1 s"
+        if pick:
+            reasons = set().union(*[r[3] for r in pick])
+            out.update(sm_mhz=float(np.median([r[1] for r in pick])), sm_max_mhz=float(np.max([r[2] for r in pick])), reasons=sorted(reasons),
+                       samples=len(pick), window=window)
         return out
 
 
@@ -370,6 +382,9 @@ def run_ours(args, cfg):
     K, W = args.steps, args.warmup
     # replicas only: every rank holds the whole operator and iterates on its own block
     seed = cfg["seed"]
+    clocks = ClockSampler(local_rank)                               # nvidia-smi beside the run from here on: its lines are time-stamped
+    if rank == 0:
+        clocks.start()
     A, c = cm.fill_synthetic(dims, nb, tdt, seed, cfg["factor"])
     nrhs_max = max(SWEEP) if (args.sweep and rank == 0) else s
     # nbasis 32 with wide blocks on the handle: keep both split-FP16 layouts (the kernel with the X operand in tensor memory is the
@@ -400,22 +415,22 @@ def run_ours(args, cfg):
 
     op.block_cg_step(W)                                             # W untimed warm-up steps
     barrier()
-    clocks = ClockSampler(local_rank)
-    if rank == 0:
-        clocks.start()
     op.profile(True)
     l0 = cm.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    from datetime import datetime
+    t_begin = datetime.now()
     e0.record()
     op.block_cg_step(K)                                             # exactly K timed steps
     e1.record()
     barrier()
+    t_end = datetime.now()
     launches = cm.launch_count() - l0
     ms = e0.elapsed_time(e1)
     apply_ms = op.profile_read()
     op.profile(False)
-    clk = clocks.stop() if rank == 0 else None
+    clk = clocks.stop(t_begin, t_end) if rank == 0 else None
     out = op.block_cg_end()
     assert out["status"] == 0, "block CG broke down inside the timed region"
     ms = max_over_ranks(ms, world, "cuda")
