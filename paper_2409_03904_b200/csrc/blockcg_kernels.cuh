@@ -764,10 +764,10 @@ deflate_update_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *B
 // Register-tiled forms of the two deflation kernels for m and s multiples of 4 (the kernels above do one output element per
 // thread and convert every operand of every multiply-add: 6.8 TFLOP/s at nev 192, nrhs 16).  Same arithmetic contract.
 // stage 1: 4 x 4 sub-blocks of C = Vev^H B per thread, the threads left over split the rows (fixed-order reduction at the end);
-// products and sums in double as above, but 16 conversions per 16 complex multiply-adds instead of 64.
+// complex128: products and sums in double as above; complex64: products and one tile's run per thread (<= 32 terms) in float, sums in double.
 // ------------------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(kLaThreads)
+__global__ void __launch_bounds__(kLaThreads, 2)
 rgram_tiled_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *__restrict__ B, int64_t n, int m, int s, int rows_per_tile,
                    zdouble *__restrict__ partial)
 {
@@ -801,20 +801,40 @@ rgram_tiled_kernel(const cplx<T> *__restrict__ Vev, int ldv, const cplx<T> *__re
         for (int e = threadIdx.x; e < nrow * s; e += kLaThreads) sB[e] = B[r0 * s + e];
         __syncthreads();
         if (active) {
-            for (int k = rg; k < nrow; k += RG) {
-                cplx<T> v[TT], b[TT];
-                gram_pipe_load<T, TT>(v, sV + k * m + a0);
-                gram_pipe_load<T, TT>(b, sB + k * s + b0);
-                double vr[TT], vi[TT], br[TT], bi[TT];
-#pragma unroll
-                for (int u = 0; u < TT; ++u) { vr[u] = (double)v[u].re; vi[u] = (double)v[u].im; br[u] = (double)b[u].re; bi[u] = (double)b[u].im; }
+            if constexpr (sizeof(T) == 4) {
+                // complex64: products and this tile's run (rows_per_tile / RG <= 32 terms) in float, the run added to the double sums --
+                // the contract of the Gram kernels (gram_partial_kernel), at the FP32 rate and without a conversion per operand
+                cplx<T> run[TT][TT];
 #pragma unroll
                 for (int a = 0; a < TT; ++a)
 #pragma unroll
-                    for (int c = 0; c < TT; ++c) {            // conj(v) * b
-                        accr[a][c] += vr[a] * br[c] + vi[a] * bi[c];
-                        acci[a][c] += vr[a] * bi[c] - vi[a] * br[c];
-                    }
+                    for (int c = 0; c < TT; ++c) { run[a][c].re = 0; run[a][c].im = 0; }
+                for (int k = rg; k < nrow; k += RG) {
+                    cplx<T> v[TT], b[TT];
+                    gram_pipe_load<T, TT>(v, sV + k * m + a0);
+                    gram_pipe_load<T, TT>(b, sB + k * s + b0);
+#pragma unroll
+                    for (int a = 0; a < TT; ++a)
+#pragma unroll
+                        for (int c = 0; c < TT; ++c) cmac_conj(run[a][c], v[a], b[c]);
+                }
+#pragma unroll
+                for (int a = 0; a < TT; ++a)
+#pragma unroll
+                    for (int c = 0; c < TT; ++c) { accr[a][c] += (double)run[a][c].re; acci[a][c] += (double)run[a][c].im; }
+            } else {
+                for (int k = rg; k < nrow; k += RG) {
+                    cplx<T> v[TT], b[TT];
+                    gram_pipe_load<T, TT>(v, sV + k * m + a0);
+                    gram_pipe_load<T, TT>(b, sB + k * s + b0);
+#pragma unroll
+                    for (int a = 0; a < TT; ++a)
+#pragma unroll
+                        for (int c = 0; c < TT; ++c) {            // conj(v) * b
+                            accr[a][c] += (double)v[a].re * (double)b[c].re + (double)v[a].im * (double)b[c].im;
+                            acci[a][c] += (double)v[a].re * (double)b[c].im - (double)v[a].im * (double)b[c].re;
+                        }
+                }
             }
         }
     }
