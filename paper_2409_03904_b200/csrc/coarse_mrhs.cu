@@ -1267,15 +1267,21 @@ static int deflate_impl(coarse_op *op, const void *Vev, const double *lambda, in
         DeflLambda lam;
         for (int i = 0; i < COARSE_MAX_NRHS; ++i) lam.inv[i] = i < m ? 1.0 / lambda[j0 + i] : 0.0;
         if (tiled && s / 4 <= 16) {
-            constexpr int TR = 2;
             int RL = kLaThreads / (s / 4);
             if (RL > 64) RL = 64;
+            const int TR = (s >= 32 && sizeof(T) == 4) ? 4 : 2;              // wide blocks have few row lanes: more rows per thread
             const size_t smem2 = ((size_t)2 * m * s + (size_t)RL * TR * (m + LaPad<T>::v)) * sizeof(cplx<T>);
-            auto kern = deflate_update_tiled_kernel<T, TR>;
-            CMRHS_SMEM_ATTR(kern, smem2);
             const int64_t ntiles = ceil_div(n, (int64_t)RL * TR);
             const int grid = (int)(ntiles < (int64_t)op->num_sms * 4 ? ntiles : (int64_t)op->num_sms * 4);
-            kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, RL, j0 > 0 ? 1 : 0);
+            if (TR == 4) {
+                auto kern = deflate_update_tiled_kernel<T, 4>;
+                CMRHS_SMEM_ATTR(kern, smem2);
+                kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, RL, j0 > 0 ? 1 : 0);
+            } else {
+                auto kern = deflate_update_tiled_kernel<T, 2>;
+                CMRHS_SMEM_ATTR(kern, smem2);
+                kern<<<grid, kLaThreads, smem2, stream>>>(Vj, nev, Bin, Cm, lam, (cplx<T> *)QBpar, (cplx<T> *)Bperp, n, m, s, RL, j0 > 0 ? 1 : 0);
+            }
         } else {
             const int rows2 = 64;
             const size_t smem2 = ((size_t)2 * m * s + (size_t)rows2 * m) * sizeof(cplx<T>);

@@ -139,7 +139,9 @@ def test_deflate_matches_oracle(dims, nb, s, nev, dtype):
 
 @pytest.mark.parametrize("dims,nb,s,nev,nrhs_max,dtype", [((2, 2, 2, 4), 16, 12, 192, 12, "c128"),      # 16 chunks of 12 eigenvectors
                                                           ((4, 2, 2, 4), 8, 16, 200, 64, "c64"),         # chunks 64, 64, 64, 8
-                                                          ((2, 2, 2, 4), 16, 5, 65, 64, "c128")])        # 64 + 1
+                                                          ((2, 2, 2, 4), 16, 5, 65, 64, "c128"),         # 64 + 1
+                                                          ((2, 2, 2, 4), 16, 32, 128, 32, "c64"),        # wide blocks: 4 rows per thread in stage 2
+                                                          ((2, 2, 2, 4), 16, 64, 96, 64, "c64")])        # chunks 64, 32 at width 64
 def test_deflate_with_hundreds_of_eigenvectors(dims, nb, s, nev, nrhs_max, dtype):
     # the paper deflates the coarse solve with "several hundred" eigenvectors (192 in its production runs, up to 1000 computed:
     # PAPER.md:118, 196, 384-388): more than one chunk of <= min(64, nrhs_max) vectors, in place as well (Bperp aliases B)
